@@ -1,0 +1,94 @@
+/* ORACLE — TEST INFRASTRUCTURE ONLY.
+ *
+ * oracle_ref.h — C ABI of the plain CPU oracle (HOST pointers everywhere, suffix _ref).
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+ * may load this library.  The product (paper_2211_14056_b200/, include/madme.h) never does,
+ * and the two share no source.
+ *
+ * What each function computes, and from where:
+ *   me_eval_ref        tier 1: diagram-by-diagram |M|^2 (SURVEY.md §8(c) tier 1; north_star)
+ *   me_eval_def_ref    tier 0: the definition — colour-dressed recursion + brute-force sums
+ *   philox/rambo/cuts
+ *   vegas_*            SURVEY.md §8(c) G6, G7 (Lepage's Vegas)
+ * Parity status: every function below is pinned by tests/test_oracle_*.py (closed forms,
+ * Ward identity, Lorentz/basis/Bose invariance, tier 0 <-> tier 1, RAMBO identities) except:
+ *   - the Philox BIT PATTERN: pinned against a library Philox4x32-10 where one is importable
+ *     (see tests/test_oracle_phase_space.py); otherwise "parity unpinned" beyond CPU == GPU.
+ *   - the Vegas grid-update details (alpha = 1.5, 3-point smoothing): a READING,
+ *     pinned only by closed-form integrals and fixed-point/quantile properties.
+ *   - sigma(gg -> ttbar gg): "parity unpinned" against the outside world (no published value).
+ */
+#ifndef ORACLE_REF_H
+#define ORACLE_REF_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct me_handle_ref me_handle_ref;
+#ifndef ME_PARAMS_REF_DEFINED
+#define ME_PARAMS_REF_DEFINED
+typedef struct {
+  double alpha_s, alpha_em, m_top, w_top;
+  double ptj_min, dr_min;
+} me_params_ref;
+#endif
+typedef struct {
+  int n_dim, n_bins;
+  double* edges; /* host [n_dim][n_bins+1] */
+  double alpha;
+  uint64_t seed;
+  int iteration;
+  int ps_mode; /* 0 classic RAMBO (4n uniforms), 1 diet (3n-4) */
+} vegas_grid_ref;
+typedef struct {
+  double integral, variance;
+  double sum_w, sum_w2;
+  long long n_pass;
+} vegas_result_ref;
+
+void oracle_set_threads_ref(int n);
+int oracle_get_threads_ref(void);
+
+/* --- matrix elements --- */
+int me_init_ref(const char* process, const me_params_ref* p, me_handle_ref** out);
+void me_free_ref(me_handle_ref* h);
+int me_n_external_ref(const me_handle_ref* h);
+int me_n_final_ref(const me_handle_ref* h);
+int me_eval_ref(me_handle_ref* h, const double* momenta, double* me2, long long n_ev);     /* tier 1 */
+int me_eval_def_ref(me_handle_ref* h, const double* momenta, double* me2, long long n_ev); /* tier 0 */
+/* test hooks */
+int me_set_basis_ref(me_handle_ref* h, int spin_basis, int pol_basis);
+int me_set_ward_leg_ref(me_handle_ref* h, int leg); /* -1 = off */
+int me_info_ref(const me_handle_ref* h, int what);  /* 0 n_diag, 1 n_terms, 2 n_diag with 4g, 3 n_flow, 4 n_gluon */
+int me_colour_matrix_ref(const me_handle_ref* h, double* cf /*[n_flow][n_flow]*/);
+int me_flow_perms_ref(const me_handle_ref* h, int* perms /*[n_flow][n_gluon]*/);
+int me_amplitude_def_ref(me_handle_ref* h, const double* mom, const int* hel, const int* col, double* re_im);
+int me_flows_ref(me_handle_ref* h, const double* mom, const int* hel, double* J /*[n_flow][2]*/);
+int su3_generators_ref(double* T /*[8][3][3][2]*/, double* f /*[8][8][8]*/);
+/* kind: 0 u column, 1 v column, 2 polarisation vector; out = 4 complex (re,im interleaved) */
+int wavefunction_ref(int kind, const double* p, double mass, int s, int basis, double* out);
+
+/* --- random numbers, phase space, cuts --- */
+int philox_raw_ref(const uint32_t* ctr, const uint32_t* key, uint32_t* out);
+int philox_uniform_ref(uint64_t seed, uint64_t iteration, long long first_event, int n_dim, double* rand, long long n_ev);
+int rambo_generate_ref(const double* rand, double sqrt_s, const double* masses, int n_final, int ps_mode,
+                       double* momenta, double* weights, long long n_ev);
+int cuts_ref(const double* momenta, int n_final, const int* is_gluon, double ptj_min, double dr_min, int* pass, long long n_ev);
+
+/* --- Vegas --- */
+int vegas_map_ref(const double* edges, int n_dim, int n_bins, const double* y, double* x, double* jac, int* idx, long long n);
+/* sums[0] = sum f, sums[1] = sum f^2, sums[2] = #(f != 0), sums[3 + d*n_bins + i] = S_{d,i} */
+int vegas_accumulate_ref(const double* f, const int* idx, int n_dim, int n_bins, long long n, double* sums);
+int vegas_refine_ref(double* edges, int n_dim, int n_bins, const double* S, double alpha);
+/* the physics integrand of SURVEY §8(c) G6 over events [first_event, first_event+n_ev) of this iteration;
+ * f_out (optional, may be NULL) receives the per-event f. Does NOT refine. */
+int vegas_integrand_ref(me_handle_ref* h, const vegas_grid_ref* g, double sqrt_s, long long first_event, long long n_ev,
+                        double* sums, double* f_out);
+/* one full iteration on events [0, n_ev): integrand, result, refine g->edges in place, ++g->iteration */
+int vegas_iterate_ref(me_handle_ref* h, vegas_grid_ref* g, double sqrt_s, long long n_ev, vegas_result_ref* result);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,217 @@
+"""Pins for the oracle's Philox, RAMBO and cuts (pin table I). CPU only."""
+import ctypes as C
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle import ref
+from tests.helpers import mdot
+
+
+# ---- Philox ---------------------------------------------------------------------------------------------
+def _curand_host():
+    for name in ("libcurand.so", "libcurand.so.10", "/usr/local/cuda/lib64/libcurand.so"):
+        try:
+            return C.CDLL(name)
+        except OSError:
+            continue
+    return None
+
+
+def test_philox_against_curand_library():
+    """SURVEY §8(c) G4 pin: bit pattern against a LIBRARY Philox4x32-10 (cuRAND's host generator, no GPU needed).
+    cuRAND's default host ordering emits, for seed k, the blocks of counters (0,0,j,0), j = 0,1,2,...: the
+    subsequence number lands in counter word 2 (probed, not assumed: the test checks 16 blocks and 3 seeds)."""
+    lib = _curand_host()
+    if lib is None:
+        pytest.skip("libcurand not loadable: Philox bit pattern unpinned on this box")
+    for seed in (0, 3, 0x0123456789ABCDEF):
+        gen = C.c_void_p()
+        assert lib.curandCreateGeneratorHost(C.byref(gen), 161) == 0  # CURAND_RNG_PSEUDO_PHILOX4_32_10
+        assert lib.curandSetPseudoRandomGeneratorSeed(gen, C.c_ulonglong(seed)) == 0
+        out = np.zeros(64, dtype=np.uint32)
+        assert lib.curandGenerate(gen, out.ctypes.data_as(C.c_void_p), C.c_size_t(64)) == 0
+        lib.curandDestroyGenerator(gen)
+        key = [seed & 0xFFFFFFFF, seed >> 32]
+        for j in range(16):
+            assert list(ref.philox_raw([0, 0, j, 0], key)) == list(out[4 * j:4 * j + 4])
+
+
+def test_philox_counter_sensitivity():
+    """Every counter/key word matters (a dropped word would alias streams)."""
+    base = ref.philox_raw([1, 2, 3, 4], [5, 6])
+    for w in range(4):
+        c = [1, 2, 3, 4]
+        c[w] += 1
+        assert not np.array_equal(ref.philox_raw(c, [5, 6]), base)
+    assert not np.array_equal(ref.philox_raw([1, 2, 3, 4], [6, 6]), base)
+    assert not np.array_equal(ref.philox_raw([1, 2, 3, 4], [5, 7]), base)
+
+
+def test_philox_uniform_layout_and_statistics():
+    """u in the open interval; u depends only on (seed, iteration, global event index): any sharding gives the
+    same stream; mapping of dimension d -> (pair d//2, word pair d%2) with 53-bit mantissa; moments."""
+    u = ref.philox_uniform(7, 2, 0, 5, 1 << 16)
+    assert u.min() > 0 and u.max() < 1
+    a = ref.philox_uniform(7, 2, 1000, 5, 100)
+    assert np.array_equal(a, u[1000:1100])
+    assert not np.array_equal(ref.philox_uniform(7, 3, 0, 5, 16), u[:16])
+    assert not np.array_equal(ref.philox_uniform(8, 2, 0, 5, 16), u[:16])
+    ev = 12345
+    for d in range(5):
+        o = ref.philox_raw([ev, 0, d // 2, 2], [7, 0])
+        hi, lo = int(o[2 * (d % 2)]), int(o[2 * (d % 2) + 1])
+        want = (((hi << 32 | lo) >> 11) + 0.5) / 2 ** 53
+        assert u[ev, d] == want
+    n = u.size
+    assert abs(u.mean() - 0.5) < 5 / math.sqrt(12 * n)
+    assert abs((u ** 2).mean() - 1 / 3) < 5 * math.sqrt(4 / 45 / n)
+    c = np.corrcoef(u.T)
+    assert np.max(np.abs(c - np.eye(5))) < 5 / math.sqrt(u.shape[0])
+    assert abs(np.corrcoef(u[:-1, 0], u[1:, 0])[0, 1]) < 5 / math.sqrt(u.shape[0])
+    # 64-bit event index reaches the second counter word
+    hi_ev = (1 << 32) + 5
+    assert ref.philox_uniform(7, 2, hi_ev, 2, 1)[0, 0] != ref.philox_uniform(7, 2, 5, 2, 1)[0, 0]
+
+
+# ---- RAMBO ----------------------------------------------------------------------------------------------
+CASES = [((0.0, 0.0), 100.0), ((173.0, 173.0), 1000.0), ((173.0, 173.0, 0.0), 1000.0), ((173.0, 173.0, 0.0, 0.0), 1000.0),
+         ((0.0, 0.0, 0.0, 0.0), 1000.0), ((10.0, 80.0, 0.0, 30.0, 5.0), 500.0)]
+
+
+@pytest.mark.parametrize("ps_mode", [0, 1])
+@pytest.mark.parametrize("masses,sqrt_s", CASES)
+def test_rambo_conservation_and_mass_shell(masses, sqrt_s, ps_mode):
+    """SURVEY §8(c) G1 pins: sum p = (sqrt_s,0,0,0), p_i^2 = m_i^2 (1e-12 s typical; 1e-9 s worst case of the
+    ill-conditioned near-parallel configurations of classic RAMBO), incoming legs (sqrt_s/2)(1,0,0,+-1)."""
+    n = len(masses)
+    if ps_mode == 1 and n < 3:
+        pytest.skip("diet RAMBO needs n >= 3 here")
+    nd = 4 * n if ps_mode == 0 else 3 * n - 4
+    u = ref.philox_uniform(42, 0, 0, nd, 20000)
+    mom, w = ref.rambo_generate(u, sqrt_s, masses, ps_mode)
+    tot = mom[:, 2:].sum(1)
+    tot[:, 0] -= sqrt_s
+    dev = np.abs(tot).max(1) / sqrt_s
+    assert np.median(dev) < 1e-14 and dev.max() < 1e-9
+    m2 = mdot(mom[:, 2:], mom[:, 2:])
+    devm = np.abs(m2 - np.array(masses) ** 2).max(1) / sqrt_s ** 2
+    assert np.median(devm) < 1e-14 and devm.max() < 1e-9
+    assert np.all(mom[:, 2:, 0] > 0) and np.all(w > 0)
+    assert np.array_equal(mom[:, 0], np.tile([sqrt_s / 2, 0, 0, sqrt_s / 2], (20000, 1)))
+    assert np.array_equal(mom[:, 1], np.tile([sqrt_s / 2, 0, 0, -sqrt_s / 2], (20000, 1)))
+
+
+def test_rambo_massless_weight_closed_form():
+    """W0 = (pi/2)^{n-1} s^{n-2} / [(n-1)!(n-2)!] (2 pi)^{4-3n}; n=2: 1/(8 pi)."""
+    for n in (2, 3, 4, 5):
+        for mode in ((0, 1) if n > 2 else (0,)):
+            nd = 4 * n if mode == 0 else 3 * n - 4
+            u = ref.philox_uniform(1, 0, 0, nd, 50)
+            s = 1000.0 ** 2
+            _, w = ref.rambo_generate(u, 1000.0, [0.0] * n, mode)
+            want = (math.pi / 2) ** (n - 1) * s ** (n - 2) / (math.factorial(n - 1) * math.factorial(n - 2)) * (2 * math.pi) ** (4 - 3 * n)
+            assert np.max(np.abs(w / want - 1)) < 1e-13
+    _, w = ref.rambo_generate(ref.philox_uniform(1, 0, 0, 8, 4), 100.0, [0.0, 0.0])
+    assert np.max(np.abs(w * 8 * math.pi - 1)) < 1e-14
+
+
+def test_rambo_two_body_massive_weight():
+    """n = 2 closed forms: W(m,m) = beta/(8 pi); unequal masses W = lambda^{1/2}(s,m1^2,m2^2)/(8 pi s)."""
+    u = ref.philox_uniform(1, 0, 0, 8, 200)
+    m, rs = 173.0, 1000.0
+    _, w = ref.rambo_generate(u, rs, [m, m])
+    assert np.max(np.abs(w / (math.sqrt(1 - 4 * m * m / rs ** 2) / (8 * math.pi)) - 1)) < 1e-12
+    m1, m2 = 80.0, 250.0
+    _, w = ref.rambo_generate(u, rs, [m1, m2])
+    s = rs * rs
+    lam = (s - (m1 + m2) ** 2) * (s - (m1 - m2) ** 2)
+    assert np.max(np.abs(w / (math.sqrt(lam) / (8 * math.pi * s)) - 1)) < 1e-12
+
+
+def test_rambo_massive_three_body_volume():
+    """<W> = massive phase-space volume.  Independent value: 1-D numerical quadrature of the textbook recursion
+    Phi_3(s; m,m,0) = int dM^2/(2 pi) Phi_2(s; M^2, 0) Phi_2(M^2; m, m),  Phi_2 = lambda^{1/2}/(8 pi s)."""
+    from scipy import integrate
+    m, rs = 173.0, 1000.0
+    s = rs * rs
+
+    def f(M2):
+        return (1 / (2 * math.pi)) * ((s - M2) / (8 * math.pi * s)) * (math.sqrt(1 - 4 * m * m / M2) / (8 * math.pi))
+
+    vol, _ = integrate.quad(f, 4 * m * m, s, epsabs=0, epsrel=1e-10)
+    for mode in (0, 1):
+        nd = 12 if mode == 0 else 5
+        u = ref.philox_uniform(9, 0, 0, nd, 400000)
+        _, w = ref.rambo_generate(u, rs, [m, m, 0.0], mode)
+        err = w.std() / math.sqrt(len(w))
+        assert abs(w.mean() - vol) < 4.5 * err, (w.mean(), vol, err)
+        assert err / vol < 2e-3
+
+
+def test_rambo_isotropy_and_energy_sharing():
+    """Massless: <cos theta_i> = 0, <E_i> = sqrt_s / n for both variants."""
+    for mode in (0, 1):
+        n = 4
+        nd = 16 if mode == 0 else 8
+        u = ref.philox_uniform(5, 0, 0, nd, 200000)
+        mom, _ = ref.rambo_generate(u, 1000.0, [0.0] * n, mode)
+        p = mom[:, 2:]
+        cos = p[..., 3] / p[..., 0]
+        assert np.max(np.abs(cos.mean(0))) < 5 * math.sqrt(1 / 3 / 200000)
+        assert np.max(np.abs(p[..., 0].mean(0) / 250.0 - 1)) < 5e-3
+
+
+def test_rambo_diet_matches_classic_distributions():
+    """SURVEY §8(c) G2 pin: for n = 4 the distributions of m12^2, m34^2, E1, E4 agree with classic RAMBO."""
+    N = 300000
+    moms = []
+    for mode, nd in ((0, 16), (1, 8)):
+        u = ref.philox_uniform(77 + mode, 0, 0, nd, N)
+        moms.append(ref.rambo_generate(u, 1000.0, [0.0] * 4, mode)[0][:, 2:])
+    s = 1e6
+    obs = []
+    for p in moms:
+        m12 = mdot(p[:, 0] + p[:, 1], p[:, 0] + p[:, 1]) / s
+        m34 = mdot(p[:, 2] + p[:, 3], p[:, 2] + p[:, 3]) / s
+        m14 = mdot(p[:, 0] + p[:, 3], p[:, 0] + p[:, 3]) / s
+        obs.append(np.stack([m12, m34, m14, m12 ** 2, m34 * m14, p[:, 0, 0] / 1e3, p[:, 3, 0] / 1e3, (p[:, 3, 0] / 1e3) ** 2,
+                             (p[:, 1, 0] / 1e3) * (p[:, 2, 3] / 1e3) ** 2], 1))
+    a, b = obs
+    z = (a.mean(0) - b.mean(0)) / np.sqrt(a.var(0) / N + b.var(0) / N)
+    assert np.max(np.abs(z)) < 4.5, z
+    # closed form for massless n = 4: <m12^2/s> = 1/6 (each of the six pairs carries the same share of s)
+    assert abs(a[:, 0].mean() - 1 / 6) < 5 * a[:, 0].std() / math.sqrt(N)
+    assert abs(b[:, 0].mean() - 1 / 6) < 5 * b[:, 0].std() / math.sqrt(N)
+
+
+# ---- cuts -----------------------------------------------------------------------------------------------
+def test_cuts_hand_built_events():
+    """pT(g) > 20, DeltaR(g, X) > 0.4 with true rapidity, dphi wrapped, strict inequalities."""
+    def vec(pt, y, phi, m=0.0):
+        mt = math.sqrt(pt * pt + m * m)
+        return [mt * math.cosh(y), pt * math.cos(phi), pt * math.sin(phi), mt * math.sinh(y)]
+
+    beams = [[500, 0, 0, 500], [500, 0, 0, -500]]
+    isg = [0, 0, 1, 1]
+
+    def ev(g1, g2, t=(100, 0.3, 0.1), tb=(90, -0.5, 2.5)):
+        return np.array([beams + [vec(*t, m=173.0), vec(*tb, m=173.0), vec(*g1), vec(*g2)]])
+
+    assert ref.cuts(ev((50, 0.0, 1.0), (40, 1.0, -2.0)), isg, 20, 0.4)[0] == 1
+    assert ref.cuts(ev((19.999, 0.0, 1.0), (40, 1.0, -2.0)), isg, 20, 0.4)[0] == 0        # pT fails
+    assert ref.cuts(ev((50, 0.0, 1.0), (40, 0.2, 1.3)), isg, 20, 0.4)[0] == 0             # dR(g,g) = 0.36
+    assert ref.cuts(ev((50, 0.0, 1.0), (40, 0.3, 1.3)), isg, 20, 0.4)[0] == 1             # dR(g,g) = 0.424
+    assert ref.cuts(ev((50, 0.3, 0.3), (40, 1.0, -2.0)), isg, 20, 0.4)[0] == 0            # dR(g,t) = 0.2
+    # dphi wraps: phi = 3.1 and -3.1 are 0.083 apart
+    assert ref.cuts(ev((50, 0.0, 3.1), (40, 0.0, -3.1)), isg, 20, 0.4)[0] == 0
+    # rapidity, not pseudorapidity, for the massive top: pick t with y far from eta
+    t = (5.0, 0.05, 1.0)   # eta(t) = 0.05/... top nearly at rest transversely: y=0.05 but pseudo-rapidity large
+    g = (50, 0.3, 1.0)
+    assert ref.cuts(ev(g, (40, 1.5, -2.0), t=t), isg, 20, 0.4)[0] == 0                    # dy = 0.25 < 0.4
+    # disabled cuts
+    assert ref.cuts(ev((1.0, 0.0, 1.0), (40, 0.01, 1.0)), isg, 0, 0)[0] == 1
+    # config 2: dR only to t, tbar
+    assert ref.cuts(ev((50, 0.3, 0.3), (40, 1.0, -2.0))[:, :5], [0, 0, 1], 20, 0.4)[0] == 0

@@ -1,0 +1,102 @@
+"""Pins for the oracle's Vegas pieces (SURVEY.md §8(c) G7 'Pins'): closed-form integrals, fixed end points,
+alpha = 0 fixed point, <jac> = 1, quantile convergence.  The grid-update details (alpha = 1.5, 3-point smoothing)
+are a READING of Lepage's algorithm (DESIGN.md R-G7), not fixed by the paper.  CPU only."""
+import math
+
+import numpy as np
+
+from oracle import ref
+
+
+def run_vegas(f, D, n_it, n_ev, alpha=1.5, nb=50, seed=4):
+    edges = np.tile(np.linspace(0, 1, nb + 1), (D, 1))
+    res = []
+    for it in range(n_it):
+        y = ref.philox_uniform(seed, it, 0, D, n_ev)
+        x, jac, idx = ref.vegas_map(edges, y)
+        fv = jac * f(x)
+        sums = ref.vegas_accumulate(fv, idx, nb)
+        I = sums[0] / n_ev
+        var = (sums[1] / n_ev - I * I) / (n_ev - 1)
+        res.append((I, var))
+        edges = ref.vegas_refine(edges, sums[3:], alpha)
+    return edges, res
+
+
+def test_map_uniform_grid_is_identity():
+    edges = np.tile(np.linspace(0, 1, 51), (3, 1))
+    y = ref.philox_uniform(1, 0, 0, 3, 1000)
+    x, jac, idx = ref.vegas_map(edges, y)
+    assert np.max(np.abs(x - y)) < 1e-15 and np.max(np.abs(jac - 1)) < 1e-13
+    assert np.array_equal(idx, np.minimum((y * 50).astype(int), 49))
+
+
+def test_jacobian_averages_to_one_and_integral_of_one():
+    """On any grid, int jac dy = 1 exactly per dimension: sample mean -> 1; integrand 1 integrates to 1."""
+    rng = np.random.default_rng(0)
+    e = np.sort(rng.uniform(size=(4, 49)), axis=1)
+    edges = np.concatenate([np.zeros((4, 1)), e, np.ones((4, 1))], 1)
+    y = ref.philox_uniform(2, 0, 0, 4, 400000)
+    x, jac, idx = ref.vegas_map(edges, y)
+    assert abs(jac.mean() - 1) < 5 * jac.std() / math.sqrt(len(jac))
+    assert x.min() >= 0 and x.max() <= 1
+    # x lies in the bin it claims
+    for d in range(4):
+        assert np.all(x[:, d] >= edges[d, idx[:, d]] - 1e-15) and np.all(x[:, d] <= edges[d, idx[:, d] + 1] + 1e-15)
+
+
+def test_alpha_zero_is_a_fixed_point_and_endpoints_stay():
+    f = lambda x: np.exp(-50 * ((x - 0.3) ** 2).sum(1))
+    edges, _ = run_vegas(f, 2, 2, 20000, alpha=0.0)
+    assert np.max(np.abs(edges - np.linspace(0, 1, 51))) < 1e-13
+    edges, _ = run_vegas(f, 2, 4, 20000, alpha=1.5)
+    assert np.all(edges[:, 0] == 0) and np.all(edges[:, -1] == 1)
+    assert np.all(np.diff(edges, axis=1) > 0)
+
+
+def test_separable_gaussian_closed_form():
+    """int over [0,1]^4 of prod_d exp(-(x_d-mu)^2/(2 s^2)) = [s sqrt(2 pi) (Phi((1-mu)/s) - Phi(-mu/s))]^4."""
+    mu, s, D = 0.4, 0.05, 4
+    f = lambda x: np.exp(-((x - mu) ** 2).sum(1) / (2 * s * s))
+    one = s * math.sqrt(2 * math.pi) * 0.5 * (math.erf((1 - mu) / s / math.sqrt(2)) - math.erf(-mu / s / math.sqrt(2)))
+    exact = one ** D
+    edges, res = run_vegas(f, D, 6, 40000)
+    I = np.array([r[0] for r in res])
+    var = np.array([r[1] for r in res])
+    # each iteration is unbiased; adaptation shrinks the error by a large factor
+    for Ij, vj in zip(I, var):
+        assert abs(Ij - exact) < 5 * math.sqrt(vj)
+    assert var[-1] < var[0] / 50
+    comb = (I / var).sum() / (1 / var).sum()
+    assert abs(comb - exact) < 5 * (1 / var).sum() ** -0.5
+
+
+def test_edges_converge_to_quantiles_in_1d():
+    """With alpha = 1 repeated refinement puts equal sum f^2 ... in 1-D for f ∝ density p the optimal Vegas grid
+    equalises int |f| per bin; check the adapted grid's median edge against the |f|-quantile within a bin width."""
+    f = lambda x: 3 * x[:, 0] ** 2
+    edges, res = run_vegas(f, 1, 12, 100000, alpha=1.0, nb=50)
+    # CDF of |f| is x^3 -> median at 0.5^(1/3)
+    med = edges[0, 25]
+    assert abs(med - 0.5 ** (1 / 3)) < 0.03
+    assert abs(edges[0, 5] - 0.1 ** (1 / 3)) < 0.06
+    I = res[-1][0]
+    assert abs(I - 1) < 5 * math.sqrt(res[-1][1])
+    assert res[-1][1] < res[0][1] / 20
+
+
+def test_refine_hand_case():
+    """Two bins, alpha = 1, S = (1, 3): smoothing gives s = (2, 2) -> weights equal -> edge stays at 0.5.
+    Three bins, S = (0, 0, 6), alpha = 1: s = (0, 2, 3), r = (0, .4, .6), w = (0, (r-1)/ln r ...) by hand."""
+    e = ref.vegas_refine(np.array([[0, 0.5, 1.0]]), np.array([[1.0, 3.0]]), 1.0)
+    assert np.allclose(e, [[0, 0.5, 1.0]])
+    S = np.array([[0.0, 0.0, 6.0]])
+    e0 = np.array([[0, 1 / 3, 2 / 3, 1.0]])
+    e = ref.vegas_refine(e0, S, 1.0)[0]
+    r = np.array([0.0, 0.4, 0.6])
+    w = np.array([0.0, (0.4 - 1) / math.log(0.4), (0.6 - 1) / math.log(0.6)])
+    tgt = w.sum() / 3
+    # new edge 1 at cumulative tgt: inside old bin 1 (bin 0 has zero weight)
+    want1 = 1 / 3 + (tgt / w[1]) / 3
+    want2 = (1 / 3 + (2 * tgt / w[1]) / 3) if 2 * tgt <= w[1] else (2 / 3 + ((2 * tgt - w[1]) / w[2]) / 3)
+    assert abs(e[1] - want1) < 1e-14 and abs(e[2] - want2) < 1e-14 and e[0] == 0 and e[3] == 1
