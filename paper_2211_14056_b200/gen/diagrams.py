@@ -1,0 +1,382 @@
+"""Build-time diagram generator: process -> list of off-shell currents + closing amplitudes + colour flows.
+
+This replaces the MG5_aMC + jinja transpiler layers of the paper (Fig. 2): there is no
+MadGraph here, so the Feynman diagrams of a process are enumerated directly and the
+colour-flow coefficient table is derived numerically from explicit SU(3) tensors.
+It shares no source with oracle/ (which enumerates at run time in C++ with its own data structures).
+
+Model: one fermion line per flavour; vertices {f fbar V, ggg, gggg}; "V" is the gluon for the top line
+and the photon for the lepton lines.
+
+A *diagram* is a tree whose leaves are the external legs.  Every diagram is evaluated "closed" at its
+centroid vertex: the vertex whose hanging subtrees all have <= n/2 leaves (ties — a propagator
+splitting the legs n/2 | n/2 — go to the side that holds leg 0).  The hanging subtrees are the off-shell
+currents; structurally identical subtrees are shared between diagrams.  A subtree / diagram containing a
+four-gluon vertex splits into three colour-pure terms.
+
+Powers of i and of the coupling carried by vertices and propagators are NOT applied numerically: every
+object carries a symbolic phase in {1, i, -1, -i}, which ends up in the flow coefficient of the term.
+Feynman rules, all momenta incoming:
+    f fbar V   : i g gamma^mu T^a            ggg : g f^{abc} [...]        gggg : -i g^2 [...]
+    fermion propagator  i (qslash + m)/(q^2 - m^2)       vector propagator  -i g^{mu nu}/q^2
+"""
+import itertools
+from collections import namedtuple
+
+import numpy as np
+
+# ---- legs ---------------------------------------------------------------------------------------------------
+# kind ids match csrc/helas.cuh::LegKind
+LEG_V_IN, LEG_V_OUT, LEG_F_OUT, LEG_FB_OUT, LEG_F_IN, LEG_FB_IN = range(6)
+Leg = namedtuple("Leg", "kind flavour massive")  # flavour: 'g' | 'a' for vectors, 't' | 'e' | 'mu' for fermions
+
+PROCESSES = {
+    # name: (legs, coupling-constant name, averaging denominator S of SURVEY §8(c) F)
+    "epem_mupmum": ([Leg(LEG_F_IN, "e", False), Leg(LEG_FB_IN, "e", False),
+                     Leg(LEG_F_OUT, "mu", False), Leg(LEG_FB_OUT, "mu", False)], "ee", 4),
+    "gg_ttx": ([Leg(LEG_V_IN, "g", False), Leg(LEG_V_IN, "g", False),
+                Leg(LEG_F_OUT, "t", True), Leg(LEG_FB_OUT, "t", True)], "gs", 4 * 64),
+    "gg_ttxg": ([Leg(LEG_V_IN, "g", False), Leg(LEG_V_IN, "g", False), Leg(LEG_F_OUT, "t", True),
+                 Leg(LEG_FB_OUT, "t", True), Leg(LEG_V_OUT, "g", False)], "gs", 4 * 64),
+    "gg_ttxgg": ([Leg(LEG_V_IN, "g", False), Leg(LEG_V_IN, "g", False), Leg(LEG_F_OUT, "t", True),
+                  Leg(LEG_FB_OUT, "t", True), Leg(LEG_V_OUT, "g", False), Leg(LEG_V_OUT, "g", False)],
+                 "gs", 4 * 64 * 2),
+}
+VECTOR_OF = {"t": "g", "e": "a", "mu": "a"}
+
+# ---- SU(3) ---------------------------------------------------------------------------------------------------
+
+
+def su3():
+    """Gell-Mann T^a = lambda^a/2 and f^{abc} from [T^a, T^b] = i f^{abc} T^c."""
+    l = np.zeros((8, 3, 3), dtype=complex)
+    l[0][0, 1] = l[0][1, 0] = 1
+    l[1][0, 1] = -1j
+    l[1][1, 0] = 1j
+    l[2][0, 0] = 1
+    l[2][1, 1] = -1
+    l[3][0, 2] = l[3][2, 0] = 1
+    l[4][0, 2] = -1j
+    l[4][2, 0] = 1j
+    l[5][1, 2] = l[5][2, 1] = 1
+    l[6][1, 2] = -1j
+    l[6][2, 1] = 1j
+    l[7] = np.diag([1, 1, -2]) / np.sqrt(3)
+    T = l / 2
+    f = np.zeros((8, 8, 8))
+    for a in range(8):
+        for b in range(8):
+            comm = T[a] @ T[b] - T[b] @ T[a]
+            for c in range(8):
+                f[a, b, c] = (-2j * np.trace(comm @ T[c])).real  # Tr(T^c T^d) = delta/2
+    return T, f
+
+
+_T, _F = su3()
+
+# ---- objects ---------------------------------------------------------------------------------------------------
+# type: ('V', vflavour) | ('O', flavour) row spinor | ('I', flavour) column spinor
+# op  : 'EXT' | 'FFV_ROW' (O,V->O) | 'FFV_COL' (I,V->I) | 'FFV_VEC' (O,I->V) | 'VVV' (V,V->V) | 'VVVV1/2/3' (V,V,V->V)
+
+
+class Obj:
+    __slots__ = ("id", "legs", "type", "op", "args", "phase", "_col", "skel", "has4g")
+
+    def __init__(self, id, legs, type, op, args, phase):
+        self.id, self.legs, self.type, self.op, self.args, self.phase = id, tuple(sorted(legs)), type, op, args, phase
+        self._col = None
+        self.skel = None    # structural key: the three colour terms of one 4g subtree share it
+        self.has4g = False
+
+
+class Term:
+    """One colour-pure closing amplitude."""
+    __slots__ = ("op", "args", "phase", "which", "diagram", "flows")
+
+    def __init__(self, op, args, phase, which, diagram):
+        self.op, self.args, self.phase, self.which, self.diagram, self.flows = op, args, phase, which, diagram, None
+
+
+def _set_partitions(items, k):
+    """All unordered partitions of `items` (list) into exactly k non-empty blocks."""
+    items = list(items)
+    if k == 1:
+        yield [items]
+        return
+    if len(items) < k:
+        return
+    first, rest = items[0], items[1:]
+    # first alone + partition of the rest into k-1
+    for p in _set_partitions(rest, k - 1):
+        yield [[first]] + p
+    # first joins one block of a partition of rest into k
+    for p in _set_partitions(rest, k):
+        for i in range(len(p)):
+            yield p[:i] + [[first] + p[i]] + p[i + 1:]
+
+
+class Program:
+    """The evaluated-closed-at-centroid diagram list of one process."""
+
+    def __init__(self, name):
+        self.name = name
+        self.legs, self.coupling, self.avg = PROCESSES[name]
+        self.n = len(self.legs)
+        self.objs = []
+        self._memo = {}
+        self.terms = []
+        self.n_diagrams = 0
+        self.n_diagrams_4g = 0
+        self._ext = {}
+        self._diagrams = {}
+        for i, leg in enumerate(self.legs):
+            if leg.kind in (LEG_V_IN, LEG_V_OUT):
+                t = ("V", leg.flavour)
+            elif leg.kind in (LEG_F_OUT, LEG_FB_IN):
+                t = ("O", leg.flavour)
+            else:
+                t = ("I", leg.flavour)
+            self._ext[i] = self._new((i,), t, "EXT", (), 1)
+        self._close()
+        self._colour()
+
+    # -- enumeration ------------------------------------------------------------------------------------------
+    def _new(self, legs, type, op, args, phase):
+        o = Obj(len(self.objs), legs, type, op, args, phase)
+        o.skel = (op[:4] if op.startswith("VVVV") else op, tuple(sorted(legs)), tuple(self.objs[a].skel for a in args))
+        o.has4g = op.startswith("VVVV") or any(self.objs[a].has4g for a in args)
+        self.objs.append(o)
+        return o
+
+    def subtrees(self, legs):
+        """All distinct subtrees (as off-shell currents, propagator included) with leaf set `legs`."""
+        key = tuple(sorted(legs))
+        if key in self._memo:
+            return self._memo[key]
+        if len(key) == 1:
+            res = [self._ext[key[0]]]
+            self._memo[key] = res
+            return res
+        res = []
+        for parts in _set_partitions(key, 2):
+            for A in self.subtrees(parts[0]):
+                for B in self.subtrees(parts[1]):
+                    res.extend(self._join2(key, A, B))
+        for parts in _set_partitions(key, 3):
+            for A in self.subtrees(parts[0]):
+                for B in self.subtrees(parts[1]):
+                    for C in self.subtrees(parts[2]):
+                        if A.type == B.type == C.type == ("V", "g"):
+                            # vertex -i g^2, propagator -i  -> phase -1
+                            ph = A.phase * B.phase * C.phase * (-1)
+                            for w in (1, 2, 3):
+                                res.append(self._new(key, ("V", "g"), "VVVV%d" % w, (A.id, B.id, C.id), ph))
+        self._memo[key] = res
+        return res
+
+    def _join2(self, key, A, B):
+        out = []
+        for X, Y in ((A, B), (B, A)):
+            kx, fx = X.type
+            ky, fy = Y.type
+            if kx == "O" and ky == "V" and VECTOR_OF[fx] == fy:
+                # vertex i g, propagator i -> -1
+                out.append(self._new(key, X.type, "FFV_ROW", (X.id, Y.id), X.phase * Y.phase * (-1)))
+            if kx == "I" and ky == "V" and VECTOR_OF[fx] == fy:
+                out.append(self._new(key, X.type, "FFV_COL", (X.id, Y.id), X.phase * Y.phase * (-1)))
+            if kx == "O" and ky == "I" and fx == fy:
+                # vertex i g, propagator -i -> +1
+                out.append(self._new(key, ("V", VECTOR_OF[fx]), "FFV_VEC", (X.id, Y.id), X.phase * Y.phase))
+        if A.type == B.type == ("V", "g"):
+            # vertex g (real), propagator -i
+            out.append(self._new(key, ("V", "g"), "VVV", (A.id, B.id), A.phase * B.phase * (-1j)))
+        return out
+
+    def _close(self):
+        n = self.n
+        allowed = lambda part: 2 * len(part) < n or (2 * len(part) == n and 0 not in part)
+        all_legs = list(range(n))
+        for parts in _set_partitions(all_legs, 3):
+            if not all(allowed(p) for p in parts):
+                continue
+            for A in self.subtrees(parts[0]):
+                for B in self.subtrees(parts[1]):
+                    for C in self.subtrees(parts[2]):
+                        self._close3(A, B, C)
+        for parts in _set_partitions(all_legs, 4):
+            if not all(allowed(p) for p in parts):
+                continue
+            for combo in itertools.product(*[self.subtrees(p) for p in parts]):
+                if all(o.type == ("V", "g") for o in combo):
+                    d = self._count_diagram(combo, True)
+                    ph = np.prod([o.phase for o in combo]) * (-1j)  # vertex -i g^2
+                    for w in (1, 2, 3):
+                        self.terms.append(Term("VVVV_AMP", tuple(o.id for o in combo), ph, w, d))
+
+    def _count_diagram(self, combo, closing_4g):
+        key = (closing_4g, tuple(sorted(o.skel for o in combo)))
+        if key not in self._diagrams:
+            self._diagrams[key] = len(self._diagrams)
+            self.n_diagrams += 1
+            if closing_4g or any(o.has4g for o in combo):
+                self.n_diagrams_4g += 1
+        return self._diagrams[key]
+
+    def _close3(self, A, B, C):
+        objs = (A, B, C)
+        kinds = [o.type[0] for o in objs]
+        if sorted(kinds) == ["I", "O", "V"]:
+            O = objs[kinds.index("O")]
+            I = objs[kinds.index("I")]
+            V = objs[kinds.index("V")]
+            if O.type[1] == I.type[1] and VECTOR_OF[O.type[1]] == V.type[1]:
+                d = self._count_diagram(objs, False)
+                self.terms.append(Term("FFV_AMP", (O.id, V.id, I.id), O.phase * I.phase * V.phase * 1j, 0, d))
+        elif all(o.type == ("V", "g") for o in objs):
+            d = self._count_diagram(objs, False)
+            self.terms.append(Term("VVV_AMP", (A.id, B.id, C.id), A.phase * B.phase * C.phase, 0, d))
+
+    # -- colour ------------------------------------------------------------------------------------------------
+    # colour tensor of an object: (array, labels); labels = external coloured legs it contains + 'out'
+    def _coloured(self, leg):
+        return self.legs[leg].flavour in ("g", "t")
+
+    def _col(self, o):
+        if o._col is not None:
+            return o._col
+        A = [self._col(self.objs[a]) for a in o.args]
+        if o.op == "EXT":
+            leg = o.legs[0]
+            if not self._coloured(leg):
+                r = (np.ones(()), [])
+            else:
+                d = 8 if self.legs[leg].flavour == "g" else 3
+                r = (np.eye(d, dtype=complex), [leg, "out"])
+        elif not all(self._coloured(l) for l in o.legs):
+            r = (np.ones(()), [])
+        elif o.op == "FFV_ROW":   # psibar_m (T^c)_{mn} -> open n
+            r = self._contract("mcn", _T.transpose(1, 0, 2), A[0], "m", A[1], "c", out="n")
+        elif o.op == "FFV_COL":   # (T^c)_{mn} psi_n -> open m
+            r = self._contract("mcn", _T.transpose(1, 0, 2), A[0], "n", A[1], "c", out="m")
+        elif o.op == "FFV_VEC":   # psibar_m (T^c)_{mn} psi_n -> open c
+            r = self._contract("mcn", _T.transpose(1, 0, 2), A[0], "m", A[1], "n", out="c")
+        elif o.op == "VVV":       # f^{x y e}
+            r = self._contract("xye", _F, A[0], "x", A[1], "y", out="e")
+        else:
+            ff = {"VVVV1": np.einsum("xye,zde->xyzd", _F, _F), "VVVV2": np.einsum("xze,yde->xyzd", _F, _F),
+                  "VVVV3": np.einsum("xde,yze->xyzd", _F, _F)}[o.op]
+            r = self._contract("xyzd", ff, A[0], "x", A[1], "y", A[2], "z", out="d")
+        o._col = r
+        return r
+
+    @staticmethod
+    def _contract(vlabels, vertex, *rest, out=None):
+        """Contract a vertex tensor with operand tensors over their 'out' axes."""
+        ops = list(zip(rest[0::2], rest[1::2]))
+        letters = iter("abcdefghijklmnopqrstuvwxyz".upper())
+        sub_v = {c: next(letters) for c in vlabels}
+        inputs, arrays, keep = [], [], []
+        for (arr, labels), vl in ops:
+            s = ""
+            for lab in labels:
+                if lab == "out":
+                    s += sub_v[vl]
+                else:
+                    ch = next(letters)
+                    s += ch
+                    keep.append((lab, ch))
+            inputs.append(s)
+            arrays.append(arr)
+        keep.sort(key=lambda t: t[0])
+        out_s = "".join(ch for _, ch in keep) + (sub_v[out] if out else "")
+        expr = "".join(sub_v[c] for c in vlabels) + "," + ",".join(inputs) + "->" + out_s
+        res = np.einsum(expr, vertex, *arrays, optimize=True)
+        return res, [lab for lab, _ in keep] + (["out"] if out else [])
+
+    def _colour(self):
+        col_legs = [i for i in range(self.n) if self._coloured(i)]
+        glu = [i for i in col_legs if self.legs[i].flavour == "g"]
+        self.gluons = glu
+        if not col_legs:
+            self.flow_perms = [()]
+            self.cf_num = np.array([[1]], dtype=np.int64)
+            self.cf_den = 1
+            for t in self.terms:
+                t.flows = [(0, complex(t.phase))]
+            return
+        q = [i for i in col_legs if self.legs[i].kind == LEG_F_OUT][0]
+        qb = [i for i in col_legs if self.legs[i].kind == LEG_FB_OUT][0]
+        perms = list(itertools.permutations(glu))
+        self.flow_perms = perms
+        # basis tensors B_sigma[legs in ascending order] = (T^{a_s1} ... T^{a_sn})_{i j}
+        basis = []
+        for s in perms:
+            # build einsum: chain of T's
+            letters = {g: "abcdefgh"[k] for k, g in enumerate(glu)}
+            idx = "ijklmnopq"
+            expr_in = []
+            for k, g in enumerate(s):
+                expr_in.append(letters[g] + idx[k] + idx[k + 1])
+            lab = {q: idx[0], qb: idx[len(s)]}
+            lab.update(letters)
+            out = "".join(lab[l] for l in col_legs)
+            basis.append(np.einsum(",".join(expr_in) + "->" + out, *[_T] * len(s)))
+        nb = len(basis)
+        Bm = np.array([b.ravel() for b in basis])
+        cf = (Bm.conj() @ Bm.T)
+        assert np.allclose(cf.imag, 0)
+        cf = cf.real
+        den = {2: 3, 3: 9, 4: 54}.get(len(glu), None)
+        if den is None:
+            den = 2 * 3 ** len(glu)
+        num = np.rint(cf * den)
+        assert np.allclose(num, cf * den, atol=1e-9), "colour matrix is not integer/den"
+        self.cf_num = num.astype(np.int64)
+        self.cf_den = den
+        cfi = np.linalg.inv(cf)
+        for t in self.terms:
+            ops = [self._col(self.objs[a]) for a in t.args]
+            if t.op == "FFV_AMP":
+                C = self._contract("mcn", _T.transpose(1, 0, 2), ops[0], "m", ops[1], "c", ops[2], "n")
+            elif t.op == "VVV_AMP":
+                C = self._contract("xyz", _F, ops[0], "x", ops[1], "y", ops[2], "z")
+            else:
+                ff = {1: np.einsum("xye,zwe->xyzw", _F, _F), 2: np.einsum("xze,ywe->xyzw", _F, _F),
+                      3: np.einsum("xwe,yze->xyzw", _F, _F)}[t.which]
+                C = self._contract("xyzw", ff, ops[0], "x", ops[1], "y", ops[2], "z", ops[3], "w")
+            arr, labels = C
+            assert labels == col_legs, (labels, col_legs)
+            proj = Bm.conj() @ arr.ravel()
+            c = cfi @ proj
+            assert np.allclose(Bm.T @ c, arr.ravel(), atol=1e-9), "colour factor outside the flow basis"
+            c = c * t.phase
+            flows = []
+            for f in range(nb):
+                if abs(c[f]) < 1e-9:
+                    continue
+                z = complex(round(c[f].real), round(c[f].imag))
+                assert abs(z - c[f]) < 1e-9 and abs(z) == 1.0 and (z.real == 0 or z.imag == 0), c[f]
+                flows.append((f, z))
+            t.flows = flows
+
+    # -- views --------------------------------------------------------------------------------------------------
+    def used_objects(self):
+        """Objects reachable from the closing terms, in dependency order (ids ascending = creation order is NOT
+        dependency-safe for memoised recursion, so sort by leaf count then id)."""
+        used = set()
+
+        def visit(i):
+            if i in used:
+                return
+            used.add(i)
+            for a in self.objs[i].args:
+                visit(a)
+        for t in self.terms:
+            for a in t.args:
+                visit(a)
+        return sorted((self.objs[i] for i in used), key=lambda o: (len(o.legs), o.id))
+
+    def summary(self):
+        return dict(process=self.name, n_diagrams=self.n_diagrams, n_diagrams_4g=self.n_diagrams_4g,
+                    n_terms=len(self.terms), n_flows=len(self.flow_perms),
+                    n_currents=sum(1 for o in self.used_objects() if o.op != "EXT"))

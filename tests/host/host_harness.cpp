@@ -1,0 +1,67 @@
+// TEST-ONLY harness: runs the GENERATED matrix-element programs (csrc/generated/*.inc, csrc/helas.cuh,
+// csrc/me_tasks.cuh) on the CPU by emulating the 32 lanes of a warp one after the other.  It exists so the
+// generator's diagram / colour / phase logic and the vertex routines can be checked against the oracle in the
+// `-m "not gpu"` suite, where no GPU is available.  It is compiled by tests/test_generated_host.py with g++ and
+// is NOT part of the product library: libmadme.so has no CPU path.
+#include <cmath>
+#include <cstring>
+#include <vector>
+#include "../../paper_2211_14056_b200/csrc/generated/epem_mupmum.inc"
+#include "../../paper_2211_14056_b200/csrc/generated/gg_ttx.inc"
+#include "../../paper_2211_14056_b200/csrc/generated/gg_ttxg.inc"
+#include "../../paper_2211_14056_b200/csrc/generated/gg_ttxgg.inc"
+
+using namespace madme;
+
+template <class P> struct Tables;
+#define DEF_TABLES(P, U)                                        \
+  template <> struct Tables<P> {                                \
+    static const int* tasks() { static const int t[] = U##_TASK_TABLE; return t; }      \
+    static const int* masks() { static const int t[] = U##_SUB_MASKS; return t; }       \
+    static const int* kind() { static const int t[] = U##_LEG_KIND; return t; }         \
+    static const int* massive() { static const int t[] = U##_LEG_MASSIVE; return t; }   \
+    static const int* ext_off() { static const int t[] = U##_EXT_OFF; return t; }       \
+  };
+DEF_TABLES(epem_mupmum, EPEM_MUPMUM)
+DEF_TABLES(gg_ttx, GG_TTX)
+DEF_TABLES(gg_ttxg, GG_TTXG)
+DEF_TABLES(gg_ttxgg, GG_TTXGG)
+
+template <class P, int L> struct Levels {
+  static void run(int lane, double* sm, const int* tab, double mass);
+};
+template <class P> void run_levels(double* sm, double mass) {
+  const int* tab = Tables<P>::tasks();
+  if (P::N_LEVELS >= 1) for (int lane = 0; lane < 32; ++lane) P::level0(lane, sm, tab, mass);
+  if constexpr (P::N_LEVELS >= 2) for (int lane = 0; lane < 32; ++lane) P::level1(lane, sm, tab, mass);
+}
+
+template <class P> void eval(const double* mom, double* me2, long long n, double mass, double coupling, double* per_hel) {
+  std::vector<double> sm(P::SMEM_DOUBLES);
+  double g2 = 1;
+  for (int i = 0; i < P::COUPLING_POWER; ++i) g2 *= coupling;
+  const double scale = g2 / (double(P::CF_DEN) * double(P::AVG_DEN));
+  for (long long e = 0; e < n; ++e) {
+    for (int lane = 0; lane < 32; ++lane)
+      me_phase0(lane, sm.data(), mom + e * 4 * P::N_EXT, P::N_EXT, P::N_SUB, Tables<P>::masks(), Tables<P>::kind(),
+                Tables<P>::massive(), Tables<P>::ext_off(), mass);
+    run_levels<P>(sm.data(), mass);
+    double s = 0;
+    for (int h = 0; h < P::N_HEL; ++h) {
+      const double v = P::closings(sm.data(), h);
+      if (per_hel) per_hel[e * P::N_HEL + h] = v * scale;
+      s += v;
+    }
+    me2[e] = s * scale;
+  }
+}
+
+extern "C" int host_me_eval(const char* proc, const double* mom, double* me2, long long n, double mass, double coupling,
+                            double* per_hel) {
+  if (!strcmp(proc, "epem_mupmum")) eval<epem_mupmum>(mom, me2, n, mass, coupling, per_hel);
+  else if (!strcmp(proc, "gg_ttx")) eval<gg_ttx>(mom, me2, n, mass, coupling, per_hel);
+  else if (!strcmp(proc, "gg_ttxg")) eval<gg_ttxg>(mom, me2, n, mass, coupling, per_hel);
+  else if (!strcmp(proc, "gg_ttxgg")) eval<gg_ttxgg>(mom, me2, n, mass, coupling, per_hel);
+  else return -1;
+  return 0;
+}
