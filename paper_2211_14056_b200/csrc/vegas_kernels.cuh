@@ -1,0 +1,184 @@
+// vegas_kernels.cuh — the fused integrand kernel (steps a1-a11) and the deterministic reduction / refinement
+// kernels (a11, a12) of vegas_iterate.  PAPER.md:29,35: Vegas with "the events ... computed in parallel";
+// BASELINE.json:configs[4]: "fused RAMBO + Vegas map + me_eval + weighted accumulation and grid refinement on
+// device".  Grid-update details are DESIGN.md readings R-G7.
+#pragma once
+#include "me_kernel.cuh"
+#include "phase_space.cuh"
+
+namespace madme {
+
+constexpr int VEGAS_MAX_DIM = 4 * PS_MAX_FINAL;
+constexpr double PB_GEV2 = 0.3893793721e9;  // (hbar c)^2 in pb GeV^2
+
+struct VegasArgs {
+  const double* edges;  // dev [n_dim][n_bins+1]
+  int n_dim, n_bins, ps_mode;
+  unsigned long long seed;
+  unsigned iteration;
+  long long first_event, n_ev;
+  double sqrt_s, w0, prefactor;  // prefactor = C / (2 s)
+  double masses[PS_MAX_FINAL];
+  unsigned gluon_mask;
+  double ptj_min, dr_min, mass, scale;
+};
+
+// Fused integrand.  A warp takes 32 consecutive events: lane l generates event l (Philox -> Vegas map -> RAMBO ->
+// cuts; one event per thread), then the warp evaluates |M|^2 of each surviving event cooperatively (one helicity
+// combination per lane) with the momenta handed over by shuffles — nothing goes through HBM in between.
+// Output per event: f (8 B) and the D bin indices packed one byte each (n_bins <= 255) into idx_out[ev][ceil(D/8)].
+template <class P>
+__global__ void __launch_bounds__(256) vegas_integrand_kernel(VegasArgs a, double* __restrict__ f_out,
+                                                              unsigned long long* __restrict__ idx_out, int idx_words) {
+  constexpr int NF = P::N_EXT - 2;
+  extern __shared__ __align__(16) double smem[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, warps = blockDim.x >> 5;
+  double* mom_s = smem + warp * EventSmem<P>::DOUBLES;
+  double* sm = mom_s + 4 * P::N_EXT;
+  const long long n_batches = (a.n_ev + 31) / 32;
+  for (long long b = static_cast<long long>(blockIdx.x) * warps + warp; b < n_batches;
+       b += static_cast<long long>(gridDim.x) * warps) {
+    const long long ev = b * 32 + lane;
+    const bool live = ev < a.n_ev;
+    double y[VEGAS_MAX_DIM], x[VEGAS_MAX_DIM], p[NF][4];
+    unsigned long long packed[2] = {0ull, 0ull};
+    double w = 0.0;
+    bool pass = false;
+    if (live) {
+      philox_fill<VEGAS_MAX_DIM>(a.seed, a.iteration, static_cast<uint64_t>(a.first_event + ev), a.n_dim, y);
+      double jac = 1.0;
+#pragma unroll
+      for (int d = 0; d < VEGAS_MAX_DIM; ++d) {
+        if (d < a.n_dim) {
+          int bin;
+          x[d] = vegas_map_1d(a.edges + d * (a.n_bins + 1), a.n_bins, y[d], jac, bin);
+          packed[d >> 3] |= static_cast<unsigned long long>(bin) << (8 * (d & 7));
+        } else {
+          x[d] = 0.5;
+        }
+      }
+      const double wps = rambo_event<NF>(x, a.sqrt_s, a.masses, a.ps_mode, a.w0, p);
+      pass = passes_cuts<NF>(p, a.gluon_mask, a.ptj_min, a.dr_min);
+      w = jac * wps;
+    }
+    const unsigned todo = __ballot_sync(0xffffffffu, pass);
+    double me2_mine = 0.0;
+    const double e_beam = 0.5 * a.sqrt_s;
+    for (unsigned rest = todo; rest; rest &= rest - 1) {
+      const int src = __ffs(rest) - 1;
+      // hand event src's momenta to the warp: lanes 0..7 write the beams, lane 8+4i+mu writes p[i][mu]
+      if (lane < 8) mom_s[lane] = (lane == 0 || lane == 4) ? e_beam : (lane == 3 ? e_beam : (lane == 7 ? -e_beam : 0.0));
+#pragma unroll
+      for (int i = 0; i < NF; ++i)
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu) {
+          const double v = __shfl_sync(0xffffffffu, p[i][mu], src);
+          if (lane == 8 + 4 * i + mu) mom_s[8 + 4 * i + mu] = v;
+        }
+      __syncwarp();
+      const double r = warp_me2<P>(lane, sm, mom_s, a.mass, a.scale, nullptr);
+      if (lane == src) me2_mine = r;
+      __syncwarp();
+    }
+    if (live) {
+      const double f = pass ? w * me2_mine * a.prefactor : 0.0;
+      f_out[ev] = f;
+      for (int k = 0; k < idx_words; ++k) idx_out[ev * idx_words + k] = packed[k];
+    }
+  }
+}
+
+// a11, deterministic: block c owns the contiguous event chunk [c*chunk, (c+1)*chunk); thread t < n_dim*n_bins owns
+// histogram cell (d, i) = (t / n_bins, t % n_bins) and adds f^2 of the chunk's events in event order; threads
+// n_dim*n_bins + {0,1,2} own sum f, sum f^2 and the pass count.  partial: [gridDim.x][3 + n_dim*n_bins].
+constexpr int VEGAS_RED_TILE = 1024;
+__global__ void __launch_bounds__(512) vegas_reduce_chunks(const double* __restrict__ f, const unsigned long long* __restrict__ idx,
+                                                           int idx_words, int n_dim, int n_bins, long long n_ev, long long chunk,
+                                                           double* __restrict__ partial) {
+  __shared__ double f_s[VEGAS_RED_TILE];
+  __shared__ unsigned long long idx_s[2 * VEGAS_RED_TILE];
+  const int cells = n_dim * n_bins, t = threadIdx.x;
+  const int d = t / n_bins, i = t - d * n_bins;
+  const long long begin = blockIdx.x * chunk, end = min(n_ev, begin + chunk);
+  double acc = 0.0;
+  for (long long base = begin; base < end; base += VEGAS_RED_TILE) {
+    const long long left = end - base;
+    const int n = left < VEGAS_RED_TILE ? static_cast<int>(left) : VEGAS_RED_TILE;
+    for (int e = t; e < n; e += blockDim.x) {
+      f_s[e] = f[base + e];
+      for (int k = 0; k < idx_words; ++k) idx_s[e * idx_words + k] = idx[(base + e) * idx_words + k];
+    }
+    __syncthreads();
+    if (t < cells) {
+      const int word = d >> 3, shift = 8 * (d & 7);
+      for (int e = 0; e < n; ++e) {
+        const double v = f_s[e];
+        if (static_cast<int>((idx_s[e * idx_words + word] >> shift) & 0xffull) == i) acc += v * v;
+      }
+    } else if (t == cells) {
+      for (int e = 0; e < n; ++e) acc += f_s[e];
+    } else if (t == cells + 1) {
+      for (int e = 0; e < n; ++e) acc += f_s[e] * f_s[e];
+    } else if (t == cells + 2) {
+      for (int e = 0; e < n; ++e) acc += (f_s[e] != 0.0) ? 1.0 : 0.0;
+    }
+    __syncthreads();
+  }
+  const int n_out = cells + 3;
+  if (t < cells) partial[static_cast<long long>(blockIdx.x) * n_out + 3 + t] = acc;
+  else if (t < cells + 3) partial[static_cast<long long>(blockIdx.x) * n_out + (t - cells)] = acc;
+}
+// second stage: entry j of sums = partial[0][j] + partial[1][j] + ... in chunk order
+__global__ void vegas_reduce_final(const double* __restrict__ partial, int n_chunks, int n_out, double* __restrict__ sums) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= n_out) return;
+  double acc = 0.0;
+  for (int c = 0; c < n_chunks; ++c) acc += partial[static_cast<long long>(c) * n_out + j];
+  sums[j] = acc;
+}
+
+// a12: grid refinement, one thread per dimension (n_dim * n_bins = 400 numbers: latency, not throughput).
+// smooth (3-point), normalise, damp w = [(r-1)/ln r]^alpha, then walk the cumulative damped weight so that every
+// new bin holds the same share, interpolating linearly inside old bins; end points stay exactly 0 and 1.
+constexpr int VEGAS_MAX_BINS = 255;
+__global__ void vegas_refine_kernel(double* __restrict__ edges, int n_dim, int n_bins, const double* __restrict__ S, double alpha) {
+  const int d = blockIdx.x * blockDim.x + threadIdx.x;
+  if (d >= n_dim || n_bins < 2) return;
+  double* e = edges + static_cast<long long>(d) * (n_bins + 1);
+  const double* Sd = S + static_cast<long long>(d) * n_bins;
+  double w[VEGAS_MAX_BINS], ne[VEGAS_MAX_BINS + 1];
+  double tot = 0.0;
+  for (int i = 0; i < n_bins; ++i) {
+    double s;
+    if (i == 0) s = (Sd[0] + Sd[1]) / 2.0;
+    else if (i == n_bins - 1) s = (Sd[n_bins - 2] + Sd[n_bins - 1]) / 2.0;
+    else s = (Sd[i - 1] + Sd[i] + Sd[i + 1]) / 3.0;
+    w[i] = s;
+    tot += s;
+  }
+  if (!(tot > 0.0)) return;
+  double wtot = 0.0;
+  for (int i = 0; i < n_bins; ++i) {
+    const double r = w[i] / tot;
+    double v;
+    if (r <= 0.0) v = 0.0;
+    else if (r == 1.0) v = 1.0;
+    else v = pow((r - 1.0) / log(r), alpha);
+    w[i] = v;
+    wtot += v;
+  }
+  const double target = wtot / n_bins;
+  int j = 0;
+  double acc = 0.0;
+  ne[0] = 0.0;
+  ne[n_bins] = 1.0;
+  for (int i = 1; i < n_bins; ++i) {
+    const double need = i * target;
+    while (j < n_bins - 1 && acc + w[j] < need) { acc += w[j]; ++j; }
+    const double frac = (w[j] > 0.0) ? (need - acc) / w[j] : 0.0;
+    ne[i] = e[j] + frac * (e[j + 1] - e[j]);
+  }
+  for (int i = 0; i <= n_bins; ++i) e[i] = ne[i];
+}
+
+}  // namespace madme

@@ -1,0 +1,64 @@
+"""The build-time generator (gen/) and the vertex library (csrc/helas.cuh), checked WITHOUT a GPU: the generated
+programs are compiled with g++ (tests/host/host_harness.cpp emulates the 32 lanes sequentially) and compared with
+the oracle.  The harness is test-only; libmadme.so has no CPU path."""
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+import pytest
+
+from oracle import ref
+from paper_2211_14056_b200.gen import diagrams, emit
+from paper_2211_14056_b200.workloads import BY_NAME, PARAMS
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+@pytest.fixture(scope="module")
+def host():
+    emit.emit_all()
+    so = os.path.join(HERE, "host", "libhost_harness.so")
+    src = os.path.join(HERE, "host", "host_harness.cpp")
+    subprocess.check_call(["g++", "-std=c++17", "-O1", "-shared", "-fPIC", "-o", so, src])
+    lib = C.CDLL(so)
+    lib.host_me_eval.argtypes = [C.c_char_p, C.c_void_p, C.c_void_p, C.c_longlong, C.c_double, C.c_double, C.c_void_p]
+    return lib
+
+
+def _momenta(cfg, n):
+    w = BY_NAME[cfg]
+    r = ref.philox_uniform(w.seed, 0, 0, w.n_dim, n)
+    return ref.rambo_generate(r, w.sqrt_s, w.masses, w.ps_mode)[0]
+
+
+@pytest.mark.parametrize("name,nd,n4,nt,nf", [("gg_ttx", 3, 0, 3, 2), ("gg_ttxg", 16, 1, 18, 6), ("gg_ttxgg", 123, 18, 159, 24)])
+def test_generator_counts(name, nd, n4, nt, nf):
+    """PAPER.md:57-58 (36 = 16 + 4x5, 267 = 123 + 4x36) and tests/golden/diagram_counts.txt."""
+    s = diagrams.Program(name).summary()
+    assert (s["n_diagrams"], s["n_diagrams_4g"], s["n_terms"], s["n_flows"]) == (nd, n4, nt, nf)
+
+
+def test_generator_colour_matrix_golden():
+    rows = {}
+    for line in open(os.path.join(HERE, "golden", "colour_matrix_rows.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        n, den, row, _ = [x.strip() for x in line.split("|")]
+        rows[int(n)] = (int(den), [int(x) for x in row.split()])
+    for name, n in (("gg_ttx", 2), ("gg_ttxg", 3), ("gg_ttxgg", 4)):
+        P = diagrams.Program(name)
+        assert P.cf_den == rows[n][0]
+        assert list(P.cf_num[0]) == rows[n][1]
+
+
+@pytest.mark.parametrize("cfg,n", [("config0", 64), ("config1", 64), ("config2", 32), ("config3", 12)])
+def test_generated_program_matches_oracle(host, cfg, n):
+    w = BY_NAME[cfg]
+    mom = _momenta(cfg, n)
+    out = np.empty(n)
+    qed = w.process == "epem_mupmum"
+    g = np.sqrt(4 * np.pi * (PARAMS["alpha_em"] if qed else PARAMS["alpha_s"]))
+    assert host.host_me_eval(w.process.encode(), mom.ctypes.data, out.ctypes.data, n, 0.0 if qed else PARAMS["m_top"], g, None) == 0
+    expect = ref.MatrixElementRef(w.process).eval(mom)
+    assert np.max(np.abs(out / expect - 1)) < 1e-11
