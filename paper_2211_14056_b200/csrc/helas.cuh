@@ -295,6 +295,27 @@ ME_HD cplx ffv_amp(const wf4& q, const wf4& V, const wf4& p) {
   r = cfma(q.c[3], x.c[3], r);
   return r;
 }
+// Propagator-cut closing: J += i^K (U . C), U the open (un-propagated) current over one half of the legs, C the
+// propagated current over the other half.  MINK: vector line, Minkowski contraction (+,-,-,-); otherwise a fermion
+// line, plain sum over the four spinor components.  Every component is 4 FMAs straight into the flow accumulator.
+template <int K> ME_HD void cacc(double& jr, double& ji, cplx a, cplx b) {
+  if (K == 0) {        // + a b
+    jr = fma(a.re, b.re, fma(-a.im, b.im, jr)); ji = fma(a.re, b.im, fma(a.im, b.re, ji));
+  } else if (K == 2) { // - a b
+    jr = fma(-a.re, b.re, fma(a.im, b.im, jr)); ji = fma(-a.re, b.im, fma(-a.im, b.re, ji));
+  } else if (K == 1) { // + i a b
+    jr = fma(-a.re, b.im, fma(-a.im, b.re, jr)); ji = fma(a.re, b.re, fma(-a.im, b.im, ji));
+  } else {             // - i a b
+    jr = fma(a.re, b.im, fma(a.im, b.re, jr)); ji = fma(-a.re, b.re, fma(a.im, b.im, ji));
+  }
+}
+template <int K, bool MINK> ME_HD void dot_acc(double& jr, double& ji, const wf4& u, const wf4& c) {
+  cacc<K>(jr, ji, u.c[0], c.c[0]);
+  cacc<MINK ? ((K + 2) & 3) : K>(jr, ji, u.c[1], c.c[1]);
+  cacc<MINK ? ((K + 2) & 3) : K>(jr, ji, u.c[2], c.c[2]);
+  cacc<MINK ? ((K + 2) & 3) : K>(jr, ji, u.c[3], c.c[3]);
+}
+
 // [VVV1_0-like]  (X.Y)((K_X-K_Y).Z) + (Y.Z)((K_Y-K_Z).X) + (Z.X)((K_Z-K_X).Y)
 ME_HD cplx vvv_amp(const wf4& X, const vec4& KX, const wf4& Y, const vec4& KY, const wf4& Z, const vec4& KZ) {
   vec4 dxy, dyz, dzx;

@@ -6,7 +6,7 @@
 // off-shell current is computed once per combination of the helicities of ITS OWN legs ("helicity recycling",
 // me_tasks.cuh) and HBM sees 32 n_ext bytes in and 8 bytes out per event.
 //
-// Steps: a5 me_phase0 -> a6 P::level*  -> a7-a9 P::closings(h) per lane -> a10 warp sum.
+// Steps: a5 me_phase0 -> a6 P::stage(s) -> a7-a9 P::closings(h) per lane -> a10 warp sum (x2: parity).
 #pragma once
 #include "generated/epem_mupmum.inc"
 #include "generated/gg_ttx.inc"
@@ -19,12 +19,14 @@ namespace madme {
 template <class P> struct Tables;
 #define MADME_DEF_TABLES(P, U)                                                  \
   __device__ const int U##_tasks_d[] = U##_TASK_TABLE;                          \
+  __device__ const int U##_combos_d[] = U##_COMBO_TABLE;                        \
   __device__ const int U##_masks_d[] = U##_SUB_MASKS;                           \
   __device__ const int U##_kind_d[] = U##_LEG_KIND;                             \
   __device__ const int U##_massive_d[] = U##_LEG_MASSIVE;                       \
   __device__ const int U##_extoff_d[] = U##_EXT_OFF;                            \
   template <> struct Tables<P> {                                                \
     static __device__ __forceinline__ const int* tasks() { return U##_tasks_d; }     \
+    static __device__ __forceinline__ const int* combos() { return U##_combos_d; }   \
     static __device__ __forceinline__ const int* masks() { return U##_masks_d; }     \
     static __device__ __forceinline__ const int* kind() { return U##_kind_d; }       \
     static __device__ __forceinline__ const int* massive() { return U##_massive_d; } \
@@ -38,10 +40,14 @@ MADME_DEF_TABLES(gg_ttxgg, GG_TTXGG)
 // doubles of shared memory per event: momenta [n_ext][4] + the generated scratch layout, 16-byte aligned
 template <class P> struct EventSmem { static constexpr int DOUBLES = ((4 * P::N_EXT + P::SMEM_DOUBLES + 1) / 2) * 2; };
 
-template <class P> __device__ __forceinline__ void run_levels(int lane, double* sm, double mass) {
+template <class P> __device__ __forceinline__ void run_stages(int lane, double* sm, double mass) {
   const int* tab = Tables<P>::tasks();
-  if constexpr (P::N_LEVELS >= 1) { P::level0(lane, sm, tab, mass); __syncwarp(); }
-  if constexpr (P::N_LEVELS >= 2) { P::level1(lane, sm, tab, mass); __syncwarp(); }
+  const int* ctab = Tables<P>::combos();
+#pragma unroll
+  for (int s = 0; s < P::N_STAGES; ++s) {
+    P::stage(s, lane, sm, tab, ctab, mass);
+    __syncwarp();
+  }
 }
 
 // |M|^2 of the event whose momenta sit in mom_s (shared, [n_ext][4]); every lane returns the helicity-summed,
@@ -51,16 +57,20 @@ __device__ __forceinline__ double warp_me2(int lane, double* sm, const double* m
   me_phase0(lane, sm, mom_s, P::N_EXT, P::N_SUB, Tables<P>::masks(), Tables<P>::kind(), Tables<P>::massive(),
             Tables<P>::ext_off(), mass);
   __syncwarp();
-  run_levels<P>(lane, sm, mass);
+  run_stages<P>(lane, sm, mass);
   double s = 0.0;
-  for (int h = lane; h < P::N_HEL; h += 32) {
+  for (int h = lane; h < P::N_HEL_EVAL; h += 32) {
     const double v = P::closings(sm, h);
-    if (hel_out) hel_out[h] = v * scale;
+    if (hel_out) {  // full index: leg 0 at +1 is bit 0; the parity partner has every helicity flipped
+      const int hf = (h << 1) | 1;
+      hel_out[hf] = v * scale;
+      hel_out[(P::N_HEL - 1) ^ hf] = v * scale;
+    }
     s += v;
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-  return s * scale;
+  return 2.0 * s * scale;
 }
 
 // MAXWARPS bounds the CTA size (register budget); the actual events-per-CTA is blockDim.x / 32 (a run-time knob:

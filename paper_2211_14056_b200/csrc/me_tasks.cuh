@@ -7,15 +7,19 @@
 //
 // Scratch layout of one event (doubles), produced by gen/emit.py for each process:
 //   subset blocks  : 8 doubles per used leg subset S:  K_S[4], 1/K_S^2, 1/(K_S^2 - m_t^2), pad, pad
-//   wavefunctions  : object o over the leg set S has 2^|S| helicity variants ("helicity recycling":
-//                    a current depends only on the helicities of its own legs), stored as
+//   wavefunctions  : object o over the leg set S has one helicity variant per combination of the helicities of
+//                    ITS OWN legs ("helicity recycling"), stored as
 //                    [component c = 0..3][variant v][re, im]   ->  double offset  OFF_o + 2*(c*nv + v)
 //                    so that the 32 lanes' 16-byte loads of one component fall into <= 128 contiguous bytes.
-// Variant index v = sum_k b_{l_k} 2^k over the legs l_0 < l_1 < ... of S, b = 0 for helicity -1, 1 for +1.
+//   Leg 0 is fixed at helicity +1 (parity: |M(-h)|^2 = |M(h)|^2, the sum is doubled at the end), so
+//   variant index v = sum_k b_{l_k} 2^k over the legs l_0 < l_1 < ... of S OTHER THAN LEG 0, b = 0 for helicity -1,
+//   1 for +1, and nv = 2^(number of those legs).
+//   The first PERSISTENT_DOUBLES hold what the closings read; the rest is a transient region that the top-level
+//   currents of successive rounds reuse once their colour-ordered combinations have been formed.
 //
 // The steps:
 //   a5  me_phase0      : K_S and propagator denominators for every subset, external wavefunctions
-//   a6  me_run_level   : off-shell currents, one (current, variant) task per lane, level by level
+//   a6  P::stage(s)    : off-shell currents and their combinations, one (object, variant) task per lane, stage by stage
 //   a7-a10             : generated straight-line code (csrc/generated/*.inc), one helicity per lane
 #pragma once
 #include "helas.cuh"
@@ -24,7 +28,13 @@ namespace madme {
 
 constexpr int ME_TASK_INTS = 16;
 // task row: 0 out, 1 out_stride, 2 a, 3 a_stride, 4 b, 5 b_stride, 6 c, 7 c_stride,
-//           8 ksub_out, 9 ksub_a, 10 ksub_b, 11 massive, 12 out2, 13 out3, 14 ksub_c, 15 pad
+//           8 ksub_out, 9 ksub_a, 10 ksub_b, 11 massive, 12 out2, 13 out3, 14 ksub_c, 15 unpropagated
+// combo row: 0 out, 1 stride, 2 n, then n x (input offset, k) : out = sum_j i^k_j in_j
+#if defined(__CUDA_ARCH__)
+#define ME_FENCE() asm volatile("" ::: "memory")  // keeps ptxas from hoisting every shared-memory load to the top
+#else
+#define ME_FENCE()
+#endif
 enum MeOp { OP_FFV_ROW = 0, OP_FFV_COL = 1, OP_FFV_VEC = 2, OP_VVV = 3, OP_VVVV = 4 };
 
 ME_HD wf4 ld_wf(const double* p, int stride) {
@@ -84,8 +94,12 @@ ME_HD void me_phase0(int lane, double* sm, const double* mom, int n_ext, int n_s
   for (int l = lane; l < n_ext; l += 32) {
     wf4 w[2];
     external_wavefunction(leg_kind[l], mom + 4 * l, leg_massive[l] ? mass : 0.0, w);
-    st_wf(sm + ext_off[l], 4, w[0]);
-    st_wf(sm + ext_off[l] + 2, 4, w[1]);
+    if (l == 0) {
+      st_wf(sm + ext_off[0], 2, w[1]);  // leg 0: helicity +1 only (parity)
+    } else {
+      st_wf(sm + ext_off[l], 4, w[0]);
+      st_wf(sm + ext_off[l] + 2, 4, w[1]);
+    }
   }
 }
 
@@ -95,18 +109,22 @@ ME_HD void me_run_task(int op, double* sm, const int* t, double mass) {
   const wf4 B = ld_wf(sm + t[4], t[5]);
   const double* ks = sm + t[8];
   const double m = t[11] ? mass : 0.0;
+  const bool open = t[15] != 0;  // the current stops at its vertex: no propagator (the U side of a propagator cut)
+  const double invk2 = open ? 1.0 : ks[4];
   if (op == OP_FFV_ROW) {
-    st_wf(sm + t[0], t[1], ffv_row(A, B, ld_k(ks), m, t[11] ? ks[5] : ks[4]));
+    const wf4 x = slash_row(A, B);
+    st_wf(sm + t[0], t[1], open ? x : prop_row(ld_k(ks), -1.0, m, t[11] ? ks[5] : ks[4], x));
   } else if (op == OP_FFV_COL) {
-    st_wf(sm + t[0], t[1], ffv_col(A, B, ld_k(ks), m, t[11] ? ks[5] : ks[4]));
+    const wf4 x = slash_col(B, A);
+    st_wf(sm + t[0], t[1], open ? x : prop_col(ld_k(ks), 1.0, m, t[11] ? ks[5] : ks[4], x));
   } else if (op == OP_FFV_VEC) {
-    st_wf(sm + t[0], t[1], ffv_vec(A, B, ks[4]));
+    st_wf(sm + t[0], t[1], ffv_vec(A, B, invk2));
   } else if (op == OP_VVV) {
-    st_wf(sm + t[0], t[1], vvv_vec(A, ld_k(sm + t[9]), B, ld_k(sm + t[10]), ks[4]));
+    st_wf(sm + t[0], t[1], vvv_vec(A, ld_k(sm + t[9]), B, ld_k(sm + t[10]), invk2));
   } else {
     const wf4 C = ld_wf(sm + t[6], t[7]);
     wf4 t1, t2, t3;
-    vvvv_vec(A, B, C, ks[4], t1, t2, t3);
+    vvvv_vec(A, B, C, invk2, t1, t2, t3);
     st_wf(sm + t[0], t[1], t1);
     st_wf(sm + t[12], t[1], t2);
     st_wf(sm + t[13], t[1], t3);
@@ -116,6 +134,24 @@ ME_HD void me_run_task(int op, double* sm, const int* t, double mass) {
 // all tasks [begin, end) of one (level, op) group, 32 lanes at a time
 ME_HD void me_run_group(int op, int lane, double* sm, const int* tab, int begin, int end, double mass) {
   for (int i = begin + lane; i < end; i += 32) me_run_task(op, sm, tab + ME_TASK_INTS * i, mass);
+}
+
+// colour-ordered combinations: out = sum_j i^{k_j} in_j (same leg set, same variant)
+ME_HD void me_run_combos(int lane, double* sm, const int* ctab, int begin, int end) {
+  for (int i = begin + lane; i < end; i += 32) {
+    const int* t = ctab + ME_TASK_INTS * i;
+    wf4 acc = ld_wf(sm + t[3], t[1]);  // first member always enters with coefficient 1
+    for (int j = 1; j < t[2]; ++j) {
+      const wf4 x = ld_wf(sm + t[3 + 2 * j], t[1]);
+      const int k = t[4 + 2 * j];
+      for (int c = 0; c < 4; ++c) {
+        const double re = (k & 1) ? -x.c[c].im : x.c[c].re, im = (k & 1) ? x.c[c].re : x.c[c].im;
+        acc.c[c].re += (k & 2) ? -re : re;
+        acc.c[c].im += (k & 2) ? -im : im;
+      }
+    }
+    st_wf(sm + t[0], t[1], acc);
+  }
 }
 
 }  // namespace madme

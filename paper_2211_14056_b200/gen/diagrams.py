@@ -14,6 +14,18 @@ splitting the legs n/2 | n/2 — go to the side that holds leg 0).  The hanging 
 currents; structurally identical subtrees are shared between diagrams.  A subtree / diagram containing a
 four-gluon vertex splits into three colour-pure terms.
 
+Propagator-cut closings.  When n is even, a diagram whose centroid vertex has a hanging subtree C with exactly
+n/2 legs (it never holds leg 0) is not evaluated at that vertex: the other subtrees of the vertex are merged
+into the UN-propagated current U over the complementary n/2 legs (it holds leg 0) and the diagram is the plain
+contraction U . C (a 4-component dot product instead of a vertex).  `factorise()` then sums, per colour flow,
+the U's and the C's of one leg split into colour-ordered combinations first (every current depends only on the
+helicities of its own n/2 legs), so that a flow receives ONE dot product per split — the colour-ordered
+recursion is recovered from the Feynman diagrams, not assumed.
+
+Parity.  QCD and QED conserve parity: |M(-h)|^2 = |M(h)|^2 for the colour-summed squared amplitude, so only the
+helicity combinations with leg 0 at +1 are evaluated and the sum is doubled (a DECLARED 2x
+saving; the flops reported are the ones executed).  Objects holding leg 0 therefore have half the variants.
+
 Powers of i and of the coupling carried by vertices and propagators are NOT applied numerically: every
 object carries a symbolic phase in {1, i, -1, -i}, which ends up in the flow coefficient of the term.
 Feynman rules, all momenta incoming:
@@ -80,10 +92,11 @@ _T, _F = su3()
 
 
 class Obj:
-    __slots__ = ("id", "legs", "type", "op", "args", "phase", "_col", "skel", "has4g")
+    __slots__ = ("id", "legs", "type", "op", "args", "phase", "_col", "skel", "has4g", "prop")
 
-    def __init__(self, id, legs, type, op, args, phase):
+    def __init__(self, id, legs, type, op, args, phase, prop=True):
         self.id, self.legs, self.type, self.op, self.args, self.phase = id, tuple(sorted(legs)), type, op, args, phase
+        self.prop = prop    # False: the current stops at its vertex (no propagator): the U side of a propagator cut
         self._col = None
         self.skel = None    # structural key: the three colour terms of one 4g subtree share it
         self.has4g = False
@@ -129,6 +142,9 @@ class Program:
         self.n_diagrams_4g = 0
         self._ext = {}
         self._diagrams = {}
+        self._unprop = {}
+        self.combos = []     # colour-ordered sums of half-split currents (factorise)
+        self.dots = []       # (flow, combo/object id of U side, of C side, phase z, 'V'|'F')
         for i, leg in enumerate(self.legs):
             if leg.kind in (LEG_V_IN, LEG_V_OUT):
                 t = ("V", leg.flavour)
@@ -139,10 +155,11 @@ class Program:
             self._ext[i] = self._new((i,), t, "EXT", (), 1)
         self._close()
         self._colour()
+        self.factorise()
 
     # -- enumeration ------------------------------------------------------------------------------------------
-    def _new(self, legs, type, op, args, phase):
-        o = Obj(len(self.objs), legs, type, op, args, phase)
+    def _new(self, legs, type, op, args, phase, prop=True):
+        o = Obj(len(self.objs), legs, type, op, args, phase, prop)
         o.skel = (op[:4] if op.startswith("VVVV") else op, tuple(sorted(legs)), tuple(self.objs[a].skel for a in args))
         o.has4g = op.startswith("VVVV") or any(self.objs[a].has4g for a in args)
         self.objs.append(o)
@@ -208,6 +225,10 @@ class Program:
                 continue
             for combo in itertools.product(*[self.subtrees(p) for p in parts]):
                 if all(o.type == ("V", "g") for o in combo):
+                    half = [o for o in combo if 2 * len(o.legs) == n]
+                    if half:
+                        self._close_cut(half[0], [o for o in combo if o is not half[0]], True)
+                        continue
                     d = self._count_diagram(combo, True)
                     ph = np.prod([o.phase for o in combo]) * (-1j)  # vertex -i g^2
                     for w in (1, 2, 3):
@@ -222,8 +243,58 @@ class Program:
                 self.n_diagrams_4g += 1
         return self._diagrams[key]
 
+    # the un-propagated current over the legs of X u Y (u Z): the vertex without the propagator behind it
+    def _unprop_current(self, parts):
+        key = tuple(sorted(o.id for o in parts))
+        if key in self._unprop:
+            return self._unprop[key]
+        legs = tuple(sorted(l for o in parts for l in o.legs))
+        res = []
+        if len(parts) == 2:
+            A, B = parts
+            for X, Y in ((A, B), (B, A)):
+                kx, fx = X.type
+                ky, fy = Y.type
+                if kx == "O" and ky == "V" and VECTOR_OF[fx] == fy:     # vertex i g
+                    res.append(self._new(legs, X.type, "FFV_ROW", (X.id, Y.id), X.phase * Y.phase * 1j, prop=False))
+                if kx == "I" and ky == "V" and VECTOR_OF[fx] == fy:
+                    res.append(self._new(legs, X.type, "FFV_COL", (X.id, Y.id), X.phase * Y.phase * 1j, prop=False))
+                if kx == "O" and ky == "I" and fx == fy:
+                    res.append(self._new(legs, ("V", VECTOR_OF[fx]), "FFV_VEC", (X.id, Y.id), X.phase * Y.phase * 1j, prop=False))
+            if A.type == B.type == ("V", "g"):                          # vertex g (real)
+                res.append(self._new(legs, ("V", "g"), "VVV", (A.id, B.id), A.phase * B.phase, prop=False))
+        else:
+            A, B, C = parts
+            if A.type == B.type == C.type == ("V", "g"):                # vertex -i g^2
+                ph = A.phase * B.phase * C.phase * (-1j)
+                for w in (1, 2, 3):
+                    res.append(self._new(legs, ("V", "g"), "VVVV%d" % w, (A.id, B.id, C.id), ph, prop=False))
+        self._unprop[key] = res
+        return res
+
+    def _close_cut(self, big, others, closing_4g):
+        """Diagram = (vertex of `others`, left open) . (propagated current `big` over n/2 legs)."""
+        made = False
+        for U in self._unprop_current(others):
+            ku, fu = U.type
+            kc, fc = big.type
+            if ku == "V" and kc == "V" and fu == fc:
+                kind = "V"
+            elif {ku, kc} == {"O", "I"} and fu == fc:
+                kind = "F"
+            else:
+                continue
+            if not made:
+                d = self._count_diagram(tuple(others) + (big,), closing_4g)
+                made = True
+            self.terms.append(Term("DOT_" + kind, (U.id, big.id), U.phase * big.phase, 0, d))
+
     def _close3(self, A, B, C):
         objs = (A, B, C)
+        half = [o for o in objs if 2 * len(o.legs) == self.n]
+        if half:
+            self._close_cut(half[0], [o for o in objs if o is not half[0]], False)
+            return
         kinds = [o.type[0] for o in objs]
         if sorted(kinds) == ["I", "O", "V"]:
             O = objs[kinds.index("O")]
@@ -302,7 +373,7 @@ class Program:
             self.cf_num = np.array([[1]], dtype=np.int64)
             self.cf_den = 1
             for t in self.terms:
-                t.flows = [(0, complex(t.phase))]
+                t.flows = [(0, complex(np.round(t.phase)))]
             return
         q = [i for i in col_legs if self.legs[i].kind == LEG_F_OUT][0]
         qb = [i for i in col_legs if self.legs[i].kind == LEG_FB_OUT][0]
@@ -340,6 +411,10 @@ class Program:
                 C = self._contract("mcn", _T.transpose(1, 0, 2), ops[0], "m", ops[1], "c", ops[2], "n")
             elif t.op == "VVV_AMP":
                 C = self._contract("xyz", _F, ops[0], "x", ops[1], "y", ops[2], "z")
+            elif t.op == "DOT_V":   # gluon propagator: delta^{ab}
+                C = self._contract("xy", np.eye(8), ops[0], "x", ops[1], "y")
+            elif t.op == "DOT_F":   # quark propagator: delta_{ij}
+                C = self._contract("xy", np.eye(3), ops[0], "x", ops[1], "y")
             else:
                 ff = {1: np.einsum("xye,zwe->xyzw", _F, _F), 2: np.einsum("xze,ywe->xyzw", _F, _F),
                       3: np.einsum("xwe,yze->xyzw", _F, _F)}[t.which]
@@ -359,6 +434,63 @@ class Program:
                 flows.append((f, z))
             t.flows = flows
 
+    # -- propagator-cut closings: colour-ordered combinations -------------------------------------------------
+    def _combo(self, members):
+        """members: [(obj id, coefficient in {+-1, +-i})], first coefficient 1.  A single member is the object itself."""
+        if len(members) == 1:
+            assert members[0][1] == 1
+            return members[0][0]
+        key = tuple(members)
+        if key not in self._combo_ids:
+            first = self.objs[members[0][0]]
+            o = self._new(first.legs, first.type, "COMBO", tuple(m[0] for m in members), 1, prop=first.prop)
+            self.combo_coefs[o.id] = [m[1] for m in members]
+            self.combos.append(o)
+            self._combo_ids[key] = o.id
+        return self._combo_ids[key]
+
+    def factorise(self):
+        """Per leg split and colour flow f: sum_{ij} c^f_ij U_i.C_j = sum_r z_r (sum_i a_i U_i).(sum_j b_j C_j)
+        by exact rank-1 peeling of the {0,+-1,+-i} matrix c^f; the sums over i and j are taken once per helicity
+        variant of n/2 legs, the dot product once per helicity combination."""
+        self._combo_ids, self.combo_coefs = {}, {}
+        nf = len(self.flow_perms)
+        groups = {}
+        for t in self.terms:
+            if t.op.startswith("DOT"):
+                groups.setdefault(self.objs[t.args[0]].legs, []).append(t)
+        unit = lambda z: abs(abs(z) - 1) < 1e-9 and (abs(z.real) < 1e-9 or abs(z.imag) < 1e-9)
+        rnd = lambda z: complex(round(z.real), round(z.imag))
+        for legs in sorted(groups):
+            terms = groups[legs]
+            us = sorted({t.args[0] for t in terms})
+            cs = sorted({t.args[1] for t in terms})
+            kind = terms[0].op[-1]
+            M = np.zeros((nf, len(us), len(cs)), dtype=complex)
+            for t in terms:
+                for f, z in t.flows:
+                    M[f, us.index(t.args[0]), cs.index(t.args[1])] += z
+            for f in range(nf):
+                R = M[f].copy()
+                guard = 0
+                while np.any(np.abs(R) > 1e-9):
+                    guard += 1
+                    assert guard <= 16
+                    i0, j0 = [int(x) for x in np.argwhere(np.abs(R) > 1e-9)[0]]
+                    piv = R[i0, j0]
+                    a = R[:, j0] / piv          # a[i0] = 1
+                    b = R[i0, :] / piv          # b[j0] = 1
+                    R = R - piv * np.outer(a, b)
+                    R[np.abs(R) < 1e-9] = 0
+                    ma = [(us[i], rnd(a[i])) for i in range(len(us)) if abs(a[i]) > 1e-9]
+                    mb = [(cs[j], rnd(b[j])) for j in range(len(cs)) if abs(b[j]) > 1e-9]
+                    assert unit(piv) and all(unit(z) for _, z in ma + mb), (piv, ma, mb)
+                    # normalise so that the first member has coefficient 1; the phases go to the dot product
+                    za, zb = ma[0][1], mb[0][1]
+                    ma = [(o, rnd(z / za)) for o, z in ma]
+                    mb = [(o, rnd(z / zb)) for o, z in mb]
+                    self.dots.append((f, self._combo(ma), self._combo(mb), rnd(piv * za * zb), kind))
+
     # -- views --------------------------------------------------------------------------------------------------
     def used_objects(self):
         """Objects reachable from the closing terms, in dependency order (ids ascending = creation order is NOT
@@ -372,11 +504,17 @@ class Program:
             for a in self.objs[i].args:
                 visit(a)
         for t in self.terms:
-            for a in t.args:
-                visit(a)
-        return sorted((self.objs[i] for i in used), key=lambda o: (len(o.legs), o.id))
+            if not t.op.startswith("DOT"):      # DOT terms are evaluated through self.dots
+                for a in t.args:
+                    visit(a)
+        for _, u, c, _, _ in self.dots:
+            visit(u)
+            visit(c)
+        return sorted((self.objs[i] for i in used), key=lambda o: (len(o.legs), o.op == "COMBO", o.id))
 
     def summary(self):
         return dict(process=self.name, n_diagrams=self.n_diagrams, n_diagrams_4g=self.n_diagrams_4g,
                     n_terms=len(self.terms), n_flows=len(self.flow_perms),
-                    n_currents=sum(1 for o in self.used_objects() if o.op != "EXT"))
+                    n_currents=sum(1 for o in self.used_objects() if o.op not in ("EXT", "COMBO")),
+                    n_combos=sum(1 for o in self.used_objects() if o.op == "COMBO"), n_dots=len(self.dots),
+                    n_vertex_closings=sum(1 for t in self.terms if not t.op.startswith("DOT")))

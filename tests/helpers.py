@@ -47,3 +47,14 @@ def closed_form_gg_ttx(mom, alpha_s, m):
     gs2 = 4 * np.pi * alpha_s
     t1, t2, rho = (m * m - t) / s, (m * m - u) / s, 4 * m * m / s
     return gs2 ** 2 * (1 / (6 * t1 * t2) - 3.0 / 8) * (t1 ** 2 + t2 ** 2 + rho - rho ** 2 / (4 * t1 * t2))
+
+
+def me_tolerance(mom, rtol=1e-10):
+    """Per-event relative tolerance for |M|^2 comparisons: rtol (BASELINE.json:north_star) for physical input, widened
+    by the input's own momentum non-conservation delta = max|sum k| / sqrt(s).  |M|^2 is only defined on momentum-
+    conserving, on-shell input; classic RAMBO with n = 2 loses conservation to ~1e-9 on the few events whose two
+    generated massless vectors are nearly collinear (huge conformal boost), and there every evaluation (oracle,
+    closed form, kernels) is a different function of the unphysical input.  DESIGN.md §Tolerances."""
+    tot = mom[:, :2].sum(1) - mom[:, 2:].sum(1)
+    delta = np.abs(tot).max(1) / (mom[:, 0, 0] + mom[:, 1, 0])
+    return rtol + 20.0 * delta

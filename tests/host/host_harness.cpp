@@ -17,6 +17,7 @@ template <class P> struct Tables;
 #define DEF_TABLES(P, U)                                        \
   template <> struct Tables<P> {                                \
     static const int* tasks() { static const int t[] = U##_TASK_TABLE; return t; }      \
+    static const int* combos() { static const int t[] = U##_COMBO_TABLE; return t; }    \
     static const int* masks() { static const int t[] = U##_SUB_MASKS; return t; }       \
     static const int* kind() { static const int t[] = U##_LEG_KIND; return t; }         \
     static const int* massive() { static const int t[] = U##_LEG_MASSIVE; return t; }   \
@@ -27,13 +28,9 @@ DEF_TABLES(gg_ttx, GG_TTX)
 DEF_TABLES(gg_ttxg, GG_TTXG)
 DEF_TABLES(gg_ttxgg, GG_TTXGG)
 
-template <class P, int L> struct Levels {
-  static void run(int lane, double* sm, const int* tab, double mass);
-};
 template <class P> void run_levels(double* sm, double mass) {
-  const int* tab = Tables<P>::tasks();
-  if (P::N_LEVELS >= 1) for (int lane = 0; lane < 32; ++lane) P::level0(lane, sm, tab, mass);
-  if constexpr (P::N_LEVELS >= 2) for (int lane = 0; lane < 32; ++lane) P::level1(lane, sm, tab, mass);
+  for (int s = 0; s < P::N_STAGES; ++s)
+    for (int lane = 0; lane < 32; ++lane) P::stage(s, lane, sm, Tables<P>::tasks(), Tables<P>::combos(), mass);
 }
 
 template <class P> void eval(const double* mom, double* me2, long long n, double mass, double coupling, double* per_hel) {
@@ -47,12 +44,12 @@ template <class P> void eval(const double* mom, double* me2, long long n, double
                 Tables<P>::massive(), Tables<P>::ext_off(), mass);
     run_levels<P>(sm.data(), mass);
     double s = 0;
-    for (int h = 0; h < P::N_HEL; ++h) {
+    for (int h = 0; h < P::N_HEL_EVAL; ++h) {
       const double v = P::closings(sm.data(), h);
-      if (per_hel) per_hel[e * P::N_HEL + h] = v * scale;
+      if (per_hel) per_hel[e * P::N_HEL_EVAL + h] = v * scale;
       s += v;
     }
-    me2[e] = s * scale;
+    me2[e] = 2.0 * s * scale;
   }
 }
 
