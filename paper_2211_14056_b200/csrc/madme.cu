@@ -407,7 +407,8 @@ int vegas_integrand(me_handle* h, const vegas_grid* g, double sqrt_s, long long 
   const int nf = h->n_ext - 2, D = g->n_dim, nb = g->n_bins;
   if ((g->ps_mode != 0 && g->ps_mode != 1) || D != (g->ps_mode == 0 ? 4 * nf : 3 * nf - 4))
     return fail(ME_EDIM, "vegas_integrand: n_dim must be 4 n_final (ps_mode 0) or 3 n_final - 4 (ps_mode 1)%s%s");
-  if (nb < 1 || nb > VEGAS_MAX_BINS || D * nb + 3 > 512) return fail(ME_EDIM, "vegas_integrand: n_bins 1..255 and n_dim*n_bins <= 509%s%s");
+  if (nb < 1 || nb > VEGAS_MAX_BINS || D * nb + 3 > 512 * VEGAS_RED_PER_THREAD)
+    return fail(ME_EDIM, "vegas_integrand: n_bins 1..255 and n_dim*n_bins <= 2045%s%s");
   if (!(sqrt_s > 2.0 * h->par.m_top)) return fail(ME_EINVAL, "vegas_integrand: sqrt_s below threshold%s%s");
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const int n_out = 3 + D * nb, words = (D + 7) / 8;

@@ -88,19 +88,29 @@ __global__ void __launch_bounds__(256) vegas_integrand_kernel(VegasArgs a, doubl
   }
 }
 
-// a11, deterministic: block c owns the contiguous event chunk [c*chunk, (c+1)*chunk); thread t < n_dim*n_bins owns
-// histogram cell (d, i) = (t / n_bins, t % n_bins) and adds f^2 of the chunk's events in event order; threads
-// n_dim*n_bins + {0,1,2} own sum f, sum f^2 and the pass count.  partial: [gridDim.x][3 + n_dim*n_bins].
+// a11, deterministic: block c owns the contiguous event chunk [c*chunk, (c+1)*chunk); output entry j (j = 0,1,2: sum f,
+// sum f^2, pass count; j = 3 + d*n_bins + i: histogram cell (d, i)) is owned by thread j % 512 and receives the chunk's
+// events in event order.  partial: [gridDim.x][3 + n_dim*n_bins].  Up to VEGAS_RED_PER_THREAD entries per thread.
 constexpr int VEGAS_RED_TILE = 1024;
+constexpr int VEGAS_RED_PER_THREAD = 4;
 __global__ void __launch_bounds__(512) vegas_reduce_chunks(const double* __restrict__ f, const unsigned long long* __restrict__ idx,
                                                            int idx_words, int n_dim, int n_bins, long long n_ev, long long chunk,
                                                            double* __restrict__ partial) {
   __shared__ double f_s[VEGAS_RED_TILE];
   __shared__ unsigned long long idx_s[2 * VEGAS_RED_TILE];
-  const int cells = n_dim * n_bins, t = threadIdx.x;
-  const int d = t / n_bins, i = t - d * n_bins;
+  const int n_out = n_dim * n_bins + 3, t = threadIdx.x;
   const long long begin = blockIdx.x * chunk, end = min(n_ev, begin + chunk);
-  double acc = 0.0;
+  double acc[VEGAS_RED_PER_THREAD];
+  int word[VEGAS_RED_PER_THREAD], shift[VEGAS_RED_PER_THREAD], bin[VEGAS_RED_PER_THREAD];
+#pragma unroll
+  for (int k = 0; k < VEGAS_RED_PER_THREAD; ++k) {
+    acc[k] = 0.0;
+    const int j = t + 512 * k, cell = j - 3;
+    const int d = cell >= 0 ? cell / n_bins : 0;
+    word[k] = d >> 3;
+    shift[k] = 8 * (d & 7);
+    bin[k] = cell >= 0 ? cell - d * n_bins : -1;
+  }
   for (long long base = begin; base < end; base += VEGAS_RED_TILE) {
     const long long left = end - base;
     const int n = left < VEGAS_RED_TILE ? static_cast<int>(left) : VEGAS_RED_TILE;
@@ -109,24 +119,32 @@ __global__ void __launch_bounds__(512) vegas_reduce_chunks(const double* __restr
       for (int k = 0; k < idx_words; ++k) idx_s[e * idx_words + k] = idx[(base + e) * idx_words + k];
     }
     __syncthreads();
-    if (t < cells) {
-      const int word = d >> 3, shift = 8 * (d & 7);
-      for (int e = 0; e < n; ++e) {
-        const double v = f_s[e];
-        if (static_cast<int>((idx_s[e * idx_words + word] >> shift) & 0xffull) == i) acc += v * v;
+#pragma unroll
+    for (int k = 0; k < VEGAS_RED_PER_THREAD; ++k) {
+      const int j = t + 512 * k;
+      if (j >= n_out) continue;
+      double a = acc[k];
+      if (j == 0) {
+        for (int e = 0; e < n; ++e) a += f_s[e];
+      } else if (j == 1) {
+        for (int e = 0; e < n; ++e) a += f_s[e] * f_s[e];
+      } else if (j == 2) {
+        for (int e = 0; e < n; ++e) a += (f_s[e] != 0.0) ? 1.0 : 0.0;
+      } else {
+        for (int e = 0; e < n; ++e) {
+          const double v = f_s[e];
+          if (static_cast<int>((idx_s[e * idx_words + word[k]] >> shift[k]) & 0xffull) == bin[k]) a += v * v;
+        }
       }
-    } else if (t == cells) {
-      for (int e = 0; e < n; ++e) acc += f_s[e];
-    } else if (t == cells + 1) {
-      for (int e = 0; e < n; ++e) acc += f_s[e] * f_s[e];
-    } else if (t == cells + 2) {
-      for (int e = 0; e < n; ++e) acc += (f_s[e] != 0.0) ? 1.0 : 0.0;
+      acc[k] = a;
     }
     __syncthreads();
   }
-  const int n_out = cells + 3;
-  if (t < cells) partial[static_cast<long long>(blockIdx.x) * n_out + 3 + t] = acc;
-  else if (t < cells + 3) partial[static_cast<long long>(blockIdx.x) * n_out + (t - cells)] = acc;
+#pragma unroll
+  for (int k = 0; k < VEGAS_RED_PER_THREAD; ++k) {
+    const int j = t + 512 * k;
+    if (j < n_out) partial[static_cast<long long>(blockIdx.x) * n_out + j] = acc[k];
+  }
 }
 // second stage: entry j of sums = partial[0][j] + partial[1][j] + ... in chunk order
 __global__ void vegas_reduce_final(const double* __restrict__ partial, int n_chunks, int n_out, double* __restrict__ sums) {
