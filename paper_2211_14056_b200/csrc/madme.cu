@@ -60,7 +60,23 @@ struct me_handle {
 
 namespace {
 
+// W (events = warps per CTA) is a run-time choice among the compiled instances; MADME_WARPS overrides it — the
+// threads-per-block scan of PAPER.md:78-84 (Fig. 3) is repeated with it.
 template <class P> struct ProcInfo {
+  template <int W> static int geom(int* regs, int* ctas) {
+    cudaFuncAttributes fa;
+    CU(cudaFuncGetAttributes(&fa, me_eval_kernel<P, W>));
+    const int bytes = W * EventSmem<P>::DOUBLES * 8;
+    if (cudaFuncSetAttribute(me_eval_kernel<P, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) != cudaSuccess ||
+        cudaFuncSetAttribute(vegas_integrand_kernel<P, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) != cudaSuccess) {
+      (void)cudaGetLastError();
+      *ctas = 0;
+      return ME_OK;
+    }
+    *regs = fa.numRegs;
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas, me_eval_kernel<P, W>, 32 * W, bytes));
+    return ME_OK;
+  }
   static int fill(me_handle* h, int n4g) {
     h->n_ext = P::N_EXT; h->n_hel = P::N_HEL; h->n_flow = P::N_FLOW; h->n_diag = P::N_DIAGRAMS;
     h->n_terms = P::N_TERMS; h->n_diag4g = n4g; h->n_cur = P::N_CURRENTS; h->flops = P::FLOPS_PER_EVENT;
@@ -68,52 +84,56 @@ template <class P> struct ProcInfo {
     double c = 1.0;
     for (int i = 0; i < P::COUPLING_POWER / 2; ++i) c *= g2;
     h->scale = c / (double(P::CF_DEN) * double(P::AVG_DEN));
-    // geometry: as many events (warps) per SM as shared memory and registers allow
-    cudaFuncAttributes fa;
-    CU(cudaFuncGetAttributes(&fa, me_eval_kernel<P, 8>));
-    h->regs = fa.numRegs;
-    const int ev_bytes = EventSmem<P>::DOUBLES * 8;
-    int dev = 0, max_smem = 0;
+    int dev = 0;
     CU(cudaGetDevice(&dev));
     CU(cudaDeviceGetAttribute(&h->sms, cudaDevAttrMultiProcessorCount, dev));
-    CU(cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
-    int warps = 8;
+    const int cand[4] = {1, 2, 4, 8};
+    int regs[4] = {0, 0, 0, 0}, ctas[4] = {0, 0, 0, 0}, rc;
+    if ((rc = geom<1>(&regs[0], &ctas[0])) || (rc = geom<2>(&regs[1], &ctas[1])) || (rc = geom<4>(&regs[2], &ctas[2])) ||
+        (rc = geom<8>(&regs[3], &ctas[3])))
+      return rc;
+    int pick = -1;
     const char* env = getenv("MADME_WARPS");
-    if (env && atoi(env) >= 1 && atoi(env) <= 8) warps = atoi(env);
-    else {
-      // pick the warps/CTA in 1..8 that maximises resident warps per SM (ties: larger CTA)
+    if (env) {
+      for (int k = 0; k < 4; ++k)
+        if (atoi(env) == cand[k] && ctas[k] > 0) pick = k;
+      if (pick < 0) return fail(ME_EINVAL, "MADME_WARPS must be 1, 2, 4 or 8 (and fit on an SM)%s%s");
+    } else {
+      // most resident warps per SM; ties go to the larger CTA (fuller lanes in the current stages)
       int best = 0;
-      for (int w = 1; w <= 8; ++w) {
-        if (w * ev_bytes > max_smem) break;
-        const int per_sm = (max_smem + 1024) / (w * ev_bytes + 1024);
-        const int by_regs = 65536 / (fa.numRegs * 32 * w);
-        const int res = w * (per_sm < by_regs ? per_sm : by_regs);
-        if (res >= best) { best = res; warps = w; }
-      }
+      for (int k = 0; k < 4; ++k)
+        if (cand[k] * ctas[k] >= best && ctas[k] > 0) { best = cand[k] * ctas[k]; pick = k; }
+      if (pick < 0) return fail(ME_ECUDA, "me_eval kernel does not fit on an SM%s%s");
     }
-    h->warps = warps;
-    h->smem_bytes = warps * ev_bytes;
-    CU(cudaFuncSetAttribute(me_eval_kernel<P, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_bytes));
-    CU(cudaFuncSetAttribute(vegas_integrand_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_bytes));
-    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&h->ctas_per_sm, me_eval_kernel<P, 8>, warps * 32, h->smem_bytes));
-    if (h->ctas_per_sm < 1) return fail(ME_ECUDA, "me_eval kernel does not fit on an SM%s%s");
+    h->warps = cand[pick];
+    h->regs = regs[pick];
+    h->ctas_per_sm = ctas[pick];
+    h->smem_bytes = h->warps * EventSmem<P>::DOUBLES * 8;
     h->grid = h->sms * h->ctas_per_sm;
     return ME_OK;
   }
   static int eval(me_handle* h, const double* mom, double* me2, double* hel, long long n, cudaStream_t s) {
     const long long need = (n + h->warps - 1) / h->warps;
-    const int grid = static_cast<int>(need < h->grid ? need : h->grid);
-    me_eval_kernel<P, 8><<<grid, h->warps * 32, h->smem_bytes, s>>>(mom, me2, hel, n, h->mass, h->scale);
+    const int grid = static_cast<int>(need < h->grid ? need : h->grid), T = 32 * h->warps;
+    switch (h->warps) {
+      case 1: me_eval_kernel<P, 1><<<grid, T, h->smem_bytes, s>>>(mom, me2, hel, n, h->mass, h->scale); break;
+      case 2: me_eval_kernel<P, 2><<<grid, T, h->smem_bytes, s>>>(mom, me2, hel, n, h->mass, h->scale); break;
+      case 4: me_eval_kernel<P, 4><<<grid, T, h->smem_bytes, s>>>(mom, me2, hel, n, h->mass, h->scale); break;
+      default: me_eval_kernel<P, 8><<<grid, T, h->smem_bytes, s>>>(mom, me2, hel, n, h->mass, h->scale); break;
+    }
     CU(cudaGetLastError());
     return ME_OK;
   }
   static int integrand(me_handle* h, const VegasArgs& a, double* f, unsigned long long* idx, int words, cudaStream_t s) {
-    int per_sm = 0;
-    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, vegas_integrand_kernel<P>, h->warps * 32, h->smem_bytes));
-    if (per_sm < 1) return fail(ME_ECUDA, "vegas_integrand kernel does not fit on an SM%s%s");
-    const long long batches = (a.n_ev + 31) / 32, need = (batches + h->warps - 1) / h->warps;
-    const long long full = static_cast<long long>(h->sms) * per_sm;
-    vegas_integrand_kernel<P><<<static_cast<int>(need < full ? need : full), h->warps * 32, h->smem_bytes, s>>>(a, f, idx, words);
+    const int T = 32 * h->warps;
+    const long long need = (a.n_ev + T - 1) / T;
+    const int grid = static_cast<int>(need < h->grid ? need : h->grid);
+    switch (h->warps) {
+      case 1: vegas_integrand_kernel<P, 1><<<grid, T, h->smem_bytes, s>>>(a, f, idx, words); break;
+      case 2: vegas_integrand_kernel<P, 2><<<grid, T, h->smem_bytes, s>>>(a, f, idx, words); break;
+      case 4: vegas_integrand_kernel<P, 4><<<grid, T, h->smem_bytes, s>>>(a, f, idx, words); break;
+      default: vegas_integrand_kernel<P, 8><<<grid, T, h->smem_bytes, s>>>(a, f, idx, words); break;
+    }
     CU(cudaGetLastError());
     return ME_OK;
   }

@@ -14,28 +14,34 @@
 //   Leg 0 is fixed at helicity +1 (parity: |M(-h)|^2 = |M(h)|^2, the sum is doubled at the end), so
 //   variant index v = sum_k b_{l_k} 2^k over the legs l_0 < l_1 < ... of S OTHER THAN LEG 0, b = 0 for helicity -1,
 //   1 for +1, and nv = 2^(number of those legs).
-//   The first PERSISTENT_DOUBLES hold what the closings read; the rest is a transient region that the top-level
-//   currents of successive rounds reuse once their colour-ordered combinations have been formed.
+//   The first BASE_DOUBLES hold what every round reads (subset blocks, external wavefunctions, the currents that feed
+//   other currents); the rest is the ROUND region, reused by successive rounds of leg splits (gen/emit.py).
 //
 // The steps:
 //   a5  me_phase0      : K_S and propagator denominators for every subset, external wavefunctions
-//   a6  P::stage(s)    : off-shell currents and their combinations, one (object, variant) task per lane, stage by stage
-//   a7-a10             : generated straight-line code (csrc/generated/*.inc), one helicity per lane
+//   a6  me_run_row     : off-shell currents and their combinations, one (object, variant) task per thread, stage by stage
+//   a7-a10             : generated straight-line code (csrc/generated/*.inc: dots, colour), one helicity per lane
 #pragma once
 #include "helas.cuh"
 
 namespace madme {
 
-constexpr int ME_TASK_INTS = 16;
-// task row: 0 out, 1 out_stride, 2 a, 3 a_stride, 4 b, 5 b_stride, 6 c, 7 c_stride,
-//           8 ksub_out, 9 ksub_a, 10 ksub_b, 11 massive, 12 out2, 13 out3, 14 ksub_c, 15 unpropagated
-// combo row: 0 out, 1 stride, 2 n, then n x (input offset, k) : out = sum_j i^k_j in_j
+// One task = one (object, helicity variant), encoded in 128 bits so that a lane fetches its task with one load:
+//   x: out | a << 16                      (offsets in doubles into the event's scratch)
+//   y: b   | c << 16
+//   z: ksub_out | ksub_a << 8 | ksub_b << 16 | op << 24 | massive << 27 | open << 28      (ksub = subset index)
+//   w: log2(nv) of out | of a << 4 | of b << 8 | of c << 12 | n_members << 16 | phase codes (2 bits each) << 20
+// component stride of an object = 2 nv doubles.  The three colour terms of a four-gluon current are laid out
+// back to back (out, out + 8 nv, out + 16 nv).  OP_COMBO: out = sum_j i^{k_j} member_j with members (a, b, c, and
+// a fourth in the ksub_a/ksub_b bytes' place: z & 0xffff).  Rows are grouped in warp-wide iterations of one op
+// (padded with OP_NOP), iterations in stages; a warp barrier separates stages.
+struct MeRow { unsigned x, y, z, w; };
+enum MeOp { OP_FFV_ROW = 0, OP_FFV_COL = 1, OP_FFV_VEC = 2, OP_VVV = 3, OP_VVVV = 4, OP_COMBO = 5, OP_NOP = 7 };
 #if defined(__CUDA_ARCH__)
 #define ME_FENCE() asm volatile("" ::: "memory")  // keeps ptxas from hoisting every shared-memory load to the top
 #else
 #define ME_FENCE()
 #endif
-enum MeOp { OP_FFV_ROW = 0, OP_FFV_COL = 1, OP_FFV_VEC = 2, OP_VVV = 3, OP_VVVV = 4 };
 
 ME_HD wf4 ld_wf(const double* p, int stride) {
   wf4 w;
@@ -69,9 +75,10 @@ ME_HD vec4 ld_k(const double* p) {
 
 // a5: subset momenta + denominators, external wavefunctions.  `mom` = this event's [n_ext][4] (E,px,py,pz),
 // physical momenta; legs 0,1 incoming.  sub_masks[s] = bitmask of legs of subset s (block s at sm + 8 s).
-ME_HD void me_phase0(int lane, double* sm, const double* mom, int n_ext, int n_sub, const int* sub_masks,
+// Work items idx, idx + step, ... (subsets, then legs) of ONE event.
+ME_HD void me_phase0(int idx, int step, double* sm, const double* mom, int n_ext, int n_sub, const int* sub_masks,
                      const int* leg_kind, const int* leg_massive, const int* ext_off, double mass) {
-  for (int s = lane; s < n_sub; s += 32) {
+  for (int s = idx; s < n_sub; s += step) {
     const int m = sub_masks[s];
     double K[4] = {0.0, 0.0, 0.0, 0.0};
     int cnt = 0;
@@ -91,7 +98,7 @@ ME_HD void me_phase0(int lane, double* sm, const double* mom, int n_ext, int n_s
       o[4] = 0.0; o[5] = 0.0;
     }
   }
-  for (int l = lane; l < n_ext; l += 32) {
+  for (int l = idx; l < n_ext; l += step) {
     wf4 w[2];
     external_wavefunction(leg_kind[l], mom + 4 * l, leg_massive[l] ? mass : 0.0, w);
     if (l == 0) {
@@ -103,55 +110,60 @@ ME_HD void me_phase0(int lane, double* sm, const double* mom, int n_ext, int n_s
   }
 }
 
-// a6: one off-shell current variant
-ME_HD void me_run_task(int op, double* sm, const int* t, double mass) {
-  const wf4 A = ld_wf(sm + t[2], t[3]);
-  const wf4 B = ld_wf(sm + t[4], t[5]);
-  const double* ks = sm + t[8];
-  const double m = t[11] ? mass : 0.0;
-  const bool open = t[15] != 0;  // the current stops at its vertex: no propagator (the U side of a propagator cut)
+// i^k x
+ME_HD cplx times_ik(cplx x, int k) {
+  const double re = (k & 1) ? -x.im : x.re, im = (k & 1) ? x.re : x.im;
+  return mk((k & 2) ? -re : re, (k & 2) ? -im : im);
+}
+
+// a6: one task
+ME_HD void me_run_row(const MeRow r, double* sm, double mass) {
+  const int op = (r.z >> 24) & 7;
+  if (op == OP_NOP) return;
+  const int out = r.x & 0xffff, so = 2 << (r.w & 15);
+  const wf4 A = ld_wf(sm + (r.x >> 16), 2 << ((r.w >> 4) & 15));
+  if (op == OP_COMBO) {
+    // colour-ordered combination of currents over the same legs (same variant, same stride)
+    const int n = (r.w >> 16) & 15;
+    wf4 acc = A;  // the first member always enters with coefficient 1
+    const int off[3] = {static_cast<int>(r.y & 0xffff), static_cast<int>(r.y >> 16), static_cast<int>(r.z & 0xffff)};
+    for (int j = 1; j < n; ++j) {
+      const wf4 x = ld_wf(sm + off[j - 1], so);
+      const int k = (r.w >> (20 + 2 * j)) & 3;
+      for (int c = 0; c < 4; ++c) acc.c[c] = acc.c[c] + times_ik(x.c[c], k);
+    }
+    st_wf(sm + out, so, acc);
+    return;
+  }
+  const wf4 B = ld_wf(sm + (r.y & 0xffff), 2 << ((r.w >> 8) & 15));
+  const double* ks = sm + 8 * (r.z & 0xff);
+  const bool massive = (r.z >> 27) & 1;
+  const bool open = (r.z >> 28) & 1;  // the current stops at its vertex: no propagator (U side of a propagator cut)
+  const double m = massive ? mass : 0.0;
   const double invk2 = open ? 1.0 : ks[4];
   if (op == OP_FFV_ROW) {
     const wf4 x = slash_row(A, B);
-    st_wf(sm + t[0], t[1], open ? x : prop_row(ld_k(ks), -1.0, m, t[11] ? ks[5] : ks[4], x));
+    st_wf(sm + out, so, open ? x : prop_row(ld_k(ks), -1.0, m, massive ? ks[5] : ks[4], x));
   } else if (op == OP_FFV_COL) {
     const wf4 x = slash_col(B, A);
-    st_wf(sm + t[0], t[1], open ? x : prop_col(ld_k(ks), 1.0, m, t[11] ? ks[5] : ks[4], x));
+    st_wf(sm + out, so, open ? x : prop_col(ld_k(ks), 1.0, m, massive ? ks[5] : ks[4], x));
   } else if (op == OP_FFV_VEC) {
-    st_wf(sm + t[0], t[1], ffv_vec(A, B, invk2));
+    st_wf(sm + out, so, ffv_vec(A, B, invk2));
   } else if (op == OP_VVV) {
-    st_wf(sm + t[0], t[1], vvv_vec(A, ld_k(sm + t[9]), B, ld_k(sm + t[10]), invk2));
+    st_wf(sm + out, so, vvv_vec(A, ld_k(sm + 8 * ((r.z >> 8) & 0xff)), B, ld_k(sm + 8 * ((r.z >> 16) & 0xff)), invk2));
   } else {
-    const wf4 C = ld_wf(sm + t[6], t[7]);
+    const wf4 C = ld_wf(sm + (r.y >> 16), 2 << ((r.w >> 12) & 15));
     wf4 t1, t2, t3;
     vvvv_vec(A, B, C, invk2, t1, t2, t3);
-    st_wf(sm + t[0], t[1], t1);
-    st_wf(sm + t[12], t[1], t2);
-    st_wf(sm + t[13], t[1], t3);
+    st_wf(sm + out, so, t1);
+    st_wf(sm + out + 4 * so, so, t2);
+    st_wf(sm + out + 8 * so, so, t3);
   }
 }
 
-// all tasks [begin, end) of one (level, op) group, 32 lanes at a time
-ME_HD void me_run_group(int op, int lane, double* sm, const int* tab, int begin, int end, double mass) {
-  for (int i = begin + lane; i < end; i += 32) me_run_task(op, sm, tab + ME_TASK_INTS * i, mass);
-}
-
-// colour-ordered combinations: out = sum_j i^{k_j} in_j (same leg set, same variant)
-ME_HD void me_run_combos(int lane, double* sm, const int* ctab, int begin, int end) {
-  for (int i = begin + lane; i < end; i += 32) {
-    const int* t = ctab + ME_TASK_INTS * i;
-    wf4 acc = ld_wf(sm + t[3], t[1]);  // first member always enters with coefficient 1
-    for (int j = 1; j < t[2]; ++j) {
-      const wf4 x = ld_wf(sm + t[3 + 2 * j], t[1]);
-      const int k = t[4 + 2 * j];
-      for (int c = 0; c < 4; ++c) {
-        const double re = (k & 1) ? -x.c[c].im : x.c[c].re, im = (k & 1) ? x.c[c].re : x.c[c].im;
-        acc.c[c].re += (k & 2) ? -re : re;
-        acc.c[c].im += (k & 2) ? -im : im;
-      }
-    }
-    st_wf(sm + t[0], t[1], acc);
-  }
+// rows [begin, end) of one stage, 32 lanes at a time (host emulation and reference semantics of the device loop)
+ME_HD void me_run_rows(int lane, double* sm, const MeRow* tab, int begin, int end, double mass) {
+  for (int i = begin + lane; i < end; i += 32) me_run_row(tab[i], sm, mass);
 }
 
 }  // namespace madme

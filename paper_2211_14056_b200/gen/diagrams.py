@@ -14,9 +14,9 @@ splitting the legs n/2 | n/2 — go to the side that holds leg 0).  The hanging 
 currents; structurally identical subtrees are shared between diagrams.  A subtree / diagram containing a
 four-gluon vertex splits into three colour-pure terms.
 
-Propagator-cut closings.  When n is even, a diagram whose centroid vertex has a hanging subtree C with exactly
-n/2 legs (it never holds leg 0) is not evaluated at that vertex: the other subtrees of the vertex are merged
-into the UN-propagated current U over the complementary n/2 legs (it holds leg 0) and the diagram is the plain
+Propagator-cut closings.  A diagram is not evaluated at its centroid vertex: one hanging subtree C of that vertex
+that does not hold leg 0 stays a propagated current, the other subtrees of the vertex are merged into the
+UN-propagated ("open") current U over the complementary legs (it holds leg 0), and the diagram is the plain
 contraction U . C (a 4-component dot product instead of a vertex).  `factorise()` then sums, per colour flow,
 the U's and the C's of one leg split into colour-ordered combinations first (every current depends only on the
 helicities of its own n/2 legs), so that a flow receives ONE dot product per split — the colour-ordered
@@ -55,6 +55,7 @@ PROCESSES = {
                  "gs", 4 * 64 * 2),
 }
 VECTOR_OF = {"t": "g", "e": "a", "mu": "a"}
+CUT_ALL = True   # every diagram is the contraction of an open current U with a propagated current C (see _pick_cut)
 
 # ---- SU(3) ---------------------------------------------------------------------------------------------------
 
@@ -225,9 +226,9 @@ class Program:
                 continue
             for combo in itertools.product(*[self.subtrees(p) for p in parts]):
                 if all(o.type == ("V", "g") for o in combo):
-                    half = [o for o in combo if 2 * len(o.legs) == n]
-                    if half:
-                        self._close_cut(half[0], [o for o in combo if o is not half[0]], True)
+                    cut = self._pick_cut(combo)
+                    if cut is not None:
+                        self._close_cut(cut, [o for o in combo if o is not cut], True)
                         continue
                     d = self._count_diagram(combo, True)
                     ph = np.prod([o.phase for o in combo]) * (-1j)  # vertex -i g^2
@@ -289,11 +290,23 @@ class Program:
                 made = True
             self.terms.append(Term("DOT_" + kind, (U.id, big.id), U.phase * big.phase, 0, d))
 
+    def _pick_cut(self, objs):
+        """The hanging subtree that stays a propagated current C when the closing vertex is folded into the open
+        current U of the others: never the one holding leg 0 (so that U does, and has half the variants by parity);
+        the one with the most legs (U then spans the fewest), ties to the highest leg number (fewest distinct leg
+        splits).  CUT_ALL = False restricts this to the n/2 | n/2 splits and closes the rest at the vertex."""
+        cands = [o for o in objs if 0 not in o.legs]
+        if not CUT_ALL:
+            cands = [o for o in cands if 2 * len(o.legs) == self.n]
+        if not cands:
+            return None
+        return max(cands, key=lambda o: (len(o.legs), max(o.legs)))
+
     def _close3(self, A, B, C):
         objs = (A, B, C)
-        half = [o for o in objs if 2 * len(o.legs) == self.n]
-        if half:
-            self._close_cut(half[0], [o for o in objs if o is not half[0]], False)
+        cut = self._pick_cut(objs)
+        if cut is not None:
+            self._close_cut(cut, [o for o in objs if o is not cut], False)
             return
         kinds = [o.type[0] for o in objs]
         if sorted(kinds) == ["I", "O", "V"]:

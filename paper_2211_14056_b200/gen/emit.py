@@ -1,11 +1,15 @@
 """Emit the CUDA source of one process from its Program (gen/diagrams.py).
 
 Output: paper_2211_14056_b200/csrc/generated/<process>.inc — a struct with
-  * the scratch layout (subset blocks, persistent wavefunctions, a transient region reused round by round),
-  * the task table of the off-shell currents (step a6) and the table of their colour-ordered combinations,
-    executed cooperatively by the warp in STAGES (stage(s, lane, ...) ; warp barrier between stages),
-  * straight-line code for ONE helicity combination executed by one lane (steps a7-a9): the propagator-cut dot
-    products accumulated straight into the colour-flow vector J, the remaining vertex closings, J^dagger CF J.
+  * the scratch layout of one event: a BASE region (subset momenta, external wavefunctions, the currents that
+    feed other currents) and one ROUND region that successive rounds reuse,
+  * one table of 128-bit task rows (me_tasks.cuh::MeRow) in execution order: the base currents level by level,
+    then for every round the open / propagated currents of its leg splits and their colour-ordered combinations,
+  * per round, straight-line code `dots(r, sm, h, jr, ji)` for ONE helicity combination (one lane): the
+    propagator-cut dot products of the round's leg splits, accumulated straight into the colour-flow vector J
+    (steps a7-a8), and `colour(jr, ji)` = J^dagger CF J (step a9).
+A round is: tasks -> barrier -> combinations -> barrier -> dots -> barrier; J stays in registers across rounds, so an
+event needs BASE + max(ROUND) doubles of shared memory, not the sum over all leg splits.
 The file is `__host__ __device__` so tests/ can run it on the CPU for debugging.
 
 Run `python -m paper_2211_14056_b200.gen.emit` to regenerate all processes (done by build()).
@@ -15,20 +19,20 @@ import os
 from .diagrams import PROCESSES, Program
 
 OPCODE = {"FFV_ROW": 0, "FFV_COL": 1, "FFV_VEC": 2, "VVV": 3, "VVVV1": 4}
-OPNAME = {0: "OP_FFV_ROW", 1: "OP_FFV_COL", 2: "OP_FFV_VEC", 3: "OP_VVV", 4: "OP_VVVV"}
+OP_COMBO, OP_NOP = 5, 7
 HERE = os.path.dirname(os.path.abspath(__file__))
 OUT_DIR = os.path.join(os.path.dirname(HERE), "csrc", "generated")
-N_ROUNDS = int(os.environ.get("MADME_GEN_ROUNDS", "3"))   # transient-region reuse (shared-memory footprint knob)
+N_ROUNDS = int(os.environ.get("MADME_GEN_ROUNDS", "6"))   # shared-memory footprint knob (see Layout)
+GROUP_PAD = 4   # rows of one op come in multiples of this (a CTA of 8 events maps 4 rows x 8 events on a warp)
 
 # fp64 operation counts of the routines in csrc/helas.cuh as written (FMA = 2, add/mul = 1; complex mul = 1 mul +
-# 1 fma per component = 6, complex fma = 8).  (prop, unprop) where the routine has both forms.
+# 1 fma per component = 6, complex fma = 8).  (propagated, open) forms.
 FLOPS = {
     "FFV_ROW": (8 + 4 * 14 + 2 + 4 * 24 + 8, 8 + 4 * 14),      # slash (4 cadd + 4 (cmul + cfma)) + (Kslash + m) x f
     "FFV_COL": (8 + 4 * 14 + 2 + 4 * 24 + 8, 8 + 4 * 14),
     "FFV_VEC": (8 * 6 + 12 * 2 + 8, 8 * 6 + 12 * 2 + 8),
     "VVV": (12 + 14 * 3 + 4 * 20, 12 + 14 * 3 + 4 * 20),
     "VVVV": (3 * 30 + 6 + 4 * 24, 3 * 30 + 6 + 4 * 24),
-    "FFV_AMP": 8 + 4 * 14 + 6 + 3 * 8, "VVV_AMP": 12 + 3 * 30 + 3 * 14 + 6 + 16, "VVVV_AMP": 6 * 30 + 3 * 6 + 6,
     "DOT": 4 * 8, "EXT": 45,
 }
 
@@ -48,172 +52,185 @@ def variant_index(sub_legs, sup_legs, v):
 
 
 class Layout:
+    """Where every object of one event lives.  A leg split = (legs of the open side U | the rest); all objects that
+    only serve one split (its open currents, its top-level propagated currents, the combinations of both sides)
+    live in the round region while that split's round is processed."""
+
     def __init__(self, P, n_rounds):
         self.P = P
         objs = P.used_objects()
         self.objs = objs
+        all_legs = tuple(range(P.n))
         subsets = sorted({o.legs for o in objs}, key=lambda s: (len(s), s))
         self.subsets = subsets
         self.sub_index = {s: i for i, s in enumerate(subsets)}
-        direct = set()
-        for t in P.terms:
-            if not t.op.startswith("DOT"):
-                direct.update(t.args)
-        for _, u, c, _, _ in P.dots:
-            direct.update((u, c))
+        feeds = set()                      # objects that are inputs of vertex tasks
         for o in objs:
             if o.op != "COMBO":
-                direct.update(o.args)
-        self.transient = {o.id for o in objs if o.op not in ("EXT", "COMBO") and o.id not in direct}
-        # rounds: the leg sets of the transient objects, packed greedily into n_rounds bins of similar size
-        sets = {}
+                feeds.update(o.args)
+        self.base = [o for o in objs if o.op == "EXT" or o.id in feeds]
+        base_ids = {o.id for o in self.base}
+        # split of every other object: U side -> its own legs; C side -> the complement
+        u_sets = {P.objs[d[1]].legs for d in P.dots}
+        self.split_of = {}
         for o in objs:
-            if o.id in self.transient:
-                sets[o.legs] = sets.get(o.legs, 0) + 8 * self.nv(o)
-        bins = [[0, []] for _ in range(max(1, min(n_rounds, len(sets))))] if sets else []
-        for legs, size in sorted(sets.items(), key=lambda kv: -kv[1]):
+            if o.id in base_ids:
+                continue
+            comp = tuple(l for l in all_legs if l not in o.legs)
+            self.split_of[o.id] = o.legs if (0 in o.legs) else comp
+            assert self.split_of[o.id] in u_sets, o.legs
+        self.splits = sorted(u_sets, key=lambda s: (len(s), s))
+        size = {s: 0 for s in self.splits}
+        for o in objs:
+            if o.id in self.split_of:
+                size[self.split_of[o.id]] += 8 * self.nv(o)
+        bins = [[0, []] for _ in range(max(1, min(n_rounds, len(self.splits))))]
+        for s_, sz in sorted(size.items(), key=lambda kv: -kv[1]):
             b = min(bins, key=lambda x: x[0])
-            b[0] += size
-            b[1].append(legs)
-        self.round_of = {legs: r for r, b in enumerate(bins) for legs in b[1]}
-        self.n_rounds = len(bins)
+            b[0] += sz
+            b[1].append(s_)
+        bins = [b for b in bins if b[1]]
+        self.rounds = [sorted(b[1], key=lambda s: (len(s), s)) for b in bins]
+        self.round_of = {s_: r for r, b in enumerate(self.rounds) for s_ in b}
         off = 8 * len(subsets)
         self.off = {}
-        for o in objs:
-            if o.id not in self.transient:
-                self.off[o.id] = off
-                off += 8 * self.nv(o)
-        self.persistent_doubles = off
-        tmax = 0
-        for r in range(self.n_rounds):
+        for o in self.base:
+            self.off[o.id] = off
+            off += 8 * self.nv(o)
+        self.base_doubles = off
+        tmax = off
+        for r in range(len(self.rounds)):
             t = off
             for o in objs:
-                if o.id in self.transient and self.round_of[o.legs] == r:
+                if o.id in self.split_of and self.round_of[self.split_of[o.id]] == r:
                     self.off[o.id] = t
                     t += 8 * self.nv(o)
             tmax = max(tmax, t)
-        self.smem_doubles = max(tmax, off)
+        self.smem_doubles = tmax
 
     def nv(self, o):
         return 1 << len(bits_of(o.legs))
 
-    def ksub(self, o):
-        return 8 * self.sub_index[o.legs]
+    def round_objs(self, r):
+        return [o for o in self.objs if o.id in self.split_of and self.round_of[self.split_of[o.id]] == r]
 
 
 def emit_process(name, n_rounds=None):
     P = Program(name)
+    assert all(t.op.startswith("DOT") for t in P.terms), "every diagram must be a propagator-cut contraction"
     L = Layout(P, N_ROUNDS if n_rounds is None else n_rounds)
     n = P.n
-    top = n // 2 if n % 2 == 0 else -1
+    nf = len(P.flow_perms)
     W = []
     w = W.append
+    s = P.summary()
     w("// GENERATED by paper_2211_14056_b200/gen/emit.py — do not edit; regenerate with")
     w("//   python -m paper_2211_14056_b200.gen.emit")
-    s = P.summary()
     w("// process %s: %d Feynman diagrams (%d with a 4-gluon vertex), %d colour-pure terms, %d colour flows"
       % (name, s["n_diagrams"], s["n_diagrams_4g"], s["n_terms"], s["n_flows"]))
     w("// (SURVEY.md §8 table; PAPER.md:57-58 Table 1 pins 16 and 123 through 36 = 16+4x5, 267 = 123+4x36)")
-    w("// evaluation: %d off-shell currents, %d colour-ordered combinations, %d propagator-cut dot products and %d vertex"
-      % (s["n_currents"], s["n_combos"], s["n_dots"], s["n_vertex_closings"]))
-    w("// closings per helicity combination; %d of %d combinations evaluated (parity, leg 0 fixed at +1)" % (1 << (n - 1), 1 << n))
+    w("// evaluation: %d off-shell currents, %d colour-ordered combinations and %d propagator-cut dot products per"
+      % (s["n_currents"], s["n_combos"], s["n_dots"]))
+    w("// helicity combination over %d leg splits in %d rounds; %d of %d combinations evaluated (parity, leg 0 at +1)"
+      % (len(L.splits), len(L.rounds), 1 << (n - 1), 1 << n))
     w("#pragma once")
     w('#include "../me_tasks.cuh"')
     w("namespace madme {")
     w("struct %s {" % name)
     w("  static constexpr int N_EXT = %d, N_HEL = %d, N_HEL_EVAL = %d, N_FLOW = %d, N_SUB = %d;"
-      % (n, 1 << n, 1 << (n - 1), len(P.flow_perms), len(L.subsets)))
-    w("  static constexpr int N_DIAGRAMS = %d, N_TERMS = %d, N_CURRENTS = %d, N_COMBOS = %d, N_DOTS = %d, N_VERTEX_CLOSINGS = %d;"
-      % (s["n_diagrams"], s["n_terms"], s["n_currents"], s["n_combos"], s["n_dots"], s["n_vertex_closings"]))
-    w("  static constexpr int SMEM_DOUBLES = %d, PERSISTENT_DOUBLES = %d;" % (L.smem_doubles, L.persistent_doubles))
+      % (n, 1 << n, 1 << (n - 1), nf, len(L.subsets)))
+    w("  static constexpr int N_DIAGRAMS = %d, N_DIAGRAMS_4G = %d, N_TERMS = %d, N_CURRENTS = %d, N_COMBOS = %d, N_DOTS = %d;"
+      % (s["n_diagrams"], s["n_diagrams_4g"], s["n_terms"], s["n_currents"], s["n_combos"], s["n_dots"]))
+    w("  static constexpr int SMEM_DOUBLES = %d, BASE_DOUBLES = %d;" % (L.smem_doubles, L.base_doubles))
     w("  static constexpr int CF_DEN = %d, AVG_DEN = %d, COUPLING_POWER = %d;  // me2 = g^(2*(n-2)) sum / (CF_DEN*AVG_DEN)"
       % (P.cf_den, P.avg, 2 * (n - 2)))
     w("  static constexpr bool QED = %s;" % ("true" if P.coupling == "ee" else "false"))
 
-    # ---- task tables, in execution order: lower levels, then the top level round by round -------------------
-    tasks, combo_rows, stages = [], [], []   # stages: list of ("tasks", [(opcode, begin, end)]) | ("combos", begin, end)
+    # ---- the task table --------------------------------------------------------------------------------------
+    rows = []
     cur_flops = 0
+    lg = lambda nv: {1: 0, 2: 1, 4: 2, 8: 3, 16: 4, 32: 5}[nv]
+    sub_i = lambda o: L.sub_index[o.legs]
 
-    def add_tasks(sel):
+    def pad(mult):
+        while len(rows) % mult:
+            rows.append((0, 0, OP_NOP << 24, 0))
+
+    def add_tasks(objs):
         nonlocal cur_flops
-        groups = []
         for opn in ("FFV_ROW", "FFV_COL", "FFV_VEC", "VVV", "VVVV1"):
-            begin = len(tasks)
-            for o in L.objs:
-                if o.op != opn or not sel(o):
+            for o in objs:
+                if o.op != opn:
                     continue
                 args = [P.objs[a] for a in o.args]
-                sibs = []
+                nv = L.nv(o)
                 if opn == "VVVV1":
                     sibs = [x for x in L.objs if x.op in ("VVVV2", "VVVV3") and x.args == o.args and x.legs == o.legs and x.prop == o.prop]
                     sibs.sort(key=lambda x: x.op)
-                    assert len(sibs) == 2
-                nv = L.nv(o)
+                    assert len(sibs) == 2 and L.off[sibs[0].id] == L.off[o.id] + 8 * nv and L.off[sibs[1].id] == L.off[o.id] + 16 * nv
+                massive = 1 if (o.type[0] in "OI" and P.legs[[l for l in o.legs if P.legs[l].kind >= 2][0]].massive) else 0
                 for v in range(nv):
-                    row = [0] * 16
-                    row[0] = L.off[o.id] + 2 * v
-                    row[1] = 2 * nv
-                    for k, a in enumerate(args):
-                        row[2 + 2 * k] = L.off[a.id] + 2 * variant_index(a.legs, o.legs, v)
-                        row[3 + 2 * k] = 2 * L.nv(a)
-                    row[8] = L.ksub(o)
-                    row[9] = L.ksub(args[0])
-                    row[10] = L.ksub(args[1])
-                    row[11] = 1 if (o.type[0] in "OI" and P.legs[[l for l in o.legs if P.legs[l].kind >= 2][0]].massive) else 0
-                    if sibs:
-                        row[12] = L.off[sibs[0].id] + 2 * v
-                        row[13] = L.off[sibs[1].id] + 2 * v
-                        row[14] = L.ksub(args[2])
-                    row[15] = 0 if o.prop else 1
-                    tasks.append(row)
+                    offs = [L.off[a.id] + 2 * variant_index(a.legs, o.legs, v) for a in args] + [0]
+                    lgs = [lg(L.nv(a)) for a in args] + [0]
+                    assert max(offs) < 65536 and L.off[o.id] + 2 * v < 65536
+                    x = (L.off[o.id] + 2 * v) | (offs[0] << 16)
+                    y = offs[1] | ((offs[2] if len(args) > 2 else 0) << 16)
+                    z = sub_i(o) | (sub_i(args[0]) << 8) | (sub_i(args[1]) << 16) | (OPCODE[opn] << 24) | (massive << 27) | ((0 if o.prop else 1) << 28)
+                    wv = lg(nv) | (lgs[0] << 4) | (lgs[1] << 8) | ((lgs[2] if len(args) > 2 else 0) << 12)
+                    rows.append((x, y, z, wv))
                     cur_flops += FLOPS["VVVV" if opn == "VVVV1" else opn][0 if o.prop else 1]
-            if len(tasks) > begin:
-                groups.append((OPCODE[opn], begin, len(tasks)))
-        if groups:
-            stages.append(("tasks", groups))
+            pad(GROUP_PAD)
+        pad(32)
 
-    def add_combos(sel):
+    def add_combos(objs):
         nonlocal cur_flops
-        begin = len(combo_rows)
-        for o in L.objs:
-            if o.op != "COMBO" or not sel(o):
+        for o in objs:
+            if o.op != "COMBO":
                 continue
             coefs = P.combo_coefs[o.id]
-            assert len(coefs) <= 6
+            assert len(coefs) <= 4 and coefs[0] == 1
             nv = L.nv(o)
             for v in range(nv):
-                row = [L.off[o.id] + 2 * v, 2 * nv, len(coefs)]
-                for a, z in zip(o.args, coefs):
-                    row += [L.off[a] + 2 * v, {1: 0, 1j: 1, -1: 2, -1j: 3}[z]]
-                row += [0] * (16 - len(row))
-                combo_rows.append(row)
+                m = [L.off[a] + 2 * v for a in o.args] + [0, 0, 0]
+                k = [{1: 0, 1j: 1, -1: 2, -1j: 3}[zc] for zc in coefs] + [0, 0, 0]
+                x = (L.off[o.id] + 2 * v) | (m[0] << 16)
+                y = m[1] | (m[2] << 16)
+                z = m[3] | (OP_COMBO << 24)
+                wv = lg(nv) | (lg(nv) << 4) | (len(coefs) << 16) | (k[1] << 22) | (k[2] << 24) | (k[3] << 26)
+                rows.append((x, y, z, wv))
                 cur_flops += 8 * (len(coefs) - 1)
-        if len(combo_rows) > begin:
-            stages.append(("combos", begin, len(combo_rows)))
+        pad(32)
 
-    levels = sorted({len(o.legs) for o in L.objs if o.op not in ("EXT", "COMBO")})
-    for lev in levels:
-        if lev != top:
-            add_tasks(lambda o, lev=lev: len(o.legs) == lev)
-    if top in levels:
-        # persistent top-level objects (used directly), then the transient ones round by round with their combos
-        add_tasks(lambda o: len(o.legs) == top and o.id not in L.transient)
-        for r in range(L.n_rounds):
-            add_tasks(lambda o, r=r: len(o.legs) == top and o.id in L.transient and L.round_of[o.legs] == r)
-            add_combos(lambda o, r=r: L.round_of.get(o.legs) == r)
-        add_combos(lambda o: o.legs not in L.round_of)
+    base_ends = []
+    for lev in sorted({len(o.legs) for o in L.base if o.op != "EXT"}):
+        add_tasks([o for o in L.base if len(o.legs) == lev and o.op != "EXT"])
+        base_ends.append(len(rows))
+    raw_ends, combo_ends = [], []
+    for r in range(len(L.rounds)):
+        ro = L.round_objs(r)
+        add_tasks(ro)
+        raw_ends.append(len(rows))
+        add_combos(ro)
+        combo_ends.append(len(rows))
 
-    w("  static constexpr int N_TASKS = %d, N_COMBO_TASKS = %d, N_STAGES = %d;" % (len(tasks), len(combo_rows), len(stages)))
-    w("  // off-shell current tasks: one row per (current, helicity variant); see me_tasks.cuh for the columns")
+    def table_fn(fname, vals):
+        w("  static ME_HD int %s(int i) {" % fname)
+        w("    switch (i) {")
+        for i, e in enumerate(vals):
+            w("      case %d: return %d;" % (i, e))
+        w("      default: return %d;" % (vals[-1] if vals else 0))
+        w("    }")
+        w("  }")
+
+    w("  static constexpr int N_ROWS = %d, N_BASE_STAGES = %d, N_ROUNDS = %d;" % (len(rows), len(base_ends), len(L.rounds)))
+    w("  // rows of base stage s end at base_end(s); round r: currents end at raw_end(r), combinations at combo_end(r)")
+    table_fn("base_end", base_ends)
+    table_fn("raw_end", raw_ends)
+    table_fn("combo_end", combo_ends)
     w("#define %s_TASK_TABLE { \\" % name.upper())
-    for row in tasks:
-        w("  " + ",".join(str(x) for x in row) + ", \\")
-    w("  0 }")
-    w("  // combination tasks: out, stride, n, then n x (input offset, power of i)")
-    w("#define %s_COMBO_TABLE { \\" % name.upper())
-    for row in combo_rows:
-        w("  " + ",".join(str(x) for x in row) + ", \\")
-    w("  0 }")
+    for r4 in rows:
+        w("  {%du,%du,%du,%du}, \\" % r4)
+    w("  {0u,0u,%du,0u} }" % (OP_NOP << 24))
     w("#define %s_SUB_MASKS { %s }" % (name.upper(), ",".join(str(sum(1 << l for l in sub)) for sub in L.subsets)))
     w("#define %s_LEG_KIND { %s }" % (name.upper(), ",".join(str(leg.kind) for leg in P.legs)))
     w("#define %s_LEG_MASSIVE { %s }" % (name.upper(), ",".join("1" if leg.massive else "0" for leg in P.legs)))
@@ -221,130 +238,66 @@ def emit_process(name, n_rounds=None):
     assert [o.legs[0] for o in L.objs if o.op == "EXT"] == list(range(n))
     w("#define %s_EXT_OFF { %s }" % (name.upper(), ",".join(str(x) for x in ext_off)))
 
-    # ---- stages ------------------------------------------------------------------------------------------------
-    w("  // a6: stage s of the cooperative current computation (a warp barrier separates stages)")
-    w("  static ME_HD void stage(int s, int lane, double* sm, const int* tab, const int* ctab, double mass) {")
-    w("    switch (s) {")
-    for si, st in enumerate(stages):
-        w("      case %d:" % si)
-        if st[0] == "tasks":
-            for (op, b, e) in st[1]:
-                w("        me_run_group(%s, lane, sm, tab, %d, %d, mass);" % (OPNAME[op], b, e))
-        else:
-            w("        me_run_combos(lane, sm, ctab, %d, %d);" % (st[1], st[2]))
-        w("        break;")
-    w("      default: break;")
-    w("    }")
-    w("  }")
-
-    # ---- closings ------------------------------------------------------------------------------------------
-    nf = len(P.flow_perms)
-    amp_flops = 0
-    w("  // a7-a9: closing amplitudes, colour-flow vector J and J^dagger CF J of helicity combination h")
-    w("  // (leg 0 has helicity +1; bit l-1 of h: helicity of leg l, 0 <-> -1, 1 <-> +1).")
-    w("  // Returns sum_{f,f'} J_f^* CFnum_{ff'} J_f'.")
-    w("  static ME_HD double closings(const double* __restrict__ sm, int h) {")
-    for l in range(1, n):
-        w("    const int b%d = (h >> %d) & 1;" % (l, l - 1))
-    w("    double jr[%d], ji[%d];" % (nf, nf))
-    w("    for (int f = 0; f < %d; ++f) { jr[f] = 0.0; ji[f] = 0.0; }" % nf)
-
+    # ---- dots, round by round ----------------------------------------------------------------------------------
     def ldw(oid):
         o = P.objs[oid]
         terms = ["%d * b%d" % (2 << k, l) for k, l in enumerate(bits_of(o.legs))]
         return "ld_wf(sm + %s, %d)" % (" + ".join([str(L.off[oid])] + terms), 2 * L.nv(o))
 
-    def ldk(oid):
-        return "ld_k(sm + %d)" % L.ksub(P.objs[oid])
-
-    def acc(var, flows):
-        out = []
-        for f, z in flows:
-            if z == 1:
-                out.append("jr[%d] += %s.re; ji[%d] += %s.im;" % (f, var, f, var))
-            elif z == -1:
-                out.append("jr[%d] -= %s.re; ji[%d] -= %s.im;" % (f, var, f, var))
-            elif z == 1j:
-                out.append("jr[%d] -= %s.im; ji[%d] += %s.re;" % (f, var, f, var))
-            elif z == -1j:
-                out.append("jr[%d] += %s.im; ji[%d] -= %s.re;" % (f, var, f, var))
-            else:
-                raise ValueError(z)
-        return " ".join(out)
-
-    # propagator-cut dot products, one block per leg split: load the C side once, then U by U
-    flow_adds = 0
-    splits = {}
-    for d in P.dots:
-        splits.setdefault(P.objs[d[1]].legs, []).append(d)
     zcode = {1: 0, 1j: 1, -1: 2, -1j: 3}
-    for legs in sorted(splits):
-        dots = splits[legs]
-        w("    {  // split %s | rest: %d dot products" % ("".join(str(l) for l in legs), len(dots)))
-        cs = sorted({d[2] for d in dots})
-        for c in cs:
-            w("      const wf4 c%d = %s;" % (c, ldw(c)))
-        for u in sorted({d[1] for d in dots}):
-            w("      { const wf4 u = %s;" % ldw(u))
-            for (f, uu, c, z, kind) in dots:
-                if uu == u:
-                    w("        dot_acc<%d, %s>(jr[%d], ji[%d], u, c%d);" % (zcode[z], "true" if kind == "V" else "false", f, f, c))
-                    amp_flops += FLOPS["DOT"]
-            w("      }")
-        w("      ME_FENCE();")
-        w("    }")
-    # remaining vertex closings
-    terms = [t for t in P.terms if not t.op.startswith("DOT")]
-    if terms:
-        w("    cplx a, a2, a3;")
-    i = 0
-    while i < len(terms):
-        t = terms[i]
-        if t.op == "FFV_AMP":
-            w("    a = ffv_amp(%s, %s, %s);" % (ldw(t.args[0]), ldw(t.args[1]), ldw(t.args[2])))
-            w("    " + acc("a", t.flows))
-            amp_flops += FLOPS["FFV_AMP"]
-            flow_adds += 2 * len(t.flows)
-            i += 1
-        elif t.op == "VVV_AMP":
-            x, y, z = t.args
-            w("    a = vvv_amp(%s, %s, %s, %s, %s, %s);" % (ldw(x), ldk(x), ldw(y), ldk(y), ldw(z), ldk(z)))
-            w("    " + acc("a", t.flows))
-            amp_flops += FLOPS["VVV_AMP"]
-            flow_adds += 2 * len(t.flows)
-            i += 1
-        else:
-            t1, t2, t3 = terms[i], terms[i + 1], terms[i + 2]
-            assert t1.args == t2.args == t3.args and (t1.which, t2.which, t3.which) == (1, 2, 3)
-            w("    vvvv_amp(%s, %s, %s, %s, a, a2, a3);" % tuple(ldw(x) for x in t1.args))
-            w("    " + acc("a", t1.flows))
-            w("    " + acc("a2", t2.flows))
-            w("    " + acc("a3", t3.flows))
-            amp_flops += FLOPS["VVVV_AMP"]
-            flow_adds += 2 * (len(t1.flows) + len(t2.flows) + len(t3.flows))
-            i += 3
-        w("    ME_FENCE();")
-    # colour contraction grouped by distinct CF numerator (9 distinct values for 4 gluons)
+    by_split = {}
+    for d in P.dots:
+        by_split.setdefault(P.objs[d[1]].legs, []).append(d)
+    amp_flops = 0
+    w("  // a7-a8: the dot products of round r for helicity combination h (leg 0 has helicity +1; bit l-1 of h is the")
+    w("  // helicity of leg l, 0 <-> -1, 1 <-> +1), accumulated into the colour-flow vector J = (jr, ji).")
+    w("  static ME_HD void dots(int r, const double* __restrict__ sm, int h, double* __restrict__ jr, double* __restrict__ ji) {")
+    for l in range(1, n):
+        w("    const int b%d = (h >> %d) & 1; (void)b%d;" % (l, l - 1, l))
+    w("    switch (r) {")
+    for r, split_list in enumerate(L.rounds):
+        w("      case %d: {" % r)
+        for legs in split_list:
+            dots = by_split[legs]
+            w("        {  // split %s | rest: %d dot products" % ("".join(str(l) for l in legs), len(dots)))
+            for c in sorted({d[2] for d in dots}):
+                w("          const wf4 c%d = %s;" % (c, ldw(c)))
+            for u in sorted({d[1] for d in dots}):
+                w("          { const wf4 u = %s;" % ldw(u))
+                for (f, uu, c, z, kind) in dots:
+                    if uu == u:
+                        w("            dot_acc<%d, %s>(jr[%d], ji[%d], u, c%d);" % (zcode[z], "true" if kind == "V" else "false", f, f, c))
+                        amp_flops += FLOPS["DOT"]
+                w("          }")
+            w("        }")
+        w("      } break;")
+    w("      default: break;")
+    w("    }")
+    w("  }")
+
+    # ---- colour contraction grouped by distinct CF numerator (9 distinct values for 4 gluons) ----
+    w("  // a9: sum_{f,f'} J_f^* CFnum_{ff'} J_f'  (CF real symmetric, integer numerators over CF_DEN)")
+    w("  static ME_HD double colour(const double* __restrict__ jr, const double* __restrict__ ji) {")
     cf = P.cf_num
     vals = sorted({int(cf[f, g]) for f in range(nf) for g in range(f, nf)}, key=lambda v: -abs(v))
     NPART = 2 if nf > 2 else 1
+    nm_of = lambda v: "s%s" % (("m%d" % -v) if v < 0 else str(v))
     for v in vals:
         for p in range(NPART):
-            w("    double s%s_%d = 0.0;" % (("m%d" % -v) if v < 0 else str(v), p))
+            w("    double %s_%d = 0.0;" % (nm_of(v), p))
     cnt = {v: 0 for v in vals}
     col_flops = 0
     for f in range(nf):
         for g in range(f, nf):
             v = int(cf[f, g])
-            nm = "s%s_%d" % ((("m%d" % -v) if v < 0 else str(v)), cnt[v] % NPART)
+            nm = "%s_%d" % (nm_of(v), cnt[v] % NPART)
             cnt[v] += 1
             w("    %s = fma(jr[%d], jr[%d], fma(ji[%d], ji[%d], %s));" % (nm, f, g, f, g, nm))
             col_flops += 4
     diag_vals = {int(cf[f, f]) for f in range(nf)}
     expr = []
     for v in vals:
-        nm = "s%s" % (("m%d" % -v) if v < 0 else str(v))
-        tot = " + ".join("%s_%d" % (nm, p) for p in range(NPART))
+        tot = " + ".join("%s_%d" % (nm_of(v), p) for p in range(NPART))
         # off-diagonal pairs count twice (CF symmetric); a value on the diagonal must not also be off-diagonal
         on_diag = v in diag_vals
         off_diag = any(int(cf[f, g]) == v for f in range(nf) for g in range(f + 1, nf))
@@ -355,10 +308,10 @@ def emit_process(name, n_rounds=None):
     w("  }")
     ext_flops = FLOPS["EXT"] * 2 * n
     nh = 1 << (n - 1)
-    per_event = ext_flops + cur_flops + nh * (amp_flops + flow_adds + col_flops)
+    per_event = ext_flops + cur_flops + nh * (amp_flops + col_flops)
     w("  // nominal fp64 flops per event as emitted (FMA = 2): externals %d + currents and combinations %d + %d helicities x"
       % (ext_flops, cur_flops, nh))
-    w("  // (dot products and vertex closings %d + flow accumulation %d + colour %d)" % (amp_flops, flow_adds, col_flops))
+    w("  // (dot products %d + colour %d)" % (amp_flops, col_flops))
     w("  static constexpr double FLOPS_PER_EVENT = %d.0;" % per_event)
     w("};")
     w("}  // namespace madme")

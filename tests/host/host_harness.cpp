@@ -16,8 +16,7 @@ using namespace madme;
 template <class P> struct Tables;
 #define DEF_TABLES(P, U)                                        \
   template <> struct Tables<P> {                                \
-    static const int* tasks() { static const int t[] = U##_TASK_TABLE; return t; }      \
-    static const int* combos() { static const int t[] = U##_COMBO_TABLE; return t; }    \
+    static const MeRow* tasks() { static const MeRow t[] = U##_TASK_TABLE; return t; }  \
     static const int* masks() { static const int t[] = U##_SUB_MASKS; return t; }       \
     static const int* kind() { static const int t[] = U##_LEG_KIND; return t; }         \
     static const int* massive() { static const int t[] = U##_LEG_MASSIVE; return t; }   \
@@ -28,9 +27,8 @@ DEF_TABLES(gg_ttx, GG_TTX)
 DEF_TABLES(gg_ttxg, GG_TTXG)
 DEF_TABLES(gg_ttxgg, GG_TTXGG)
 
-template <class P> void run_levels(double* sm, double mass) {
-  for (int s = 0; s < P::N_STAGES; ++s)
-    for (int lane = 0; lane < 32; ++lane) P::stage(s, lane, sm, Tables<P>::tasks(), Tables<P>::combos(), mass);
+template <class P> void rows(double* sm, int begin, int end, double mass) {
+  for (int lane = 0; lane < 32; ++lane) me_run_rows(lane, sm, Tables<P>::tasks(), begin, end, mass);
 }
 
 template <class P> void eval(const double* mom, double* me2, long long n, double mass, double coupling, double* per_hel) {
@@ -40,12 +38,20 @@ template <class P> void eval(const double* mom, double* me2, long long n, double
   const double scale = g2 / (double(P::CF_DEN) * double(P::AVG_DEN));
   for (long long e = 0; e < n; ++e) {
     for (int lane = 0; lane < 32; ++lane)
-      me_phase0(lane, sm.data(), mom + e * 4 * P::N_EXT, P::N_EXT, P::N_SUB, Tables<P>::masks(), Tables<P>::kind(),
+      me_phase0(lane, 32, sm.data(), mom + e * 4 * P::N_EXT, P::N_EXT, P::N_SUB, Tables<P>::masks(), Tables<P>::kind(),
                 Tables<P>::massive(), Tables<P>::ext_off(), mass);
-    run_levels<P>(sm.data(), mass);
+    int row = 0;
+    for (int s = 0; s < P::N_BASE_STAGES; ++s) { rows<P>(sm.data(), row, P::base_end(s), mass); row = P::base_end(s); }
+    std::vector<double> jr(P::N_HEL_EVAL * P::N_FLOW, 0.0), ji(P::N_HEL_EVAL * P::N_FLOW, 0.0);
+    for (int r = 0; r < P::N_ROUNDS; ++r) {
+      rows<P>(sm.data(), row, P::raw_end(r), mass);
+      rows<P>(sm.data(), P::raw_end(r), P::combo_end(r), mass);
+      row = P::combo_end(r);
+      for (int h = 0; h < P::N_HEL_EVAL; ++h) P::dots(r, sm.data(), h, &jr[h * P::N_FLOW], &ji[h * P::N_FLOW]);
+    }
     double s = 0;
     for (int h = 0; h < P::N_HEL_EVAL; ++h) {
-      const double v = P::closings(sm.data(), h);
+      const double v = P::colour(&jr[h * P::N_FLOW], &ji[h * P::N_FLOW]);
       if (per_hel) per_hel[e * P::N_HEL_EVAL + h] = v * scale;
       s += v;
     }
