@@ -1,0 +1,63 @@
+// common.cuh — shared by the translation units of libmadme.so: error reporting, the handle, and the table of
+// per-process entry points (each process's kernels are compiled in their own translation units).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include "../../include/madme.h"
+#include "vegas_common.cuh"
+
+namespace madme {
+
+extern thread_local char g_err[512];
+inline int fail(int code, const char* fmt, const char* a = "", const char* b = "") {
+  snprintf(g_err, sizeof g_err, fmt, a, b);
+  return code;
+}
+inline int cuda_fail(cudaError_t e, const char* where) { return fail(ME_ECUDA, "%s: %s", where, cudaGetErrorString(e)); }
+#define CU(call)                                                  \
+  do {                                                            \
+    cudaError_t e__ = (call);                                     \
+    if (e__ != cudaSuccess) return madme::cuda_fail(e__, #call);  \
+  } while (0)
+
+enum Proc { P_EPEM = 0, P_GGTT = 1, P_GGTTG = 2, P_GGTTGG = 3 };
+
+}  // namespace madme
+
+struct me_handle {
+  madme::Proc proc;
+  me_params par;
+  int n_ext, n_hel, n_flow, n_diag, n_terms, n_diag4g, n_cur;
+  double mass, scale, flops;
+  double masses[madme::PS_MAX_FINAL];
+  unsigned gluon_mask;
+  // launch geometry of the CTA-per-W-events kernels
+  int warps, grid, smem_bytes, regs, ctas_per_sm, sms;
+  // vegas scratch (grown on demand, never shrunk)
+  double* f_scratch = nullptr;
+  unsigned long long* idx_scratch = nullptr;
+  long long scratch_ev = 0;
+  double* partial = nullptr;
+  long long partial_len = 0;
+  double* sums_d = nullptr;
+  double* sums_h = nullptr;  // pinned
+};
+
+namespace madme {
+
+struct ProcOps {
+  int (*fill)(me_handle* h);  // constants of the generated program + launch geometry
+  int (*eval)(me_handle* h, const double* mom, double* me2, double* hel, long long n, cudaStream_t s);
+  int (*integrand)(me_handle* h, const VegasArgs& a, double* f, unsigned long long* idx, int words, cudaStream_t s);
+};
+#define MADME_DECLARE_OPS(P) const ProcOps* ops_##P##_eval(); const ProcOps* ops_##P##_vegas();
+MADME_DECLARE_OPS(epem_mupmum)
+MADME_DECLARE_OPS(gg_ttx)
+MADME_DECLARE_OPS(gg_ttxg)
+MADME_DECLARE_OPS(gg_ttxgg)
+
+}  // namespace madme

@@ -1,28 +1,14 @@
 // madme.cu — the C ABI of include/madme.h on top of the sm_100a kernels.  No CPU path: without a CUDA device
-// every compute call fails with ME_ENODEV.
-#include <cuda_runtime.h>
-#include <stdio.h>
-#include <stdlib.h>
-#include <string.h>
-
-#include "../../include/madme.h"
-#include "vegas_kernels.cuh"
+// every compute call fails with ME_ENODEV.  The per-process kernels are compiled in their own translation units
+// (proc_eval.cu, proc_vegas.cu with -DMADME_PROC=<process>) and reached through ProcOps.
+#include "common.cuh"
+#include "phase_space.cuh"
 
 using namespace madme;
 
-namespace {
+thread_local char madme::g_err[512] = "";
 
-thread_local char g_err[512] = "";
-int fail(int code, const char* fmt, const char* a = "", const char* b = "") {
-  snprintf(g_err, sizeof g_err, fmt, a, b);
-  return code;
-}
-int cuda_fail(cudaError_t e, const char* where) { return fail(ME_ECUDA, "%s: %s", where, cudaGetErrorString(e)); }
-#define CU(call)                                         \
-  do {                                                   \
-    cudaError_t e__ = (call);                            \
-    if (e__ != cudaSuccess) return cuda_fail(e__, #call); \
-  } while (0)
+namespace {
 
 bool have_device() {
   static int state = -1;
@@ -34,110 +20,6 @@ bool have_device() {
   return state == 1;
 }
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
-
-enum Proc { P_EPEM = 0, P_GGTT = 1, P_GGTTG = 2, P_GGTTGG = 3 };
-
-}  // namespace
-
-struct me_handle {
-  Proc proc;
-  me_params par;
-  int n_ext, n_hel, n_flow, n_diag, n_terms, n_diag4g, n_cur;
-  double mass, scale, flops;
-  double masses[PS_MAX_FINAL];
-  unsigned gluon_mask;
-  // launch geometry of the warp-per-event kernels
-  int warps, grid, smem_bytes, regs, ctas_per_sm, sms;
-  // vegas scratch (grown on demand, never shrunk)
-  double* f_scratch = nullptr;
-  unsigned long long* idx_scratch = nullptr;
-  long long scratch_ev = 0;
-  double* partial = nullptr;
-  long long partial_len = 0;
-  double* sums_d = nullptr;
-  double* sums_h = nullptr;  // pinned
-};
-
-namespace {
-
-// W (events = warps per CTA) is a run-time choice among the compiled instances; MADME_WARPS overrides it — the
-// threads-per-block scan of PAPER.md:78-84 (Fig. 3) is repeated with it.
-template <class P> struct ProcInfo {
-  template <int W> static int geom(int* regs, int* ctas) {
-    cudaFuncAttributes fa;
-    CU(cudaFuncGetAttributes(&fa, me_eval_kernel<P, W>));
-    const int bytes = W * EventSmem<P>::DOUBLES * 8;
-    if (cudaFuncSetAttribute(me_eval_kernel<P, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) != cudaSuccess ||
-        cudaFuncSetAttribute(vegas_integrand_kernel<P, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) != cudaSuccess) {
-      (void)cudaGetLastError();
-      *ctas = 0;
-      return ME_OK;
-    }
-    *regs = fa.numRegs;
-    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas, me_eval_kernel<P, W>, 32 * W, bytes));
-    return ME_OK;
-  }
-  static int fill(me_handle* h, int n4g) {
-    h->n_ext = P::N_EXT; h->n_hel = P::N_HEL; h->n_flow = P::N_FLOW; h->n_diag = P::N_DIAGRAMS;
-    h->n_terms = P::N_TERMS; h->n_diag4g = n4g; h->n_cur = P::N_CURRENTS; h->flops = P::FLOPS_PER_EVENT;
-    const double g2 = P::QED ? 4.0 * PS_PI * h->par.alpha_em : 4.0 * PS_PI * h->par.alpha_s;  // g^2
-    double c = 1.0;
-    for (int i = 0; i < P::COUPLING_POWER / 2; ++i) c *= g2;
-    h->scale = c / (double(P::CF_DEN) * double(P::AVG_DEN));
-    int dev = 0;
-    CU(cudaGetDevice(&dev));
-    CU(cudaDeviceGetAttribute(&h->sms, cudaDevAttrMultiProcessorCount, dev));
-    const int cand[4] = {1, 2, 4, 8};
-    int regs[4] = {0, 0, 0, 0}, ctas[4] = {0, 0, 0, 0}, rc;
-    if ((rc = geom<1>(&regs[0], &ctas[0])) || (rc = geom<2>(&regs[1], &ctas[1])) || (rc = geom<4>(&regs[2], &ctas[2])) ||
-        (rc = geom<8>(&regs[3], &ctas[3])))
-      return rc;
-    int pick = -1;
-    const char* env = getenv("MADME_WARPS");
-    if (env) {
-      for (int k = 0; k < 4; ++k)
-        if (atoi(env) == cand[k] && ctas[k] > 0) pick = k;
-      if (pick < 0) return fail(ME_EINVAL, "MADME_WARPS must be 1, 2, 4 or 8 (and fit on an SM)%s%s");
-    } else {
-      // most resident warps per SM; ties go to the larger CTA (fuller lanes in the current stages)
-      int best = 0;
-      for (int k = 0; k < 4; ++k)
-        if (cand[k] * ctas[k] >= best && ctas[k] > 0) { best = cand[k] * ctas[k]; pick = k; }
-      if (pick < 0) return fail(ME_ECUDA, "me_eval kernel does not fit on an SM%s%s");
-    }
-    h->warps = cand[pick];
-    h->regs = regs[pick];
-    h->ctas_per_sm = ctas[pick];
-    h->smem_bytes = h->warps * EventSmem<P>::DOUBLES * 8;
-    h->grid = h->sms * h->ctas_per_sm;
-    return ME_OK;
-  }
-  static int eval(me_handle* h, const double* mom, double* me2, double* hel, long long n, cudaStream_t s) {
-    const long long need = (n + h->warps - 1) / h->warps;
-    const int grid = static_cast<int>(need < h->grid ? need : h->grid), T = 32 * h->warps;
-    switch (h->warps) {
-      case 1: me_eval_kernel<P, 1><<<grid, T, h->smem_bytes, s>>>(mom, me2, hel, n, h->mass, h->scale); break;
-      case 2: me_eval_kernel<P, 2><<<grid, T, h->smem_bytes, s>>>(mom, me2, hel, n, h->mass, h->scale); break;
-      case 4: me_eval_kernel<P, 4><<<grid, T, h->smem_bytes, s>>>(mom, me2, hel, n, h->mass, h->scale); break;
-      default: me_eval_kernel<P, 8><<<grid, T, h->smem_bytes, s>>>(mom, me2, hel, n, h->mass, h->scale); break;
-    }
-    CU(cudaGetLastError());
-    return ME_OK;
-  }
-  static int integrand(me_handle* h, const VegasArgs& a, double* f, unsigned long long* idx, int words, cudaStream_t s) {
-    const int T = 32 * h->warps;
-    const long long need = (a.n_ev + T - 1) / T;
-    const int grid = static_cast<int>(need < h->grid ? need : h->grid);
-    switch (h->warps) {
-      case 1: vegas_integrand_kernel<P, 1><<<grid, T, h->smem_bytes, s>>>(a, f, idx, words); break;
-      case 2: vegas_integrand_kernel<P, 2><<<grid, T, h->smem_bytes, s>>>(a, f, idx, words); break;
-      case 4: vegas_integrand_kernel<P, 4><<<grid, T, h->smem_bytes, s>>>(a, f, idx, words); break;
-      default: vegas_integrand_kernel<P, 8><<<grid, T, h->smem_bytes, s>>>(a, f, idx, words); break;
-    }
-    CU(cudaGetLastError());
-    return ME_OK;
-  }
-};
 
 // ---- stand-alone phase-space kernels: one event per thread ------------------------------------------------
 __global__ void philox_kernel(unsigned long long seed, unsigned iteration, long long first, int n_dim, double* __restrict__ out,
@@ -272,10 +154,10 @@ int me_init(const char* process, const me_params* params, me_handle** out) {
   if (pr == P_GGTTGG) h->gluon_mask = 0xC;
   int rc;
   switch (pr) {
-    case P_EPEM: rc = ProcInfo<epem_mupmum>::fill(h, 0); break;
-    case P_GGTT: rc = ProcInfo<gg_ttx>::fill(h, 0); break;
-    case P_GGTTG: rc = ProcInfo<gg_ttxg>::fill(h, 1); break;
-    default: rc = ProcInfo<gg_ttxgg>::fill(h, 18); break;
+    case P_EPEM: rc = ops_epem_mupmum_eval()->fill(h); break;
+    case P_GGTT: rc = ops_gg_ttx_eval()->fill(h); break;
+    case P_GGTTG: rc = ops_gg_ttxg_eval()->fill(h); break;
+    default: rc = ops_gg_ttxgg_eval()->fill(h); break;
   }
   if (rc == ME_OK) {
     cudaError_t e = cudaMalloc(&h->sums_d, sizeof(double) * (3 + VEGAS_MAX_DIM * VEGAS_MAX_BINS));
@@ -326,10 +208,10 @@ static int eval_common(me_handle* h, const double* momenta, double* me2, double*
   if (n_ev == 0) return ME_OK;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   switch (h->proc) {
-    case P_EPEM: return ProcInfo<epem_mupmum>::eval(h, momenta, me2, hel, n_ev, s);
-    case P_GGTT: return ProcInfo<gg_ttx>::eval(h, momenta, me2, hel, n_ev, s);
-    case P_GGTTG: return ProcInfo<gg_ttxg>::eval(h, momenta, me2, hel, n_ev, s);
-    default: return ProcInfo<gg_ttxgg>::eval(h, momenta, me2, hel, n_ev, s);
+    case P_EPEM: return ops_epem_mupmum_eval()->eval(h, momenta, me2, hel, n_ev, s);
+    case P_GGTT: return ops_gg_ttx_eval()->eval(h, momenta, me2, hel, n_ev, s);
+    case P_GGTTG: return ops_gg_ttxg_eval()->eval(h, momenta, me2, hel, n_ev, s);
+    default: return ops_gg_ttxgg_eval()->eval(h, momenta, me2, hel, n_ev, s);
   }
 }
 int me_eval(me_handle* h, const double* momenta, double* me2, long long n_ev, void* stream) {
@@ -447,9 +329,9 @@ int vegas_integrand(me_handle* h, const vegas_grid* g, double sqrt_s, long long 
   a.gluon_mask = h->gluon_mask; a.ptj_min = h->par.ptj_min; a.dr_min = h->par.dr_min; a.mass = h->mass; a.scale = h->scale;
   double* f = f_out ? f_out : h->f_scratch;
   switch (h->proc) {
-    case P_GGTT: rc = ProcInfo<gg_ttx>::integrand(h, a, f, h->idx_scratch, words, s); break;
-    case P_GGTTG: rc = ProcInfo<gg_ttxg>::integrand(h, a, f, h->idx_scratch, words, s); break;
-    default: rc = ProcInfo<gg_ttxgg>::integrand(h, a, f, h->idx_scratch, words, s); break;
+    case P_GGTT: rc = ops_gg_ttx_vegas()->integrand(h, a, f, h->idx_scratch, words, s); break;
+    case P_GGTTG: rc = ops_gg_ttxg_vegas()->integrand(h, a, f, h->idx_scratch, words, s); break;
+    default: rc = ops_gg_ttxgg_vegas()->integrand(h, a, f, h->idx_scratch, words, s); break;
   }
   if (rc) return rc;
   vegas_reduce_chunks<<<n_chunks, 512, 0, s>>>(f, h->idx_scratch, words, D, nb, n_ev, chunk, h->partial);

@@ -88,28 +88,25 @@ __device__ __forceinline__ double cta_me2(double* smem, double mass, double scal
   }
   cta_sync<W>();
   double* base = smem + 4 * P::N_EXT;  // event e's scratch = base + e * STRIDE
-  int row = 0;
-#pragma unroll 1
-  for (int s = 0; s < P::N_BASE_STAGES; ++s) {
-    const int end = P::base_end(s);
-    run_rows<W>(tab, row, end, P::N_ROWS, base, STRIDE, mass);
-    row = end;
-    cta_sync<W>();
-  }
   static_assert(P::N_HEL_EVAL <= 32, "one helicity combination per lane");
   double jr[P::N_FLOW], ji[P::N_FLOW];
 #pragma unroll
   for (int f = 0; f < P::N_FLOW; ++f) { jr[f] = 0.0; ji[f] = 0.0; }
   const double* my = base + warp * STRIDE;
-#pragma unroll
-  for (int r = 0; r < P::N_ROUNDS; ++r) {
-    run_rows<W>(tab, row, P::raw_end(r), P::N_ROWS, base, STRIDE, mass);
+  int row = 0;
+  // ONE copy of the row interpreter and one of each round's dot products in the instruction stream: the phase loop
+  // must stay rolled (unrolled it is > 600 KB of SASS and the kernel starves on instruction fetch)
+#pragma unroll 1
+  for (int p = 0; p < P::N_PHASES; ++p) {
+    const int end = P::phase_end(p);
+    run_rows<W>(tab, row, end, P::N_ROWS, base, STRIDE, mass);
+    row = end;
     cta_sync<W>();
-    run_rows<W>(tab, P::raw_end(r), P::combo_end(r), P::N_ROWS, base, STRIDE, mass);
-    row = P::combo_end(r);
-    cta_sync<W>();
-    if (lane < P::N_HEL_EVAL) P::dots(r, my, lane, jr, ji);
-    if (r + 1 < P::N_ROUNDS) cta_sync<W>();
+    const int r = P::phase_dots(p);
+    if (r >= 0) {
+      if (lane < P::N_HEL_EVAL) P::dots(r, my, lane, jr, ji);
+      cta_sync<W>();
+    }
   }
   double v = (lane < P::N_HEL_EVAL) ? P::colour(jr, ji) : 0.0;
   if (hel_out && lane < P::N_HEL_EVAL) {  // full index: leg 0 at +1 is bit 0; the parity partner has every helicity flipped

@@ -1,0 +1,44 @@
+// proc_vegas.cu — the fused Vegas integrand for ONE process: compiled once per process with -DMADME_PROC=<process>.
+#include "common.cuh"
+#include "vegas_kernels.cuh"
+
+#ifndef MADME_PROC
+#error "compile with -DMADME_PROC=<process>"
+#endif
+#define MADME_CAT_(a, b, c) a##b##c
+#define MADME_CAT(a, b, c) MADME_CAT_(a, b, c)
+
+namespace madme {
+// a named namespace per (process, file): this file is compiled several times into one library
+namespace MADME_CAT(tu_, MADME_PROC, _v) {
+using P = MADME_PROC;
+
+template <int W> int launch(me_handle* h, const VegasArgs& a, double* f, unsigned long long* idx, int words, cudaStream_t s) {
+  static bool prepared = false;
+  if (!prepared) {
+    CU(cudaFuncSetAttribute(vegas_integrand_kernel<P, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_bytes));
+    prepared = true;
+  }
+  int per_sm = 0;
+  CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, vegas_integrand_kernel<P, W>, 32 * W, h->smem_bytes));
+  if (per_sm < 1) return fail(ME_ECUDA, "vegas_integrand kernel does not fit on an SM%s%s");
+  const long long need = (a.n_ev + 32 * W - 1) / (32 * W), full = static_cast<long long>(h->sms) * per_sm;
+  vegas_integrand_kernel<P, W><<<static_cast<int>(need < full ? need : full), 32 * W, h->smem_bytes, s>>>(a, f, idx, words);
+  CU(cudaGetLastError());
+  return ME_OK;
+}
+
+int integrand(me_handle* h, const VegasArgs& a, double* f, unsigned long long* idx, int words, cudaStream_t s) {
+  switch (h->warps) {
+    case 1: return launch<1>(h, a, f, idx, words, s);
+    case 2: return launch<2>(h, a, f, idx, words, s);
+    case 4: return launch<4>(h, a, f, idx, words, s);
+    default: return launch<8>(h, a, f, idx, words, s);
+  }
+}
+
+const ProcOps ops = {nullptr, nullptr, integrand};
+}  // namespace tu_<process>
+
+const ProcOps* MADME_CAT(ops_, MADME_PROC, _vegas)() { return &MADME_CAT(tu_, MADME_PROC, _v)::ops; }
+}  // namespace madme

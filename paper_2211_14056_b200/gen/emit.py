@@ -222,11 +222,19 @@ def emit_process(name, n_rounds=None):
         w("    }")
         w("  }")
 
-    w("  static constexpr int N_ROWS = %d, N_BASE_STAGES = %d, N_ROUNDS = %d;" % (len(rows), len(base_ends), len(L.rounds)))
-    w("  // rows of base stage s end at base_end(s); round r: currents end at raw_end(r), combinations at combo_end(r)")
-    table_fn("base_end", base_ends)
-    table_fn("raw_end", raw_ends)
-    table_fn("combo_end", combo_ends)
+    # phases: rows up to phase_end(p), barrier, then (if phase_dots(p) >= 0) the dot products of that round, barrier
+    ph_end = list(base_ends)
+    ph_dots = [-1] * len(base_ends)
+    for r in range(len(L.rounds)):
+        if raw_ends[r] > (ph_end[-1] if ph_end else 0) and combo_ends[r] > raw_ends[r]:
+            ph_end.append(raw_ends[r])
+            ph_dots.append(-1)
+        ph_end.append(combo_ends[r])
+        ph_dots.append(r)
+    w("  static constexpr int N_ROWS = %d, N_ROUNDS = %d, N_PHASES = %d;" % (len(rows), len(L.rounds), len(ph_end)))
+    w("  // phase p: task rows up to phase_end(p), barrier, then the dot products of round phase_dots(p) (if >= 0), barrier")
+    table_fn("phase_end", ph_end)
+    table_fn("phase_dots", ph_dots)
     w("#define %s_TASK_TABLE { \\" % name.upper())
     for r4 in rows:
         w("  {%du,%du,%du,%du}, \\" % r4)

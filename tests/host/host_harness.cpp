@@ -41,13 +41,13 @@ template <class P> void eval(const double* mom, double* me2, long long n, double
       me_phase0(lane, 32, sm.data(), mom + e * 4 * P::N_EXT, P::N_EXT, P::N_SUB, Tables<P>::masks(), Tables<P>::kind(),
                 Tables<P>::massive(), Tables<P>::ext_off(), mass);
     int row = 0;
-    for (int s = 0; s < P::N_BASE_STAGES; ++s) { rows<P>(sm.data(), row, P::base_end(s), mass); row = P::base_end(s); }
     std::vector<double> jr(P::N_HEL_EVAL * P::N_FLOW, 0.0), ji(P::N_HEL_EVAL * P::N_FLOW, 0.0);
-    for (int r = 0; r < P::N_ROUNDS; ++r) {
-      rows<P>(sm.data(), row, P::raw_end(r), mass);
-      rows<P>(sm.data(), P::raw_end(r), P::combo_end(r), mass);
-      row = P::combo_end(r);
-      for (int h = 0; h < P::N_HEL_EVAL; ++h) P::dots(r, sm.data(), h, &jr[h * P::N_FLOW], &ji[h * P::N_FLOW]);
+    for (int p = 0; p < P::N_PHASES; ++p) {
+      rows<P>(sm.data(), row, P::phase_end(p), mass);
+      row = P::phase_end(p);
+      const int r = P::phase_dots(p);
+      if (r >= 0)
+        for (int h = 0; h < P::N_HEL_EVAL; ++h) P::dots(r, sm.data(), h, &jr[h * P::N_FLOW], &ji[h * P::N_FLOW]);
     }
     double s = 0;
     for (int h = 0; h < P::N_HEL_EVAL; ++h) {
