@@ -28,7 +28,7 @@ PROCESSES = ["epem_mupmum", "gg_ttx", "gg_ttxg", "gg_ttxgg"]
 
 def _compile(job):
     src, obj, defs = job
-    cmd = [NVCC] + CFLAGS + defs + ["-c", "-o", obj, os.path.join(CSRC, src)]
+    cmd = [NVCC] + CFLAGS + defs + os.environ.get("MADME_NVCC_FLAGS", "").split() + ["-c", "-o", obj, os.path.join(CSRC, src)]
     res = subprocess.run(cmd, capture_output=True, text=True)
     return " ".join(cmd) + "\n" + res.stdout + res.stderr, res.returncode
 

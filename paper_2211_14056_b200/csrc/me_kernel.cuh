@@ -119,9 +119,13 @@ __device__ __forceinline__ double cta_me2(double* smem, double mass, double scal
   return 2.0 * v * scale;
 }
 
-// W events per CTA (blockDim.x = 32 W); persistent grid, batches of W consecutive events.
+// W events per CTA (blockDim.x = 32 W); persistent grid, batches of W consecutive events.  MADME_OCC_WARPS is the number
+// of resident warps per SM the register allocation is bounded for (8 -> up to 255 registers, 12 -> 168).
+#ifndef MADME_OCC_WARPS
+#define MADME_OCC_WARPS 8
+#endif
 template <class P, int W>
-__global__ void __launch_bounds__(32 * W) me_eval_kernel(const double* __restrict__ momenta, double* __restrict__ me2,
+__global__ void __launch_bounds__(32 * W, (MADME_OCC_WARPS + W - 1) / W) me_eval_kernel(const double* __restrict__ momenta, double* __restrict__ me2,
                                                          double* __restrict__ me2_hel, long long n_ev, double mass, double scale) {
   extern __shared__ __align__(16) double smem[];
   constexpr int STRIDE = EventSmem<P>::DOUBLES;

@@ -8,9 +8,11 @@
 // Scratch layout of one event (doubles), produced by gen/emit.py for each process:
 //   subset blocks  : 8 doubles per used leg subset S:  K_S[4], 1/K_S^2, 1/(K_S^2 - m_t^2), pad, pad
 //   wavefunctions  : object o over the leg set S has one helicity variant per combination of the helicities of
-//                    ITS OWN legs ("helicity recycling"), stored as
-//                    [component c = 0..3][variant v][re, im]   ->  double offset  OFF_o + 2*(c*nv + v)
-//                    so that the 32 lanes' 16-byte loads of one component fall into <= 128 contiguous bytes.
+//                    ITS OWN legs ("helicity recycling").  Storage is in GROUPS of 4 lines x 128 B, one line per
+//                    component; o owns nv consecutive 16-byte slots of each line:
+//                    component c, variant v  ->  double offset  OFF_o + 16 c + 2 v        (ME_WF_STRIDE = 16)
+//                    so that the 32 lanes' 16-byte loads of one component fall into <= 128 contiguous bytes (one
+//                    shared-memory wavefront) and the four components are one address + immediate offsets.
 //   Leg 0 is fixed at helicity +1 (parity: |M(-h)|^2 = |M(h)|^2, the sum is doubled at the end), so
 //   variant index v = sum_k b_{l_k} 2^k over the legs l_0 < l_1 < ... of S OTHER THAN LEG 0, b = 0 for helicity -1,
 //   1 for +1, and nv = 2^(number of those legs).
@@ -30,11 +32,10 @@ namespace madme {
 //   x: out | a << 16                      (offsets in doubles into the event's scratch)
 //   y: b   | c << 16
 //   z: ksub_out | ksub_a << 8 | ksub_b << 16 | op << 24 | massive << 27 | open << 28      (ksub = subset index)
-//   w: log2(nv) of out | of a << 4 | of b << 8 | of c << 12 | n_members << 16 | phase codes (2 bits each) << 20
-// component stride of an object = 2 nv doubles.  The three colour terms of a four-gluon current are laid out
-// back to back (out, out + 8 nv, out + 16 nv).  OP_COMBO: out = sum_j i^{k_j} member_j with members (a, b, c, and
-// a fourth in the ksub_a/ksub_b bytes' place: z & 0xffff).  Rows are grouped in warp-wide iterations of one op
-// (padded with OP_NOP), iterations in stages; a warp barrier separates stages.
+//   w: n_members << 16 | phase codes (2 bits each) << 20                                    (OP_COMBO)
+// OP_VVVV writes the three colour terms of a four-gluon current: out, (z >> 8) & 0xffff and w & 0xffff.
+// OP_COMBO: out = sum_j i^{k_j} member_j with members (a, b, c, and a fourth in z & 0xffff).  Rows come in groups of
+// one op (padded with OP_NOP to multiples of 4 rows), groups in stages; a barrier separates stages.
 struct MeRow { unsigned x, y, z, w; };
 enum MeOp { OP_FFV_ROW = 0, OP_FFV_COL = 1, OP_FFV_VEC = 2, OP_VVV = 3, OP_VVVV = 4, OP_COMBO = 5, OP_NOP = 7 };
 #if defined(__CUDA_ARCH__)
@@ -43,7 +44,9 @@ enum MeOp { OP_FFV_ROW = 0, OP_FFV_COL = 1, OP_FFV_VEC = 2, OP_VVV = 3, OP_VVVV 
 #define ME_FENCE()
 #endif
 
-ME_HD wf4 ld_wf(const double* p, int stride) {
+constexpr int ME_WF_STRIDE = 16;  // doubles between the components of a stored wavefunction (one 128-byte line)
+ME_HD wf4 ld_wf(const double* p) {
+  constexpr int stride = ME_WF_STRIDE;
   wf4 w;
 #if defined(__CUDA_ARCH__)
   for (int c = 0; c < 4; ++c) {
@@ -55,7 +58,8 @@ ME_HD wf4 ld_wf(const double* p, int stride) {
 #endif
   return w;
 }
-ME_HD void st_wf(double* p, int stride, const wf4& w) {
+ME_HD void st_wf(double* p, const wf4& w) {
+  constexpr int stride = ME_WF_STRIDE;
 #if defined(__CUDA_ARCH__)
   for (int c = 0; c < 4; ++c) *reinterpret_cast<double2*>(p + c * stride) = make_double2(w.c[c].re, w.c[c].im);
 #else
@@ -102,10 +106,10 @@ ME_HD void me_phase0(int idx, int step, double* sm, const double* mom, int n_ext
     wf4 w[2];
     external_wavefunction(leg_kind[l], mom + 4 * l, leg_massive[l] ? mass : 0.0, w);
     if (l == 0) {
-      st_wf(sm + ext_off[0], 2, w[1]);  // leg 0: helicity +1 only (parity)
+      st_wf(sm + ext_off[0], w[1]);  // leg 0: helicity +1 only (parity)
     } else {
-      st_wf(sm + ext_off[l], 4, w[0]);
-      st_wf(sm + ext_off[l] + 2, 4, w[1]);
+      st_wf(sm + ext_off[l], w[0]);
+      st_wf(sm + ext_off[l] + 2, w[1]);
     }
   }
 }
@@ -120,22 +124,22 @@ ME_HD cplx times_ik(cplx x, int k) {
 ME_HD void me_run_row(const MeRow r, double* sm, double mass) {
   const int op = (r.z >> 24) & 7;
   if (op == OP_NOP) return;
-  const int out = r.x & 0xffff, so = 2 << (r.w & 15);
-  const wf4 A = ld_wf(sm + (r.x >> 16), 2 << ((r.w >> 4) & 15));
+  const int out = r.x & 0xffff;
+  const wf4 A = ld_wf(sm + (r.x >> 16));
   if (op == OP_COMBO) {
     // colour-ordered combination of currents over the same legs (same variant, same stride)
     const int n = (r.w >> 16) & 15;
     wf4 acc = A;  // the first member always enters with coefficient 1
     const int off[3] = {static_cast<int>(r.y & 0xffff), static_cast<int>(r.y >> 16), static_cast<int>(r.z & 0xffff)};
     for (int j = 1; j < n; ++j) {
-      const wf4 x = ld_wf(sm + off[j - 1], so);
+      const wf4 x = ld_wf(sm + off[j - 1]);
       const int k = (r.w >> (20 + 2 * j)) & 3;
       for (int c = 0; c < 4; ++c) acc.c[c] = acc.c[c] + times_ik(x.c[c], k);
     }
-    st_wf(sm + out, so, acc);
+    st_wf(sm + out, acc);
     return;
   }
-  const wf4 B = ld_wf(sm + (r.y & 0xffff), 2 << ((r.w >> 8) & 15));
+  const wf4 B = ld_wf(sm + (r.y & 0xffff));
   const double* ks = sm + 8 * (r.z & 0xff);
   const bool massive = (r.z >> 27) & 1;
   const bool open = (r.z >> 28) & 1;  // the current stops at its vertex: no propagator (U side of a propagator cut)
@@ -143,21 +147,21 @@ ME_HD void me_run_row(const MeRow r, double* sm, double mass) {
   const double invk2 = open ? 1.0 : ks[4];
   if (op == OP_FFV_ROW) {
     const wf4 x = slash_row(A, B);
-    st_wf(sm + out, so, open ? x : prop_row(ld_k(ks), -1.0, m, massive ? ks[5] : ks[4], x));
+    st_wf(sm + out, open ? x : prop_row(ld_k(ks), -1.0, m, massive ? ks[5] : ks[4], x));
   } else if (op == OP_FFV_COL) {
     const wf4 x = slash_col(B, A);
-    st_wf(sm + out, so, open ? x : prop_col(ld_k(ks), 1.0, m, massive ? ks[5] : ks[4], x));
+    st_wf(sm + out, open ? x : prop_col(ld_k(ks), 1.0, m, massive ? ks[5] : ks[4], x));
   } else if (op == OP_FFV_VEC) {
-    st_wf(sm + out, so, ffv_vec(A, B, invk2));
+    st_wf(sm + out, ffv_vec(A, B, invk2));
   } else if (op == OP_VVV) {
-    st_wf(sm + out, so, vvv_vec(A, ld_k(sm + 8 * ((r.z >> 8) & 0xff)), B, ld_k(sm + 8 * ((r.z >> 16) & 0xff)), invk2));
+    st_wf(sm + out, vvv_vec(A, ld_k(sm + 8 * ((r.z >> 8) & 0xff)), B, ld_k(sm + 8 * ((r.z >> 16) & 0xff)), invk2));
   } else {
-    const wf4 C = ld_wf(sm + (r.y >> 16), 2 << ((r.w >> 12) & 15));
+    const wf4 C = ld_wf(sm + (r.y >> 16));
     wf4 t1, t2, t3;
     vvvv_vec(A, B, C, invk2, t1, t2, t3);
-    st_wf(sm + out, so, t1);
-    st_wf(sm + out + 4 * so, so, t2);
-    st_wf(sm + out + 8 * so, so, t3);
+    st_wf(sm + out, t1);
+    st_wf(sm + ((r.z >> 8) & 0xffff), t2);
+    st_wf(sm + (r.w & 0xffff), t3);
   }
 }
 

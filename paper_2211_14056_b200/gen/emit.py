@@ -22,7 +22,7 @@ OPCODE = {"FFV_ROW": 0, "FFV_COL": 1, "FFV_VEC": 2, "VVV": 3, "VVVV1": 4}
 OP_COMBO, OP_NOP = 5, 7
 HERE = os.path.dirname(os.path.abspath(__file__))
 OUT_DIR = os.path.join(os.path.dirname(HERE), "csrc", "generated")
-N_ROUNDS = int(os.environ.get("MADME_GEN_ROUNDS", "6"))   # shared-memory footprint knob (see Layout)
+N_ROUNDS = int(os.environ.get("MADME_GEN_ROUNDS", "4"))   # shared-memory footprint knob (see Layout)
 GROUP_PAD = 4   # rows of one op come in multiples of this (a CTA of 8 events maps 4 rows x 8 events on a warp)
 
 # fp64 operation counts of the routines in csrc/helas.cuh as written (FMA = 2, add/mul = 1; complex mul = 1 mul +
@@ -92,20 +92,36 @@ class Layout:
         bins = [b for b in bins if b[1]]
         self.rounds = [sorted(b[1], key=lambda s: (len(s), s)) for b in bins]
         self.round_of = {s_: r for r, b in enumerate(self.rounds) for s_ in b}
-        off = 8 * len(subsets)
+        # Fixed-stride storage: a GROUP is 4 lines of 128 B (one line per wavefunction component); an object with nv
+        # variants owns nv consecutive 16-byte slots (aligned to nv) in each line, so component c of variant v sits at
+        # double offset  group*64 + c*16 + (slot+v)*2 : the four component loads of a wavefunction are ONE address plus
+        # the immediates 0, 128, 256, 384 bytes, whatever nv is.
+        start = 8 * len(subsets)
+        start = ((start + 15) // 16) * 16
         self.off = {}
-        for o in self.base:
-            self.off[o.id] = off
-            off += 8 * self.nv(o)
-        self.base_doubles = off
-        tmax = off
+
+        def allocate(obj_list, first_group_off):
+            groups = []          # free slot bitmaps
+            for o in sorted(obj_list, key=lambda o: (-self.nv(o), o.id)):
+                nv = self.nv(o)
+                assert nv <= 8
+                for gi, used in enumerate(groups):
+                    slot = next((s0 for s0 in range(0, 8, nv) if not any(used[s0:s0 + nv])), None)
+                    if slot is not None:
+                        break
+                else:
+                    groups.append([False] * 8)
+                    gi, slot, used = len(groups) - 1, 0, groups[-1]
+                for k in range(nv):
+                    used[slot + k] = True
+                self.off[o.id] = first_group_off + gi * 64 + slot * 2
+            return first_group_off + len(groups) * 64
+
+        base_end = allocate(self.base, start)
+        self.base_doubles = base_end
+        tmax = base_end
         for r in range(len(self.rounds)):
-            t = off
-            for o in objs:
-                if o.id in self.split_of and self.round_of[self.split_of[o.id]] == r:
-                    self.off[o.id] = t
-                    t += 8 * self.nv(o)
-            tmax = max(tmax, t)
+            tmax = max(tmax, allocate([o for o in objs if o.id in self.split_of and self.round_of[self.split_of[o.id]] == r], base_end))
         self.smem_doubles = tmax
 
     def nv(self, o):
@@ -164,19 +180,25 @@ def emit_process(name, n_rounds=None):
                     continue
                 args = [P.objs[a] for a in o.args]
                 nv = L.nv(o)
+                sibs = []
                 if opn == "VVVV1":
                     sibs = [x for x in L.objs if x.op in ("VVVV2", "VVVV3") and x.args == o.args and x.legs == o.legs and x.prop == o.prop]
                     sibs.sort(key=lambda x: x.op)
-                    assert len(sibs) == 2 and L.off[sibs[0].id] == L.off[o.id] + 8 * nv and L.off[sibs[1].id] == L.off[o.id] + 16 * nv
+                    assert len(sibs) == 2
                 massive = 1 if (o.type[0] in "OI" and P.legs[[l for l in o.legs if P.legs[l].kind >= 2][0]].massive) else 0
                 for v in range(nv):
                     offs = [L.off[a.id] + 2 * variant_index(a.legs, o.legs, v) for a in args] + [0]
-                    lgs = [lg(L.nv(a)) for a in args] + [0]
                     assert max(offs) < 65536 and L.off[o.id] + 2 * v < 65536
                     x = (L.off[o.id] + 2 * v) | (offs[0] << 16)
                     y = offs[1] | ((offs[2] if len(args) > 2 else 0) << 16)
-                    z = sub_i(o) | (sub_i(args[0]) << 8) | (sub_i(args[1]) << 16) | (OPCODE[opn] << 24) | (massive << 27) | ((0 if o.prop else 1) << 28)
-                    wv = lg(nv) | (lgs[0] << 4) | (lgs[1] << 8) | ((lgs[2] if len(args) > 2 else 0) << 12)
+                    flags = (OPCODE[opn] << 24) | (massive << 27) | ((0 if o.prop else 1) << 28)
+                    if sibs:   # four-gluon current: no argument momenta needed; the two sibling outputs take their place
+                        z = sub_i(o) | ((L.off[sibs[0].id] + 2 * v) << 8) | flags
+                        wv = L.off[sibs[1].id] + 2 * v
+                        assert L.off[sibs[0].id] + 2 * v < 65536
+                    else:
+                        z = sub_i(o) | (sub_i(args[0]) << 8) | (sub_i(args[1]) << 16) | flags
+                        wv = 0
                     rows.append((x, y, z, wv))
                     cur_flops += FLOPS["VVVV" if opn == "VVVV1" else opn][0 if o.prop else 1]
             pad(GROUP_PAD)
@@ -196,7 +218,7 @@ def emit_process(name, n_rounds=None):
                 x = (L.off[o.id] + 2 * v) | (m[0] << 16)
                 y = m[1] | (m[2] << 16)
                 z = m[3] | (OP_COMBO << 24)
-                wv = lg(nv) | (lg(nv) << 4) | (len(coefs) << 16) | (k[1] << 22) | (k[2] << 24) | (k[3] << 26)
+                wv = (len(coefs) << 16) | (k[1] << 22) | (k[2] << 24) | (k[3] << 26)
                 rows.append((x, y, z, wv))
                 cur_flops += 8 * (len(coefs) - 1)
         pad(32)
@@ -250,7 +272,7 @@ def emit_process(name, n_rounds=None):
     def ldw(oid):
         o = P.objs[oid]
         terms = ["%d * b%d" % (2 << k, l) for k, l in enumerate(bits_of(o.legs))]
-        return "ld_wf(sm + %s, %d)" % (" + ".join([str(L.off[oid])] + terms), 2 * L.nv(o))
+        return "ld_wf(sm + %s)" % " + ".join([str(L.off[oid])] + terms)
 
     zcode = {1: 0, 1j: 1, -1: 2, -1j: 3}
     by_split = {}
