@@ -104,7 +104,7 @@ def run_reference(args, workload):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--events", type=int, default=0, help="events per step per GPU (default: the workload's n_events)")
     ap.add_argument("--workload", default="config3", choices=["config3", "config4", "config2", "config1"])
