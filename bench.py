@@ -84,7 +84,8 @@ def run_reference(args, workload):
     if int(os.environ.get("RANK", "0")) != 0:
         return
     rate0, _, cores = oracle_rate(workload, 256)
-    n = max(256, min(1 << 16, int(rate0 * 60.0 / max(1, args.steps + args.warmup))))
+    budget = float(os.environ.get("MADME_REF_SECONDS", "60"))   # total CPU-arm wall time to aim for
+    n = max(256, min(1 << 16, int(rate0 * budget / max(1, args.steps + args.warmup))))
     for _ in range(args.warmup):
         oracle_rate(workload, n)
     t = 0.0
@@ -128,8 +129,8 @@ def main():
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    n_ev = args.events or wl.n_events
-    first = rank * n_ev  # disjoint global event-index ranges: any sharding reproduces the same stream
+    from paper_2211_14056_b200.sharding import weak_shard
+    first, n_ev = weak_shard(rank, world, args.events or wl.n_events)  # disjoint global event-index ranges
     h = api.me_init(wl.process, PARAMS)
     stream = torch.cuda.current_stream()
     nf = len(wl.masses)
