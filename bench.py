@@ -25,7 +25,10 @@ if ROOT not in sys.path:
 
 METRIC = "gg->ttbar gg |M|^2 events/sec (fp64, 1 B200)"
 UNIT = "events/s"
-NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12  # SMs x DFMA lanes/SM x 2 flop x max SM clock (DESIGN.md §Roofline)
+NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12  # SMs x DFMA lanes/SM x 2 flop x max SM clock (DESIGN.md §6)
+# dram__bytes_read.sum + dram__bytes_write.sum of me_eval_kernel<gg_ttxgg, 8> per event, from the ncu --set full capture
+# summarised in profiles/r1_me_eval_summary.md (818.4 MB + 36.9 MB for 4 194 304 events; algorithmic: 200 B/event)
+NCU_DRAM_BYTES_PER_EVENT = {"gg_ttxgg": 203.9}
 
 
 class ClockSampler(threading.Thread):
@@ -267,7 +270,10 @@ def main():
                         "peak": NOMINAL_FP64_TFLOPS, "unit": "TFLOP/s", "frac": achieved / NOMINAL_FP64_TFLOPS,
                         "peak_source": "nominal fp64: 148 SMs x 64 DFMA lanes x 2 x 1.965 GHz (no fp64 entry in MEASURED_PEAKS.json)",
                         "peak_measured_dfma_chain": probe_tflops, "frac_of_measured": achieved / probe_tflops,
-                        "flops_per_event": flops_ev, "kernel_ms": kern_ms, "traffic": None},
+                        "flops_per_event": flops_ev, "kernel_ms": kern_ms,
+                        "traffic": (NCU_DRAM_BYTES_PER_EVENT[wl.process] * n_ev if (wl.process in NCU_DRAM_BYTES_PER_EVENT and not vegas) else None),
+                        "traffic_unit": "bytes per launch (ncu capture, profiles/r1_me_eval_summary.md)",
+                        "hbm_gbs_algorithmic": (32 * (nf + 2) + 8) * n_ev / (kern_ms * 1e-3) / 1e9},
            "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "clocks": clocks}
     if vegas:
         out["vegas"] = last

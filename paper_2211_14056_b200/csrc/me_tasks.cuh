@@ -133,8 +133,13 @@ ME_HD void me_run_row(const MeRow r, double* sm, double mass) {
     const int off[3] = {static_cast<int>(r.y & 0xffff), static_cast<int>(r.y >> 16), static_cast<int>(r.z & 0xffff)};
     for (int j = 1; j < n; ++j) {
       const wf4 x = ld_wf(sm + off[j - 1]);
+      // i^k = cr + i ci with cr, ci in {0, +-1}: four FMAs per component instead of a cascade of selects
       const int k = (r.w >> (20 + 2 * j)) & 3;
-      for (int c = 0; c < 4; ++c) acc.c[c] = acc.c[c] + times_ik(x.c[c], k);
+      const double cr = (k & 1) ? 0.0 : 1.0 - k, ci = (k & 1) ? 2.0 - k : 0.0;
+      for (int c = 0; c < 4; ++c) {
+        acc.c[c].re = fma(cr, x.c[c].re, fma(-ci, x.c[c].im, acc.c[c].re));
+        acc.c[c].im = fma(cr, x.c[c].im, fma(ci, x.c[c].re, acc.c[c].im));
+      }
     }
     st_wf(sm + out, acc);
     return;
@@ -145,12 +150,15 @@ ME_HD void me_run_row(const MeRow r, double* sm, double mass) {
   const bool open = (r.z >> 28) & 1;  // the current stops at its vertex: no propagator (U side of a propagator cut)
   const double m = massive ? mass : 0.0;
   const double invk2 = open ? 1.0 : ks[4];
+  // open and propagated rows sit in different groups (gen/emit.py), so these branches are warp-uniform
   if (op == OP_FFV_ROW) {
     const wf4 x = slash_row(A, B);
-    st_wf(sm + out, open ? x : prop_row(ld_k(ks), -1.0, m, massive ? ks[5] : ks[4], x));
+    if (open) st_wf(sm + out, x);
+    else st_wf(sm + out, prop_row(ld_k(ks), -1.0, m, massive ? ks[5] : ks[4], x));
   } else if (op == OP_FFV_COL) {
     const wf4 x = slash_col(B, A);
-    st_wf(sm + out, open ? x : prop_col(ld_k(ks), 1.0, m, massive ? ks[5] : ks[4], x));
+    if (open) st_wf(sm + out, x);
+    else st_wf(sm + out, prop_col(ld_k(ks), 1.0, m, massive ? ks[5] : ks[4], x));
   } else if (op == OP_FFV_VEC) {
     st_wf(sm + out, ffv_vec(A, B, invk2));
   } else if (op == OP_VVV) {

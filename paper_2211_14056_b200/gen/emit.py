@@ -23,7 +23,7 @@ OP_COMBO, OP_NOP = 5, 7
 HERE = os.path.dirname(os.path.abspath(__file__))
 OUT_DIR = os.path.join(os.path.dirname(HERE), "csrc", "generated")
 N_ROUNDS = int(os.environ.get("MADME_GEN_ROUNDS", "4"))   # shared-memory footprint knob (see Layout)
-GROUP_PAD = 4   # rows of one op come in multiples of this (a CTA of 8 events maps 4 rows x 8 events on a warp)
+GROUP_PAD = int(os.environ.get("MADME_GEN_GROUP_PAD", "4"))   # rows of one op come in multiples of this (a CTA of 8 events maps 4 rows x 8 events on a warp)
 
 # fp64 operation counts of the routines in csrc/helas.cuh as written (FMA = 2, add/mul = 1; complex mul = 1 mul +
 # 1 fma per component = 6, complex fma = 8).  (propagated, open) forms.
@@ -174,9 +174,9 @@ def emit_process(name, n_rounds=None):
 
     def add_tasks(objs):
         nonlocal cur_flops
-        for opn in ("FFV_ROW", "FFV_COL", "FFV_VEC", "VVV", "VVVV1"):
+        for opn, prop in [(a, b) for a in ("FFV_ROW", "FFV_COL", "FFV_VEC", "VVV", "VVVV1") for b in (True, False)]:
             for o in objs:
-                if o.op != opn:
+                if o.op != opn or o.prop != prop:   # open and propagated currents in separate groups: uniform branches
                     continue
                 args = [P.objs[a] for a in o.args]
                 nv = L.nv(o)

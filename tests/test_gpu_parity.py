@@ -162,7 +162,7 @@ def test_me_eval_edge_cases(handles):
 
 def test_me_eval_sampled_at_bench_size(handles):
     """configs[3] in the launch configuration bench.py times (full persistent grid): sampled events against the oracle."""
-    n = 1 << 18
+    n = BY_NAME["config3"].n_events  # 2^24: BASELINE.json:configs[3] at full size
     r = api.philox_uniform(3, 0, 0, 16, n)
     mom, _ = api.rambo_generate(r, 1000.0, (173.0, 173.0, 0.0, 0.0), 0)
     got = api.me_eval(handles["gg_ttxgg"], mom).cpu().numpy()
@@ -173,6 +173,42 @@ def test_me_eval_sampled_at_bench_size(handles):
     momo, _ = ref.rambo_generate(ro, 1000.0, (173.0, 173.0, 0.0, 0.0), 0)
     want = ref.MatrixElementRef("gg_ttxgg").eval(momo)
     assert np.max(np.abs(got[idx] / want - 1)) < ME_RTOL
+    # properties that hold at any size: Bose symmetry under the exchange of the two final gluons (a different
+    # evaluation order inside the kernel: legs 4 and 5 swap roles in every leg split)
+    sub = mom[: 1 << 16].clone()
+    sub[:, [4, 5]] = sub[:, [5, 4]]
+    swapped = api.me_eval(handles["gg_ttxgg"], sub.contiguous()).cpu().numpy()
+    assert np.max(np.abs(swapped / got[: 1 << 16] - 1)) < ME_RTOL
+
+
+def test_vegas_full_size_config4(handles):
+    """configs[4] at full size (5 iterations x 2^24 events, D = 8, 50 bins) in the launch configuration bench.py times:
+    sampled per-event weights of iteration 0 against the oracle, the iteration results against each other."""
+    w = BY_NAME["config4"]
+    n = w.n_events
+    h = handles["gg_ttxgg"]
+    g = api.VegasGrid(8, VEGAS_BINS, VEGAS_ALPHA, w.seed, 1)
+    sums, f = api.vegas_integrand(h, g, w.sqrt_s, 0, n, want_f=True)
+    f = f.cpu().numpy()
+    idx = np.concatenate([np.arange(0, n, n // 61), [n - 1]])
+    go = ref.GridRef(8, VEGAS_BINS, VEGAS_ALPHA, seed=w.seed, ps_mode=1)
+    me = ref.MatrixElementRef("gg_ttxgg")
+    want = np.array([me.vegas_integrand(go, w.sqrt_s, int(i), 1, want_f=True)[1][0] for i in idx])
+    assert np.array_equal(f[idx] != 0, want != 0)
+    nz = want != 0
+    assert np.max(np.abs(f[idx][nz] / want[nz] - 1)) < ME_RTOL
+    s = sums.cpu().numpy()
+    assert abs(s[0] / f.sum() - 1) < 1e-12 and s[2] == np.count_nonzero(f)
+    res = [api.vegas_iterate(h, g, w.sqrt_s, n) for _ in range(5)]
+    I = np.array([r["integral"] for r in res])
+    sig = np.sqrt(np.array([r["variance"] for r in res]))
+    assert np.all(np.isfinite(I)) and np.all(sig > 0) and g.iteration == 5
+    wgt = 1 / sig ** 2
+    mean = (I * wgt).sum() / wgt.sum()
+    chi2 = (((I - mean) / sig) ** 2).sum() / 4
+    assert chi2 < 10 and sig[-1] < sig[0]  # consistent iterations; the adapted grid reduces the error
+    e = g.edges.cpu().numpy()
+    assert np.all(e[:, 0] == 0) and np.all(e[:, -1] == 1) and np.all(np.diff(e, axis=1) > 0)
 
 
 # ---- a2, a11, a12 Vegas pieces ----------------------------------------------------------------------------------
