@@ -59,15 +59,19 @@ __device__ __forceinline__ void run_row(const uint4 q, double* sm, double mass) 
   r.x = q.x; r.y = q.y; r.z = q.z; r.w = q.w;
   me_run_row(r, sm, mass);
 }
+// `first` holds this thread's first row of the stage on entry (fetched during the previous stage) and of the NEXT
+// stage on return (stages are multiples of 32 rows, so that row is end + t / W): its latency hides behind the barrier
+// and the dot products in between.
 template <int W>
 __device__ __forceinline__ void run_rows(const uint4* __restrict__ tab, int begin, int end, int n_rows, double* smem, int ev_stride,
-                                         double mass) {
+                                         double mass, uint4& first) {
   const int t = threadIdx.x;
   const int ev = t % W;
   double* sm = smem + ev * ev_stride;
   int row = begin + t / W;
+  uint4 a = first;
+  first = __ldg(tab + min(end + t / W, n_rows));
   if (row >= end) return;
-  uint4 a = __ldg(tab + row);
 #pragma unroll 1
   for (;;) {
     const uint4 b = __ldg(tab + min(row + 32, n_rows));
@@ -104,12 +108,13 @@ __device__ __forceinline__ double cta_me2(double* smem, double mass, double scal
   for (int f = 0; f < P::N_FLOW; ++f) { jr[f] = 0.0; ji[f] = 0.0; }
   const double* my = base + warp * STRIDE;
   int row = 0;
+  uint4 first = __ldg(tab + threadIdx.x / W);
   // ONE copy of the row interpreter and one of each round's dot products in the instruction stream: the phase loop
   // must stay rolled (unrolled it is > 600 KB of SASS and the kernel starves on instruction fetch)
 #pragma unroll 1
   for (int p = 0; p < P::N_PHASES; ++p) {
     const int end = P::phase_end(p);
-    run_rows<W>(tab, row, end, P::N_ROWS, base, STRIDE, mass);
+    run_rows<W>(tab, row, end, P::N_ROWS, base, STRIDE, mass, first);
     row = end;
     cta_sync<W>();
     const int r = P::phase_dots(p);
