@@ -222,14 +222,38 @@ def main():
         wgt_h = torch.empty(n_e2e, dtype=torch.float64).pin_memory()
         pass_h = torch.empty(n_e2e, dtype=torch.int32).pin_memory()
 
+        # chunked and double-buffered: the H2D copy of chunk k+1 and the D2H copy of chunk k-1 run on their own streams
+        # while chunk k is computed (the public API takes a stream; buffers are per chunk, so nothing is overwritten early)
+        n_chunks = 8
+        cs = n_e2e // n_chunks
+        s_in, s_out = torch.cuda.Stream(), torch.cuda.Stream()
+
         def e2e_step():
-            rand[:n_e2e].copy_(rand_h, non_blocking=True)
-            api.rambo_generate(rand[:n_e2e], wl.sqrt_s, wl.masses, wl.ps_mode, momenta=mom[:n_e2e], weights=wgt[:n_e2e])
-            api.apply_cuts(mom[:n_e2e], wl.is_gluon, PARAMS["ptj_min"], PARAMS["dr_min"], out=passed[:n_e2e])
-            api.me_eval(h, mom[:n_e2e], me2[:n_e2e])
-            me2_h.copy_(me2[:n_e2e], non_blocking=True)
-            wgt_h.copy_(wgt[:n_e2e], non_blocking=True)
-            pass_h.copy_(passed[:n_e2e], non_blocking=True)
+            ready = []
+            for c in range(n_chunks):
+                sl = slice(c * cs, (c + 1) * cs)
+                with torch.cuda.stream(s_in):
+                    rand[sl].copy_(rand_h[sl], non_blocking=True)
+                    ev = torch.cuda.Event()
+                    ev.record(s_in)
+                    ready.append(ev)
+            for c in range(n_chunks):
+                sl = slice(c * cs, (c + 1) * cs)
+                stream.wait_event(ready[c])
+                api.rambo_generate(rand[sl], wl.sqrt_s, wl.masses, wl.ps_mode, momenta=mom[sl], weights=wgt[sl])
+                api.apply_cuts(mom[sl], wl.is_gluon, PARAMS["ptj_min"], PARAMS["dr_min"], out=passed[sl])
+                api.me_eval(h, mom[sl], me2[sl])
+                done = torch.cuda.Event()
+                done.record(stream)
+                with torch.cuda.stream(s_out):
+                    s_out.wait_event(done)
+                    me2_h[sl].copy_(me2[sl], non_blocking=True)
+                    wgt_h[sl].copy_(wgt[sl], non_blocking=True)
+                    pass_h[sl].copy_(passed[sl], non_blocking=True)
+            fin = torch.cuda.Event()
+            fin.record(s_out)
+            stream.wait_event(fin)       # the step ends when its results are on the host
+            s_in.wait_stream(stream)     # and the next step's uploads may not overwrite inputs still in use
         e2e_step()
         barrier()
         t0.record(stream)
