@@ -45,6 +45,8 @@ struct me_handle {
   long long partial_len = 0;
   double* sums_d = nullptr;
   double* sums_h = nullptr;  // pinned
+  double* vegas_stage = nullptr;  // per-CTA survivor staging of the fused integrand (L2 resident)
+  long long vegas_stage_len = 0;
 };
 
 namespace madme {

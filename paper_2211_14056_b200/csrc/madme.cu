@@ -176,6 +176,7 @@ void me_free(me_handle* h) {
   if (h->partial) cudaFree(h->partial);
   if (h->sums_d) cudaFree(h->sums_d);
   if (h->sums_h) cudaFreeHost(h->sums_h);
+  if (h->vegas_stage) cudaFree(h->vegas_stage);
   delete h;
 }
 

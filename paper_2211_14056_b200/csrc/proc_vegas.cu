@@ -23,7 +23,16 @@ template <int W> int launch(me_handle* h, const VegasArgs& a, double* f, unsigne
   CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, vegas_integrand_kernel<P, W>, 32 * W, h->smem_bytes));
   if (per_sm < 1) return fail(ME_ECUDA, "vegas_integrand kernel does not fit on an SM%s%s");
   const long long need = (a.n_ev + 32 * W - 1) / (32 * W), full = static_cast<long long>(h->sms) * per_sm;
-  vegas_integrand_kernel<P, W><<<static_cast<int>(need < full ? need : full), 32 * W, h->smem_bytes, s>>>(a, f, idx, words);
+  const int grid = static_cast<int>(need < full ? need : full);
+  const long long stage_len = static_cast<long long>(grid) * 32 * W * (4 * (P::N_EXT - 2) + 2);
+  if (stage_len > h->vegas_stage_len) {
+    CU(cudaStreamSynchronize(s));  // an earlier launch may still read the old staging area
+    if (h->vegas_stage) cudaFree(h->vegas_stage);
+    h->vegas_stage = nullptr; h->vegas_stage_len = 0;
+    CU(cudaMalloc(&h->vegas_stage, sizeof(double) * stage_len));
+    h->vegas_stage_len = stage_len;
+  }
+  vegas_integrand_kernel<P, W><<<grid, 32 * W, h->smem_bytes, s>>>(a, f, idx, words, h->vegas_stage);
   CU(cudaGetLastError());
   return ME_OK;
 }
