@@ -154,6 +154,8 @@ def main():
 
     def step(k, timed):
         if vegas:
+            if world > 1:  # strong-sharded iteration over world * n_ev events with the single 3.2 KB exchange
+                return api.vegas_iterate_sharded(h, grid, wl.sqrt_s, n_ev * world)
             return api.vegas_iterate(h, grid, wl.sqrt_s, n_ev)
         api.philox_uniform(wl.seed, k, first, wl.n_dim, n_ev, out=rand)
         api.rambo_generate(rand, wl.sqrt_s, wl.masses, wl.ps_mode, momenta=mom, weights=wgt)

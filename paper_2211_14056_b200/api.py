@@ -237,3 +237,32 @@ def fp64_peak_probe(n_iter, stream=None):
     n = C.c_double()
     _check(lib().fp64_peak_probe(n_iter, _dev(sink, torch.float64, "sink"), C.byref(n), _stream(stream)))
     return n.value
+
+
+def vegas_iterate_sharded(h, grid, sqrt_s, n_total, group=None, stream=None):
+    """One Vegas iteration over `n_total` events split across the ranks of `group`: every rank
+    integrates its contiguous event range with the fused kernel (no communication), the per-rank sum vectors
+    (3 + n_dim * n_bins doubles) are all-gathered and added in FIXED rank order, and every rank refines its own copy
+    of the grid from the identical totals — so all ranks hold bit-identical grids and the result does not depend on
+    arrival order.  The exchange is latency-bound (3.2 KB); with backend "nccl" it runs over NVLink, with "gloo" over
+    the host.  Returns the same dict as vegas_iterate, identical on every rank."""
+    import torch.distributed as dist
+    from .sharding import combine_vegas_sums, strong_shard
+    rank = dist.get_rank(group) if dist.is_initialized() else 0
+    world = dist.get_world_size(group) if dist.is_initialized() else 1
+    first, n = strong_shard(rank, world, n_total)
+    sums, _ = vegas_integrand(h, grid, sqrt_s, first, n, stream=stream)
+    if world > 1:
+        on_host = dist.get_backend(group) == "gloo"
+        mine = sums.cpu() if on_host else sums
+        parts = [torch.empty_like(mine) for _ in range(world)]
+        dist.all_gather(parts, mine, group=group)
+        sums = combine_vegas_sums(parts).to(grid.edges.device)
+    n_dim, n_bins = grid.c.n_dim, grid.c.n_bins
+    vegas_refine(grid.edges, sums[3:].reshape(n_dim, n_bins).contiguous(), grid.c.alpha, stream=stream)
+    s = sums[:3].cpu()
+    N = float(n_total)
+    integral = float(s[0]) / N
+    grid.iteration = grid.iteration + 1
+    return dict(integral=integral, variance=(float(s[1]) / N - integral * integral) / (N - 1.0), sum_w=float(s[0]),
+                sum_w2=float(s[1]), n_pass=int(s[2]))
