@@ -11,7 +11,7 @@ import torch
 from oracle import ref
 from paper_2211_14056_b200 import api
 from paper_2211_14056_b200.workloads import BY_NAME, PARAMS, VEGAS_ALPHA, VEGAS_BINS
-from tests.helpers import closed_form_epem_mupmum, closed_form_gg_ttx, me_tolerance
+from tests.helpers import closed_form_epem_mupmum, closed_form_gg_ttx, me_tolerance, random_lorentz, transform
 
 pytestmark = pytest.mark.gpu
 ME_RTOL = 1e-10
@@ -140,6 +140,21 @@ def test_me_eval_per_helicity_and_parity(handles):
         nh = hel.shape[1]
         flipped = hel[:, (nh - 1) - np.arange(nh)]
         assert np.max(np.abs(hel - flipped) / tot[:, None]) < 1e-10
+
+
+@pytest.mark.parametrize("cfg,n", [("config1", 4096), ("config2", 4096), ("config3", 4096)])
+def test_me_eval_lorentz_invariance(handles, cfg, n):
+    """A property that needs no oracle: |M|^2 is invariant under a common rotation + boost of all momenta (the kernels
+    rebuild every wavefunction in the new frame: incoming legs off the z axis, different helicity spinors)."""
+    w = BY_NAME[cfg]
+    _, mom, _ = oracle_events(cfg, n)
+    h = handles[w.process]
+    base = api.me_eval(h, dev(mom)).cpu().numpy()
+    rng = np.random.default_rng(11)
+    for _ in range(3):
+        L = random_lorentz(rng, beta_max=0.8)
+        got = api.me_eval(h, dev(transform(mom, L))).cpu().numpy()
+        assert np.max(np.abs(got / base - 1)) < 1e-9  # boosted components are up to 3x larger: a few more ulps cancel
 
 
 def test_me_eval_edge_cases(handles):
