@@ -175,6 +175,28 @@ def test_me_eval_edge_cases(handles):
         api.me_eval(h, torch.zeros((4, 4, 4), dtype=torch.float32, device="cuda"))
 
 
+@pytest.mark.parametrize("n", [1, 7, 8, 9, 255, 257])
+def test_tiny_and_ragged_batches(handles, n):
+    """Batches smaller than one CTA (8 events) and ragged tails: the CTA-cooperative kernels recompute a valid event in
+    the idle slots and must neither store it nor disturb the live ones."""
+    _, mom, _ = oracle_events("config3", n)
+    want = ref.MatrixElementRef("gg_ttxgg").eval(mom)
+    guard = torch.full((n + 8,), -7.0, dtype=torch.float64, device="cuda")
+    api.me_eval(handles["gg_ttxgg"], dev(mom), guard[:n])
+    got = guard.cpu().numpy()
+    assert np.max(np.abs(got[:n] / want - 1)) < ME_RTOL and np.all(got[n:] == -7.0)
+    g_o = ref.GridRef(8, VEGAS_BINS, VEGAS_ALPHA, seed=4, ps_mode=1)
+    g_g = api.VegasGrid(8, VEGAS_BINS, VEGAS_ALPHA, 4, 1)
+    first = (1 << 33) + 11  # event indices beyond 32 bits reach Philox counter word 1
+    so, fo = ref.MatrixElementRef("gg_ttxgg").vegas_integrand(g_o, 1000.0, first, n, want_f=True)
+    sg, fg = api.vegas_integrand(handles["gg_ttxgg"], g_g, 1000.0, first, n, want_f=True)
+    fg = fg.cpu().numpy()
+    assert np.array_equal(fg != 0, fo != 0)
+    nz = fo != 0
+    assert nz.sum() == 0 or np.max(np.abs(fg[nz] / fo[nz] - 1)) < ME_RTOL
+    assert sg.cpu().numpy()[2] == so[2]
+
+
 def test_me_eval_sampled_at_bench_size(handles):
     """configs[3] in the launch configuration bench.py times (full persistent grid): sampled events against the oracle."""
     n = BY_NAME["config3"].n_events  # 2^24: BASELINE.json:configs[3] at full size
