@@ -173,12 +173,21 @@ int vegas_refine_ref(double* edges, int n_dim, int n_bins, const double* S, doub
   return 0;
 }
 
+// Toy gluon density of the hadronic mode (reading R-N3): g(x) = 3 x^-1.2 (1-x)^5.
+// A DECLARED toy parametrisation (no LHAPDF grids in the container); it only has to be the same on both sides.
+static double toy_gluon_density(double x) { return 3.0 * std::pow(x, -1.2) * std::pow(1.0 - x, 5); }
+
 // f(x) = jac_Vegas * W_ps * Theta_cuts * me2 / (2 s) * C,  C = 0.3893793721e9 pb GeV^2
+// ps_mode 2 (hadronic, D = 3n-4+2): x_1 = x[0], x_2 = x[1] are the momentum fractions, s_hat = x_1 x_2 s, the remaining
+// 3n-4 coordinates drive RAMBO "on diet" at sqrt(s_hat) in the partonic centre-of-mass frame (p_T, rapidity differences
+// and azimuths — everything the cuts use — are invariant under the boost along z), and
+// f = jac g(x_1) g(x_2) W_ps(s_hat) Theta me2 / (2 s_hat) C; events with sqrt(s_hat) <= sum of the final masses give 0.
 int vegas_integrand_ref(me_handle_ref* h, const vegas_grid_ref* g, double sqrt_s, long long first_event, long long n_ev,
                         double* sums, double* f_out) {
   if (!h || !g || !sums || h->P.qed) return -1;
   const int nf = h->P.n_ext - 2, D = g->n_dim, nb = g->n_bins;
-  if (D != (g->ps_mode == 0 ? 4 * nf : 3 * nf - 4)) return -4;
+  if (g->ps_mode < 0 || g->ps_mode > 2) return -4;
+  if (D != (g->ps_mode == 0 ? 4 * nf : g->ps_mode == 1 ? 3 * nf - 4 : 3 * nf - 2)) return -4;
   std::vector<double> masses(nf); std::vector<int> isg(nf);
   for (int i = 0; i < nf; ++i) { masses[i] = h->P.mass[2 + i]; isg[i] = h->P.kind[2 + i] == G_OUT; }
   std::vector<double> f(n_ev); std::vector<int> idx(size_t(n_ev) * D);
@@ -189,10 +198,21 @@ int vegas_integrand_ref(me_handle_ref* h, const vegas_grid_ref* g, double sqrt_s
     double y[4 * NMAX_FINAL], x[4 * NMAX_FINAL], mom[4 * NMAX];
     philox_uniforms(g->seed, uint64_t(g->iteration), uint64_t(first_event + e), D, y);
     const double jac = vegas_map_point(g->edges, D, nb, y, x, idx.data() + e * D);
-    const double wps = rambo_event(x, sqrt_s, masses.data(), nf, g->ps_mode, mom);
     double val = 0;
-    if (passes_cuts(mom, nf, isg.data(), h->par.ptj_min, h->par.dr_min))
-      val = jac * wps * tier1_me2(*h, mom) * flux * conv;
+    if (g->ps_mode == 2) {
+      double msum = 0;
+      for (int i = 0; i < nf; ++i) msum += masses[i];
+      const double rs_hat = std::sqrt(x[0] * x[1]) * sqrt_s;
+      if (rs_hat > msum) {
+        const double wps = rambo_event(x + 2, rs_hat, masses.data(), nf, 1, mom);
+        if (passes_cuts(mom, nf, isg.data(), h->par.ptj_min, h->par.dr_min))
+          val = jac * toy_gluon_density(x[0]) * toy_gluon_density(x[1]) * wps * tier1_me2(*h, mom) / (2.0 * rs_hat * rs_hat) * conv;
+      }
+    } else {
+      const double wps = rambo_event(x, sqrt_s, masses.data(), nf, g->ps_mode, mom);
+      if (passes_cuts(mom, nf, isg.data(), h->par.ptj_min, h->par.dr_min))
+        val = jac * wps * tier1_me2(*h, mom) * flux * conv;
+    }
     f[e] = val;
   }
   vegas_accumulate_ref(f.data(), idx.data(), D, nb, n_ev, sums);

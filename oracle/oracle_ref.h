@@ -39,7 +39,7 @@ typedef struct {
   double alpha;
   uint64_t seed;
   int iteration;
-  int ps_mode; /* 0 classic RAMBO (4n uniforms), 1 diet (3n-4) */
+  int ps_mode; /* 0 classic RAMBO (4n uniforms), 1 diet (3n-4), 2 hadronic: x1, x2 + diet (3n-2), toy gluon density */
 } vegas_grid_ref;
 typedef struct {
   double integral, variance;
