@@ -111,7 +111,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--events", type=int, default=0, help="events per step per GPU (default: the workload's n_events)")
-    ap.add_argument("--workload", default="config3", choices=["config3", "config4", "config2", "config1"])
+    ap.add_argument("--workload", default="config3", choices=["config3", "config4", "config4_hadronic", "config2", "config1"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -137,7 +137,7 @@ def main():
     h = api.me_init(wl.process, PARAMS)
     stream = torch.cuda.current_stream()
     nf = len(wl.masses)
-    vegas = wl.name == "config4"
+    vegas = wl.name.startswith("config4")
 
     # resident buffers
     if vegas:

@@ -49,7 +49,10 @@ typedef struct {
   double alpha;   /* damping exponent (1.5 in config 4) */
   uint64_t seed;
   int iteration;  /* Philox counter word 3; incremented by vegas_iterate */
-  int ps_mode;    /* 0 classic RAMBO (n_dim = 4 n_final), 1 RAMBO "on diet" (n_dim = 3 n_final - 4) */
+  int ps_mode;    /* 0 classic RAMBO (n_dim = 4 n_final), 1 RAMBO "on diet" (n_dim = 3 n_final - 4),
+                     2 hadronic (vegas_* only; n_dim = 3 n_final - 2): the first two coordinates are the momentum fractions
+                     x1, x2 weighted with a DECLARED toy gluon density 3 x^-1.2 (1-x)^5, sqrt_s is the hadronic energy,
+                     the rest drives RAMBO on diet at sqrt(x1 x2) sqrt_s (no PDF grids exist here) */
 } vegas_grid;
 
 typedef struct {

@@ -308,8 +308,8 @@ int vegas_integrand(me_handle* h, const vegas_grid* g, double sqrt_s, long long 
   if (!h || !g || !g->edges || !sums || n_ev < 0 || first_event < 0) return fail(ME_EINVAL, "vegas_integrand: null pointer or negative count%s%s");
   if (h->proc == P_EPEM) return fail(ME_EINVAL, "vegas_integrand: QCD processes only%s%s");
   const int nf = h->n_ext - 2, D = g->n_dim, nb = g->n_bins;
-  if ((g->ps_mode != 0 && g->ps_mode != 1) || D != (g->ps_mode == 0 ? 4 * nf : 3 * nf - 4))
-    return fail(ME_EDIM, "vegas_integrand: n_dim must be 4 n_final (ps_mode 0) or 3 n_final - 4 (ps_mode 1)%s%s");
+  if (g->ps_mode < 0 || g->ps_mode > 2 || D != (g->ps_mode == 0 ? 4 * nf : g->ps_mode == 1 ? 3 * nf - 4 : 3 * nf - 2))
+    return fail(ME_EDIM, "vegas_integrand: n_dim must be 4 n_final (ps_mode 0), 3 n_final - 4 (1) or 3 n_final - 2 (2)%s%s");
   if (nb < 1 || nb > VEGAS_MAX_BINS || D * nb + 3 > 512 * VEGAS_RED_PER_THREAD)
     return fail(ME_EDIM, "vegas_integrand: n_bins 1..255 and n_dim*n_bins <= 2045%s%s");
   if (!(sqrt_s > 2.0 * h->par.m_top)) return fail(ME_EINVAL, "vegas_integrand: sqrt_s below threshold%s%s");

@@ -203,6 +203,12 @@ __device__ __forceinline__ double rambo_event(const double* __restrict__ r, doub
   return w0 * rambo_massive<N>(sqrt_s, m, p);
 }
 
+// toy gluon density of the hadronic Vegas mode (DESIGN.md R-N3): a DECLARED toy, g(x) = 3 x^-1.2 (1-x)^5
+__device__ __forceinline__ double toy_gluon_density(double x) {
+  const double y = 1.0 - x, y2 = y * y;
+  return 3.0 * pow(x, -1.2) * (y2 * y2 * y);
+}
+
 // ---- a4: cuts (DESIGN.md R-G5) -----------------------------------------------------------------------------
 // every final gluon: pT > ptj_min and DeltaR(g, X) = sqrt(dy^2 + dphi^2) > dr_min to every other final parton;
 // true rapidity; strict inequalities; a cut value <= 0 is off.  gluon_mask bit i <-> final particle i is a gluon.

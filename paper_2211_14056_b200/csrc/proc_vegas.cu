@@ -24,7 +24,7 @@ template <int W> int launch(me_handle* h, const VegasArgs& a, double* f, unsigne
   if (per_sm < 1) return fail(ME_ECUDA, "vegas_integrand kernel does not fit on an SM%s%s");
   const long long need = (a.n_ev + 32 * W - 1) / (32 * W), full = static_cast<long long>(h->sms) * per_sm;
   const int grid = static_cast<int>(need < full ? need : full);
-  const long long stage_len = static_cast<long long>(grid) * 32 * W * (4 * (P::N_EXT - 2) + 2);
+  const long long stage_len = static_cast<long long>(grid) * 32 * W * (4 * (P::N_EXT - 2) + 4);
   if (stage_len > h->vegas_stage_len) {
     CU(cudaStreamSynchronize(s));  // an earlier launch may still read the old staging area
     if (h->vegas_stage) cudaFree(h->vegas_stage);

@@ -18,14 +18,13 @@ __global__ void __launch_bounds__(32 * W) vegas_integrand_kernel(VegasArgs a, do
                                                                  double* __restrict__ stage_all) {
   constexpr int NF = P::N_EXT - 2;
   constexpr int STRIDE = EventSmem<P>::DOUBLES;
-  constexpr int SLOT = 4 * NF + 2;
+  constexpr int SLOT = 4 * NF + 4;  // final momenta, weight, event index, beam energy, pad
   extern __shared__ __align__(16) double smem[];
   __shared__ int warp_count[W];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   double* mom_s = smem + warp * STRIDE;
   double* stage = stage_all + static_cast<long long>(blockIdx.x) * (32 * W) * SLOT;
   const long long n_batches = (a.n_ev + 32 * W - 1) / (32 * W);
-  const double e_beam = 0.5 * a.sqrt_s;
   for (long long b = blockIdx.x; b < n_batches; b += gridDim.x) {
     const long long ev = (b * W + warp) * 32 + lane;
     const bool live = ev < a.n_ev;
@@ -33,7 +32,7 @@ __global__ void __launch_bounds__(32 * W) vegas_integrand_kernel(VegasArgs a, do
       double p[NF][4], y[VEGAS_MAX_DIM], x[VEGAS_MAX_DIM];
       unsigned long long packed[2] = {0ull, 0ull};
       bool pass = false;
-      double w = 0.0;
+      double w = 0.0, rs = a.sqrt_s;
       if (live) {
         philox_fill<VEGAS_MAX_DIM>(a.seed, a.iteration, static_cast<uint64_t>(a.first_event + ev), a.n_dim, y);
         double jac = 1.0;
@@ -47,9 +46,22 @@ __global__ void __launch_bounds__(32 * W) vegas_integrand_kernel(VegasArgs a, do
             x[d] = 0.5;
           }
         }
-        const double wps = rambo_event<NF>(x, a.sqrt_s, a.masses, a.ps_mode, a.w0, p);
-        pass = passes_cuts<NF>(p, a.gluon_mask, a.ptj_min, a.dr_min);
-        w = jac * wps * a.prefactor;
+        if (a.ps_mode == 2) {
+          // hadronic mode (DESIGN.md R-N3): x[0], x[1] are the momentum fractions, the rest drives RAMBO on diet at sqrt(s_hat)
+          double msum = 0.0;
+#pragma unroll
+          for (int i = 0; i < NF; ++i) msum += a.masses[i];
+          rs = sqrt(x[0] * x[1]) * a.sqrt_s;
+          if (rs > msum) {
+            const double wps = rambo_event<NF>(x + 2, rs, a.masses, 1, rambo_volume(NF, rs * rs), p);
+            pass = passes_cuts<NF>(p, a.gluon_mask, a.ptj_min, a.dr_min);
+            w = jac * toy_gluon_density(x[0]) * toy_gluon_density(x[1]) * wps * (PB_GEV2 / (2.0 * rs * rs));
+          }
+        } else {
+          const double wps = rambo_event<NF>(x, a.sqrt_s, a.masses, a.ps_mode, a.w0, p);
+          pass = passes_cuts<NF>(p, a.gluon_mask, a.ptj_min, a.dr_min);
+          w = jac * wps * a.prefactor;
+        }
         for (int k = 0; k < idx_words; ++k) idx_out[ev * idx_words + k] = packed[k];
         if (!pass) f_out[ev] = 0.0;
       }
@@ -67,6 +79,7 @@ __global__ void __launch_bounds__(32 * W) vegas_integrand_kernel(VegasArgs a, do
           for (int mu = 0; mu < 4; ++mu) s[4 * i + mu] = p[i][mu];
         s[4 * NF] = w;
         s[4 * NF + 1] = __longlong_as_double(ev);
+        s[4 * NF + 2] = 0.5 * rs;
       }
     }
     int n_pass = 0;
@@ -76,6 +89,7 @@ __global__ void __launch_bounds__(32 * W) vegas_integrand_kernel(VegasArgs a, do
     for (int first = 0; first < n_pass; first += W) {
       const bool valid = first + warp < n_pass;
       const double* s = stage + (valid ? first + warp : 0) * SLOT;  // idle warps re-evaluate slot 0 (finite input, not stored)
+      const double e_beam = s[4 * NF + 2];
       if (lane < 8) mom_s[lane] = (lane == 0 || lane == 3 || lane == 4) ? e_beam : (lane == 7 ? -e_beam : 0.0);
       else if (lane < 8 + 4 * NF) mom_s[lane] = s[lane - 8];
       cta_sync<W>();

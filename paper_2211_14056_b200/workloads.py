@@ -22,6 +22,9 @@ WORKLOADS = [
     Workload("config3", "gg_ttxgg", 1000.0, (M_TOP, M_TOP, 0.0, 0.0), (0, 0, 1, 1), 3, 1 << 24, 0, 16, True),
     # configs[4]: Vegas over config 3, D = 3n-4 = 8 (reading R-G3), 50 bins, 5 x 2^24 events, seed 4
     Workload("config4", "gg_ttxgg", 1000.0, (M_TOP, M_TOP, 0.0, 0.0), (0, 0, 1, 1), 4, 1 << 24, 1, 8, True),
+    # the literal "10-dimensional" reading of configs[4] — hadronic, momentum fractions x1, x2 in front of
+    # the 8 RAMBO-on-diet dimensions, a DECLARED toy gluon density (no PDF grids in the container), sqrt(S) = 13 TeV
+    Workload("config4_hadronic", "gg_ttxgg", 13000.0, (M_TOP, M_TOP, 0.0, 0.0), (0, 0, 1, 1), 4, 1 << 24, 2, 10, True),
 ]
 BY_NAME = {w.name: w for w in WORKLOADS}
 VEGAS_BINS = 50

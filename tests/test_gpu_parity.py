@@ -302,6 +302,33 @@ def test_vegas_integrand_matches_oracle(handles, proc, mode, n):
     assert np.max(np.abs(sg - so) / (np.abs(so) + 1e-300 + 1e-12 * np.abs(so).max())) < 1e-9
 
 
+@pytest.mark.parametrize("proc,n", [("gg_ttxgg", 1500 + 5), ("gg_ttxg", 2000 + 3)])
+def test_vegas_hadronic_mode_matches_oracle(handles, proc, n):
+    """ps_mode 2 (the literal 10-dimensional configs[4]: momentum fractions + RAMBO on diet, declared toy gluon density;
+    SURVEY §8(f) N3, DESIGN.md R-N3): per-event f, sums and two iterations with feedback against the oracle."""
+    nf = {"gg_ttxg": 3, "gg_ttxgg": 4}[proc]
+    D, S = 3 * nf - 2, 13000.0
+    e = _warped_grid(D, VEGAS_BINS, 7)
+    go = ref.GridRef(D, VEGAS_BINS, VEGAS_ALPHA, seed=5, ps_mode=2)
+    go.edges[:] = e
+    gg = api.VegasGrid(D, VEGAS_BINS, VEGAS_ALPHA, 5, 2, edges=dev(e))
+    me = ref.MatrixElementRef(proc)
+    so, fo = me.vegas_integrand(go, S, 77, n, want_f=True)
+    sg, fg = api.vegas_integrand(handles[proc], gg, S, 77, n, want_f=True)
+    sg, fg = sg.cpu().numpy(), fg.cpu().numpy()
+    assert np.array_equal(fg != 0, fo != 0) and (fo == 0).any()
+    nz = fo != 0
+    assert np.max(np.abs(fg[nz] / fo[nz] - 1)) < ME_RTOL
+    assert sg[2] == so[2] and abs(sg[0] / so[0] - 1) < 1e-10
+    for it in range(2):
+        ro = me.vegas_iterate(go, S, n)
+        rg = api.vegas_iterate(handles[proc], gg, S, n)
+        assert rg["n_pass"] == ro["n_pass"] and abs(rg["integral"] / ro["integral"] - 1) < 1e-9
+        assert np.max(np.abs(gg.edges.cpu().numpy() - go.edges)) < 1e-9
+    with pytest.raises(api.MadmeError):
+        api.vegas_integrand(handles[proc], api.VegasGrid(D + 1, VEGAS_BINS, VEGAS_ALPHA, 5, 2), S, 0, 10)
+
+
 def test_vegas_iterate_matches_oracle(handles):
     """Three full iterations (integrand + refinement feedback) of config 4 at a size the oracle finishes in seconds."""
     n = 6000
