@@ -120,6 +120,22 @@ ME_HD cplx times_ik(cplx x, int k) {
   return mk((k & 2) ? -re : re, (k & 2) ? -im : im);
 }
 
+// acc += i^k x for a stored wavefunction: i^k = cr + i ci with cr, ci in {0, +-1} assembled from the bits of k (no
+// int->double conversion, no select cascade), then four FMAs per component
+ME_HD void combo_add(wf4& acc, const double* p, int k) {
+  const wf4 x = ld_wf(p);
+#if defined(__CUDA_ARCH__)
+  const int one = 0x3FF00000 | ((k & 2) << 30);  // high word of +1.0 (k = 0, 1) or -1.0 (k = 2, 3)
+  const double cr = __hiloint2double((k & 1) ? 0 : one, 0), ci = __hiloint2double((k & 1) ? one : 0, 0);
+#else
+  const double sgn = (k & 2) ? -1.0 : 1.0, cr = (k & 1) ? 0.0 : sgn, ci = (k & 1) ? sgn : 0.0;
+#endif
+  for (int c = 0; c < 4; ++c) {
+    acc.c[c].re = fma(cr, x.c[c].re, fma(-ci, x.c[c].im, acc.c[c].re));
+    acc.c[c].im = fma(cr, x.c[c].im, fma(ci, x.c[c].re, acc.c[c].im));
+  }
+}
+
 // a6: one task
 ME_HD void me_run_row(const MeRow r, double* sm, double mass) {
   const int op = (r.z >> 24) & 7;
@@ -127,20 +143,12 @@ ME_HD void me_run_row(const MeRow r, double* sm, double mass) {
   const int out = r.x & 0xffff;
   const wf4 A = ld_wf(sm + (r.x >> 16));
   if (op == OP_COMBO) {
-    // colour-ordered combination of currents over the same legs (same variant, same stride)
+    // colour-ordered combination of currents over the same legs (same variant); members 2 and 3 are optional
     const int n = (r.w >> 16) & 15;
     wf4 acc = A;  // the first member always enters with coefficient 1
-    const int off[3] = {static_cast<int>(r.y & 0xffff), static_cast<int>(r.y >> 16), static_cast<int>(r.z & 0xffff)};
-    for (int j = 1; j < n; ++j) {
-      const wf4 x = ld_wf(sm + off[j - 1]);
-      // i^k = cr + i ci with cr, ci in {0, +-1}: four FMAs per component instead of a cascade of selects
-      const int k = (r.w >> (20 + 2 * j)) & 3;
-      const double cr = (k & 1) ? 0.0 : 1.0 - k, ci = (k & 1) ? 2.0 - k : 0.0;
-      for (int c = 0; c < 4; ++c) {
-        acc.c[c].re = fma(cr, x.c[c].re, fma(-ci, x.c[c].im, acc.c[c].re));
-        acc.c[c].im = fma(cr, x.c[c].im, fma(ci, x.c[c].re, acc.c[c].im));
-      }
-    }
+    combo_add(acc, sm + (r.y & 0xffff), (r.w >> 22) & 3);
+    if (n > 2) combo_add(acc, sm + (r.y >> 16), (r.w >> 24) & 3);
+    if (n > 3) combo_add(acc, sm + (r.z & 0xffff), (r.w >> 26) & 3);
     st_wf(sm + out, acc);
     return;
   }
