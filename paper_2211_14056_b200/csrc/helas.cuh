@@ -2,7 +2,7 @@
 //
 // These are the "spinors", "vertices" and "propagators" of PAPER.md:70 (§2), i.e. the HELAS-style
 // routine families BASELINE.json:north_star names (ixxxxx/oxxxxx/vxxxxx, FFV1_{0,1,2}, FFV1P0_3,
-// VVV1_0, VVV1P0_1, VVVV{1,3,4}_0, VVVV{1,3,4}P0_1), restated from the Feynman rules of
+// VVV1P0_1, VVVV{1,3,4}P0_1; the closing amplitudes FFV1_0, VVV1_0, VVVV_0 are replaced by dot products), restated from the Feynman rules of
 // SURVEY.md §8(c) B/C in the CHIRAL representation with helicity spinors and circular
 // polarisations (the oracle uses the Dirac representation with a fixed-axis spin basis, so the
 // two sides share neither code nor intermediate values; only the helicity/colour-summed |M|^2 agrees).
@@ -284,17 +284,9 @@ ME_HD void vvvv_vec(const wf4& X, const wf4& Y, const wf4& Z, double invK2, wf4&
 }
 
 // ---------------------------------------------------------------------------------------------
-// Closing amplitudes (step a7)
+// Closing amplitudes (step a7): every diagram closes as the contraction of an open current with a propagated one
+// (gen/diagrams.py); the vertex-closing forms FFV1_0 / VVV1_0 / VVVV_0 were measured and dropped (profiles/)
 // ---------------------------------------------------------------------------------------------
-// [FFV1_0-like]  psibar Vslash psi
-ME_HD cplx ffv_amp(const wf4& q, const wf4& V, const wf4& p) {
-  const wf4 x = slash_col(V, p);
-  cplx r = q.c[0] * x.c[0];
-  r = cfma(q.c[1], x.c[1], r);
-  r = cfma(q.c[2], x.c[2], r);
-  r = cfma(q.c[3], x.c[3], r);
-  return r;
-}
 // Propagator-cut closing: J += i^K (U . C), U the open (un-propagated) current over one half of the legs, C the
 // propagated current over the other half.  MINK: vector line, Minkowski contraction (+,-,-,-); otherwise a fermion
 // line, plain sum over the four spinor components.  Every component is 4 FMAs straight into the flow accumulator.
@@ -314,32 +306,6 @@ template <int K, bool MINK> ME_HD void dot_acc(double& jr, double& ji, const wf4
   cacc<MINK ? ((K + 2) & 3) : K>(jr, ji, u.c[1], c.c[1]);
   cacc<MINK ? ((K + 2) & 3) : K>(jr, ji, u.c[2], c.c[2]);
   cacc<MINK ? ((K + 2) & 3) : K>(jr, ji, u.c[3], c.c[3]);
-}
-
-// [VVV1_0-like]  (X.Y)((K_X-K_Y).Z) + (Y.Z)((K_Y-K_Z).X) + (Z.X)((K_Z-K_X).Y)
-ME_HD cplx vvv_amp(const wf4& X, const vec4& KX, const wf4& Y, const vec4& KY, const wf4& Z, const vec4& KZ) {
-  vec4 dxy, dyz, dzx;
-  for (int i = 0; i < 4; ++i) {
-    dxy.v[i] = KX.v[i] - KY.v[i];
-    dyz.v[i] = KY.v[i] - KZ.v[i];
-    dzx.v[i] = KZ.v[i] - KX.v[i];
-  }
-  cplx r = mdot(X, Y) * mdot(dxy, Z);
-  r = cfma(mdot(Y, Z), mdot(dyz, X), r);
-  r = cfma(mdot(Z, X), mdot(dzx, Y), r);
-  return r;
-}
-// [VVVV{1,3,4}_0-like]
-//   a1 (f^{xye}f^{zwe}): (X.Z)(Y.W) - (X.W)(Y.Z)
-//   a2 (f^{xze}f^{ywe}): (X.Y)(Z.W) - (X.W)(Y.Z)
-//   a3 (f^{xwe}f^{yze}): (X.Y)(Z.W) - (X.Z)(Y.W)
-ME_HD void vvvv_amp(const wf4& X, const wf4& Y, const wf4& Z, const wf4& W, cplx& a1, cplx& a2, cplx& a3) {
-  const cplx xzyw = mdot(X, Z) * mdot(Y, W);
-  const cplx xwyz = mdot(X, W) * mdot(Y, Z);
-  const cplx xyzw = mdot(X, Y) * mdot(Z, W);
-  a1 = xzyw - xwyz;
-  a2 = xyzw - xwyz;
-  a3 = xyzw - xzyw;
 }
 
 }  // namespace madme

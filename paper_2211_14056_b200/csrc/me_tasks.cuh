@@ -38,11 +38,6 @@ namespace madme {
 // one op (padded with OP_NOP to multiples of 4 rows), groups in stages; a barrier separates stages.
 struct MeRow { unsigned x, y, z, w; };
 enum MeOp { OP_FFV_ROW = 0, OP_FFV_COL = 1, OP_FFV_VEC = 2, OP_VVV = 3, OP_VVVV = 4, OP_COMBO = 5, OP_NOP = 7 };
-#if defined(__CUDA_ARCH__)
-#define ME_FENCE() asm volatile("" ::: "memory")  // keeps ptxas from hoisting every shared-memory load to the top
-#else
-#define ME_FENCE()
-#endif
 
 constexpr int ME_WF_STRIDE = 16;  // doubles between the components of a stored wavefunction (one 128-byte line)
 ME_HD wf4 ld_wf(const double* p) {
