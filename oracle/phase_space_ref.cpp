@@ -85,24 +85,41 @@ static double massive_rescale(int n, double sqrt_s, const double* m, double p[][
   return std::pow(sk / sqrt_s, 2 * n - 3) * prod * sqrt_s / sk2;
 }
 
-// classic RAMBO: r[4i+0..3] = (r1,r2,r3,r4) of final particle i
+// classic RAMBO: r[4i+0..3] = (r1,r2,r3,r4) of final particle i:
+//   q_i = q0_i (1, n_i), Q = sum q_i, M = sqrt(Q^2), then the boost to the rest frame of Q and the scaling x = sqrt_s / M.
+// The boost is evaluated in the cancellation-free form (same map, reading R-G1b; the textbook form
+// Q0^2 - |Q|^2 loses conservation to ~1e-9 sqrt_s when two q_i are nearly collinear):
+//   q_i.q_j = q0_i q0_j |n_i - n_j|^2 / 2  (>= 0, no cancellation),   Q.q_i = sum_{j != i} q_i.q_j,   M^2 = sum_i Q.q_i,
+//   p0_i = x (Q.q_i) / M,      p_i = x [ q_i - Q (q0_i + (Q.q_i)/M) / (M + Q0) ]        (3-vectors),
+// which is p0 = x (gamma q0 + b.q), p = x (q + b q0 + a (b.q) b) with b = -Q/M, gamma = Q0/M, a = 1/(1+gamma) rewritten.
 static double rambo_classic(const double* r, double sqrt_s, const double* m, int n, double p[][4]) {
   const double pi = 3.14159265358979323846;
-  double q[NMAX_FINAL][4], Q[4] = {0, 0, 0, 0};
+  double q0[NMAX_FINAL], nv[NMAX_FINAL][3], Q[4] = {0, 0, 0, 0};
   for (int i = 0; i < n; ++i) {
     const double c = 2 * r[4 * i] - 1, phi = 2 * pi * r[4 * i + 1];
-    const double q0 = -std::log(r[4 * i + 2] * r[4 * i + 3]);
+    q0[i] = -std::log(r[4 * i + 2] * r[4 * i + 3]);
     const double st = std::sqrt(1 - c * c);
-    q[i][0] = q0; q[i][1] = q0 * st * std::cos(phi); q[i][2] = q0 * st * std::sin(phi); q[i][3] = q0 * c;
-    for (int mu = 0; mu < 4; ++mu) Q[mu] += q[i][mu];
+    nv[i][0] = st * std::cos(phi); nv[i][1] = st * std::sin(phi); nv[i][2] = c;
+    Q[0] += q0[i];
+    for (int j = 0; j < 3; ++j) Q[j + 1] += q0[i] * nv[i][j];
   }
-  const double M = std::sqrt(Q[0] * Q[0] - Q[1] * Q[1] - Q[2] * Q[2] - Q[3] * Q[3]);
-  const double b[3] = {-Q[1] / M, -Q[2] / M, -Q[3] / M};
-  const double g = Q[0] / M, a = 1 / (1 + g), x = sqrt_s / M;
+  double Qq[NMAX_FINAL], M2 = 0;
   for (int i = 0; i < n; ++i) {
-    const double bq = b[0] * q[i][1] + b[1] * q[i][2] + b[2] * q[i][3];
-    p[i][0] = x * (g * q[i][0] + bq);
-    for (int j = 0; j < 3; ++j) p[i][j + 1] = x * (q[i][j + 1] + b[j] * q[i][0] + a * bq * b[j]);
+    Qq[i] = 0;
+    for (int j = 0; j < n; ++j) {
+      if (j == i) continue;
+      double d2 = 0;
+      for (int k = 0; k < 3; ++k) d2 += (nv[i][k] - nv[j][k]) * (nv[i][k] - nv[j][k]);
+      Qq[i] += q0[i] * q0[j] * 0.5 * d2;
+    }
+    M2 += Qq[i];
+  }
+  const double M = std::sqrt(M2), x = sqrt_s / M;
+  for (int i = 0; i < n; ++i) {
+    const double e = Qq[i] / M;                 // energy in the rest frame of Q, before the scaling
+    const double f = (q0[i] + e) / (M + Q[0]);
+    p[i][0] = x * e;
+    for (int j = 0; j < 3; ++j) p[i][j + 1] = x * (q0[i] * nv[i][j] - Q[j + 1] * f);
   }
   return rambo_w0(n, sqrt_s * sqrt_s) * massive_rescale(n, sqrt_s, m, p);
 }

@@ -118,33 +118,50 @@ __device__ __forceinline__ double rambo_massive(double sqrt_s, const double* __r
   return pw * prod * sqrt_s / sk2;
 }
 
-// classic RAMBO: 4 uniforms per particle (cos theta, phi, and two for the energy), then the conformal boost
+// classic RAMBO: 4 uniforms per particle (cos theta, phi, and two for the energy), then the conformal boost to the rest
+// frame of Q = sum q_i and the scaling by x = sqrt_s / M.  The boost is written without cancellations (DESIGN.md
+// R-G1b): with q_i = w_i (1, n_i) the invariants q_i.q_j = w_i w_j |n_i - n_j|^2 / 2 are sums of squares, so
+//   E_i = (Q.q_i) / M = sum_{j != i} q_i.q_j / M,   M^2 = sum_i Q.q_i,   p_i = x [ q_i - Q (w_i + E_i) / (M + Q0) ]
+// keep momentum conservation at the 1e-13 level even when two of the q_i are almost collinear (two-body case).
 template <int N>
 __device__ __forceinline__ void rambo_classic(const double* __restrict__ r, double sqrt_s, double (&p)[N][4]) {
-  double q[N][4], Q[4] = {0.0, 0.0, 0.0, 0.0};
+  double w[N], dir[N][3], Qv[3] = {0.0, 0.0, 0.0}, Q0 = 0.0;
 #pragma unroll
   for (int i = 0; i < N; ++i) {
     const double c = 2.0 * r[4 * i] - 1.0, phi = 2.0 * PS_PI * r[4 * i + 1];
-    const double q0 = -log(r[4 * i + 2] * r[4 * i + 3]);
+    w[i] = -log(r[4 * i + 2] * r[4 * i + 3]);
     const double st = sqrt(1.0 - c * c);
     double sn, cs;
     sincos(phi, &sn, &cs);
-    q[i][0] = q0;
-    q[i][1] = q0 * st * cs;
-    q[i][2] = q0 * st * sn;
-    q[i][3] = q0 * c;
+    dir[i][0] = st * cs;
+    dir[i][1] = st * sn;
+    dir[i][2] = c;
+    Q0 += w[i];
 #pragma unroll
-    for (int mu = 0; mu < 4; ++mu) Q[mu] += q[i][mu];
+    for (int k = 0; k < 3; ++k) Qv[k] += w[i] * dir[i][k];
   }
-  const double M = sqrt(Q[0] * Q[0] - Q[1] * Q[1] - Q[2] * Q[2] - Q[3] * Q[3]);
-  const double b[3] = {-Q[1] / M, -Q[2] / M, -Q[3] / M};
-  const double g = Q[0] / M, a = 1.0 / (1.0 + g), x = sqrt_s / M;
+  double inv[N], M2 = 0.0;   // inv[i] = Q.q_i
+#pragma unroll
+  for (int i = 0; i < N; ++i) inv[i] = 0.0;
+#pragma unroll
+  for (int i = 0; i < N; ++i)
+#pragma unroll
+    for (int j = i + 1; j < N; ++j) {
+      const double dx = dir[i][0] - dir[j][0], dy = dir[i][1] - dir[j][1], dz = dir[i][2] - dir[j][2];
+      const double qq = w[i] * w[j] * (0.5 * (dx * dx + dy * dy + dz * dz));
+      inv[i] += qq;
+      inv[j] += qq;
+    }
+#pragma unroll
+  for (int i = 0; i < N; ++i) M2 += inv[i];
+  const double M = sqrt(M2), x = sqrt_s / M, den = 1.0 / (M + Q0);
 #pragma unroll
   for (int i = 0; i < N; ++i) {
-    const double bq = b[0] * q[i][1] + b[1] * q[i][2] + b[2] * q[i][3];
-    p[i][0] = x * (g * q[i][0] + bq);
+    const double e = inv[i] / M;
+    const double f = (w[i] + e) * den;
+    p[i][0] = x * e;
 #pragma unroll
-    for (int j = 0; j < 3; ++j) p[i][j + 1] = x * (q[i][j + 1] + b[j] * q[i][0] + a * bq * b[j]);
+    for (int k = 0; k < 3; ++k) p[i][k + 1] = x * (w[i] * dir[i][k] - Qv[k] * f);
   }
 }
 

@@ -49,12 +49,9 @@ def closed_form_gg_ttx(mom, alpha_s, m):
     return gs2 ** 2 * (1 / (6 * t1 * t2) - 3.0 / 8) * (t1 ** 2 + t2 ** 2 + rho - rho ** 2 / (4 * t1 * t2))
 
 
-def me_tolerance(mom, rtol=1e-10):
-    """Per-event relative tolerance for |M|^2 comparisons: rtol (BASELINE.json:north_star) for physical input, widened
-    by the input's own momentum non-conservation delta = max|sum k| / sqrt(s).  |M|^2 is only defined on momentum-
-    conserving, on-shell input; classic RAMBO with n = 2 loses conservation to ~1e-9 on the few events whose two
-    generated massless vectors are nearly collinear (huge conformal boost), and there every evaluation (oracle,
-    closed form, kernels) is a different function of the unphysical input.  DESIGN.md §Tolerances."""
+def momentum_violation(mom):
+    """delta = max |sum k| / sqrt(s) of each event's own input.  |M|^2 is only defined on momentum-conserving on-shell
+    input; the cancellation-free RAMBO boost (DESIGN.md R-G1b) keeps delta below 1e-12 on every event, so the
+    1e-10 tolerance of BASELINE.json:north_star applies to every event without exception (tests assert both)."""
     tot = mom[:, :2].sum(1) - mom[:, 2:].sum(1)
-    delta = np.abs(tot).max(1) / (mom[:, 0, 0] + mom[:, 1, 0])
-    return rtol + 20.0 * delta
+    return np.abs(tot).max(1) / (mom[:, 0, 0] + mom[:, 1, 0])
