@@ -351,6 +351,20 @@ def test_vegas_iterate_matches_oracle(handles):
         assert gg.iteration == go.iteration == it + 1
 
 
+def test_vegas_two_phase_space_maps_agree(handles):
+    """The integral must not depend on how the unit cube is mapped onto phase space: D = 8 (RAMBO on diet) and D = 16
+    (classic RAMBO) agree within the Monte-Carlo error (the only pin of the value of sigma)."""
+    def run(D, mode):
+        g = api.VegasGrid(D, VEGAS_BINS, VEGAS_ALPHA, 4, mode)
+        res = [api.vegas_iterate(handles["gg_ttxgg"], g, 1000.0, 1 << 20) for _ in range(3)]
+        I = np.array([r["integral"] for r in res])
+        w = 1.0 / np.array([r["variance"] for r in res])
+        return (I * w).sum() / w.sum(), w.sum() ** -0.5
+    a, ea = run(8, 1)
+    b, eb = run(16, 0)
+    assert abs(a - b) < 5 * np.hypot(ea, eb) and ea / a < 0.01 and eb / b < 0.01
+
+
 def test_vegas_is_deterministic(handles):
     """Fixed-shape reduction: two runs give bit-identical sums."""
     res = []
