@@ -228,34 +228,28 @@ ME_HD wf4 prop_row(const vec4& K, double s, double m, double f, const wf4& q) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// Off-shell currents (step a6).  invden = 1/(K_S^2 - m^2) of the OUTPUT current.
+// Off-shell currents (step a6).  A current over the leg set S is  propagator(K_S) x sum_j i^{k_j} (bare vertex)_j
+// over the Feynman subdiagrams j that enter it (me_tasks.cuh::me_run_item): the routines below are the BARE vertices,
+// the propagators are prop_row / prop_col above ((-+Kslash_S + m)/(K_S^2 - m^2) on a fermion line) and 1/K_S^2 on a
+// vector line.
 // ---------------------------------------------------------------------------------------------
-// [FFV1_1-like]  row spinor (fermion line towards the outgoing fermion) absorbs a vector:
-//   psibar' = psibar Vslash (-Kslash_S + m) / (K_S^2 - m^2)       (arrow momentum = -K_S)
-ME_HD wf4 ffv_row(const wf4& psibar, const wf4& V, const vec4& KS, double m, double invden) {
-  return prop_row(KS, -1.0, m, invden, slash_row(psibar, V));
-}
-// [FFV1_2-like]  column spinor absorbs a vector:
-//   psi' = (Kslash_S + m) Vslash psi / (K_S^2 - m^2)              (arrow momentum = +K_S)
-ME_HD wf4 ffv_col(const wf4& psi, const wf4& V, const vec4& KS, double m, double invden) {
-  return prop_col(KS, 1.0, m, invden, slash_col(V, psi));
-}
-// [FFV1P0_3-like]  V^mu = psibar gamma^mu psi / K_S^2
+// [FFV1_1 / FFV1_2-like]  a spinor absorbs a vector: slash_row(psibar, V), slash_col(V, psi) above.
+// [FFV1P0_3-like]  V^mu = psibar gamma^mu psi
 //   J0 = q0p2+q1p3+q2p0+q3p1          J1 = (q0p3+q1p2) - (q2p1+q3p0)
 //   J2 = -i(q0p3-q1p2) + i(q2p1-q3p0) J3 = (q0p2-q1p3) - (q2p0-q3p1)
-ME_HD wf4 ffv_vec(const wf4& q, const wf4& p, double invK2) {
+ME_HD wf4 ffv_vec_bare(const wf4& q, const wf4& p) {
   const cplx p02 = q.c[0] * p.c[2], p13 = q.c[1] * p.c[3], p20 = q.c[2] * p.c[0], p31 = q.c[3] * p.c[1];
   const cplx p03 = q.c[0] * p.c[3], p12 = q.c[1] * p.c[2], p21 = q.c[2] * p.c[1], p30 = q.c[3] * p.c[0];
   wf4 r;
-  r.c[0] = invK2 * ((p02 + p13) + (p20 + p31));
-  r.c[1] = invK2 * ((p03 + p12) - (p21 + p30));
-  r.c[2] = invK2 * times_i((p21 - p30) - (p03 - p12));
-  r.c[3] = invK2 * ((p02 - p13) - (p20 - p31));
+  r.c[0] = (p02 + p13) + (p20 + p31);
+  r.c[1] = (p03 + p12) - (p21 + p30);
+  r.c[2] = times_i((p21 - p30) - (p03 - p12));
+  r.c[3] = (p02 - p13) - (p20 - p31);
   return r;
 }
 // [VVV1P0_1-like]  three-gluon vertex with legs (X,K_X), (Y,K_Y), output leg incoming momentum -K_S:
-//   V^rho = [ (X.Y)(K_X-K_Y)^rho + Y^rho ((K_Y+K_S).X) - X^rho ((K_S+K_X).Y) ] / K_S^2
-ME_HD wf4 vvv_vec(const wf4& X, const vec4& KX, const wf4& Y, const vec4& KY, double invK2) {
+//   V^rho = (X.Y)(K_X-K_Y)^rho + Y^rho ((K_Y+K_S).X) - X^rho ((K_S+K_X).Y)
+ME_HD wf4 vvv_vec_bare(const wf4& X, const vec4& KX, const wf4& Y, const vec4& KY) {
   vec4 a, b, d;
   for (int i = 0; i < 4; ++i) {
     a.v[i] = fma(2.0, KY.v[i], KX.v[i]);  // K_Y + K_S
@@ -264,15 +258,15 @@ ME_HD wf4 vvv_vec(const wf4& X, const vec4& KX, const wf4& Y, const vec4& KY, do
   }
   const cplx xy = mdot(X, Y), ax = mdot(a, X), by = mdot(b, Y);
   wf4 r;
-  for (int i = 0; i < 4; ++i) r.c[i] = invK2 * cfms(by, X.c[i], cfma(ax, Y.c[i], d.v[i] * xy));
+  for (int i = 0; i < 4; ++i) r.c[i] = cfms(by, X.c[i], cfma(ax, Y.c[i], d.v[i] * xy));
   return r;
 }
 // [VVVV{1,3,4}P0_1-like]  four-gluon vertex, the three colour (x) Lorentz terms of SURVEY §8(c) C:
 //   t1 (f^{xye}f^{zde}): (X.Z) Y - (Y.Z) X
 //   t2 (f^{xze}f^{yde}): (X.Y) Z - (Y.Z) X
-//   t3 (f^{xde}f^{yze}): (X.Y) Z - (X.Z) Y           each / K_S^2
-ME_HD void vvvv_vec(const wf4& X, const wf4& Y, const wf4& Z, double invK2, wf4& t1, wf4& t2, wf4& t3) {
-  const cplx xy = invK2 * mdot(X, Y), xz = invK2 * mdot(X, Z), yz = invK2 * mdot(Y, Z);
+//   t3 (f^{xde}f^{yze}): (X.Y) Z - (X.Z) Y
+ME_HD void vvvv_vec_bare(const wf4& X, const wf4& Y, const wf4& Z, wf4& t1, wf4& t2, wf4& t3) {
+  const cplx xy = mdot(X, Y), xz = mdot(X, Z), yz = mdot(Y, Z);
   for (int i = 0; i < 4; ++i) {
     const cplx yzx = yz * X.c[i];
     const cplx xzy = xz * Y.c[i];

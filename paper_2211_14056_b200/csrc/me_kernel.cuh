@@ -1,4 +1,4 @@
-// me_kernel.cuh — the me_eval kernel: a CTA of W warps evaluates W events at a time.
+// me_kernel.cuh — the me_eval kernel: a CTA of W = 8 warps evaluates 8 events at a time.
 //
 // the tensorised generator materialises every wavefunction as an HBM tensor over events and
 // its footprint grows with the number of diagrams; the paper's CUDA op keeps them in per-thread storage
@@ -6,37 +6,43 @@
 // region, generated/*.inc), every off-shell current is computed once per combination of the helicities of ITS OWN
 // legs ("helicity recycling", me_tasks.cuh) and HBM sees 32 n_ext bytes in and 8 bytes out per event.
 //
-// Two mappings alternate inside the CTA (the barrier between them is __syncthreads, or __syncwarp when W = 1):
-//   current stages (a5, a6): the 32 W threads share the (task row, event) pairs of the stage, W events of the same
-//       row side by side on neighbouring lanes — every warp iteration runs ONE vertex routine on full lanes;
+// Two mappings alternate inside the CTA (a __syncthreads between them):
+//   current stages (a5, a6): warp w runs items w, w + W, ... of the stage; the 32 lanes of an item are 4 helicity
+//       variants x 8 events, so the item (its vertices, operands, coefficients) is warp-uniform: no divergence, no
+//       per-lane task decoding;
 //   dot stages (a7-a10): warp w owns event w, lane = helicity combination, J (the colour-flow vector) in registers.
+// Between the dot stages of successive rounds J is PARKED IN TENSOR MEMORY (tcgen05.st / tcgen05.ld, 4 N_FLOW 32-bit
+// columns per warp), so that the current stages have the whole register file for their accumulators.
+//
+// Compiled once per process: the including translation unit defines MADME_PROC (build.py).
 #pragma once
-#include "generated/epem_mupmum.inc"
-#include "generated/gg_ttx.inc"
-#include "generated/gg_ttxg.inc"
-#include "generated/gg_ttxgg.inc"
+#ifndef MADME_PROC
+#error "compile with -DMADME_PROC=<process>"
+#endif
+#define MADME_STR_(x) #x
+#define MADME_STR(x) MADME_STR_(x)
+#define MADME_INC(p) MADME_STR(generated/p.inc)
+#include MADME_INC(MADME_PROC)
+#include "tmem.cuh"
 
 namespace madme {
 
-// per-process tables in global memory (read through L1; a few KB, shared by every warp)
-template <class P> struct Tables;
-#define MADME_DEF_TABLES(P, U)                                                  \
-  __device__ const MeRow U##_tasks_d[] = U##_TASK_TABLE;                        \
-  __device__ const int U##_masks_d[] = U##_SUB_MASKS;                           \
-  __device__ const int U##_kind_d[] = U##_LEG_KIND;                             \
-  __device__ const int U##_massive_d[] = U##_LEG_MASSIVE;                       \
-  __device__ const int U##_extoff_d[] = U##_EXT_OFF;                            \
-  template <> struct Tables<P> {                                                \
-    static __device__ __forceinline__ const MeRow* tasks() { return U##_tasks_d; }   \
-    static __device__ __forceinline__ const int* masks() { return U##_masks_d; }     \
-    static __device__ __forceinline__ const int* kind() { return U##_kind_d; }       \
-    static __device__ __forceinline__ const int* massive() { return U##_massive_d; } \
-    static __device__ __forceinline__ const int* ext_off() { return U##_extoff_d; }  \
-  };
-MADME_DEF_TABLES(epem_mupmum, EPEM_MUPMUM)
-MADME_DEF_TABLES(gg_ttx, GG_TTX)
-MADME_DEF_TABLES(gg_ttxg, GG_TTXG)
-MADME_DEF_TABLES(gg_ttxgg, GG_TTXGG)
+#define MADME_UP_epem_mupmum EPEM_MUPMUM
+#define MADME_UP_gg_ttx GG_TTX
+#define MADME_UP_gg_ttxg GG_TTXG
+#define MADME_UP_gg_ttxgg GG_TTXGG
+#define MADME_CAT2_(a, b) a##b
+#define MADME_CAT2(a, b) MADME_CAT2_(a, b)
+#define MADME_TAB(suffix) MADME_CAT2(MADME_CAT2(MADME_UP_, MADME_PROC), suffix)
+
+// the process's tables: items and members in constant memory (every lane of a warp reads the same entry), the rest
+// in global memory (read once per event by phase 0)
+__constant__ MeItem c_items[] = MADME_TAB(_ITEM_TABLE);
+__constant__ MeMember c_members[] = MADME_TAB(_MEMBER_TABLE);
+__device__ const int d_masks[] = MADME_TAB(_SUB_MASKS);
+__device__ const int d_kind[] = MADME_TAB(_LEG_KIND);
+__device__ const int d_massive[] = MADME_TAB(_LEG_MASSIVE);
+__device__ const int d_extoff[] = MADME_TAB(_EXT_OFF);
 
 // doubles of shared memory per event: momenta [n_ext][4] + the generated scratch layout; the stride between the
 // events of a CTA is = 2 doubles (16 B) mod 16 doubles (128 B), so that the same object of neighbouring events
@@ -46,81 +52,79 @@ template <class P> struct EventSmem {
   static constexpr int DOUBLES = ((RAW + 13) / 16) * 16 + 2;
 };
 
-template <int W> __device__ __forceinline__ void cta_sync() {
-  if (W == 1) __syncwarp();
-  else __syncthreads();
-}
+constexpr int ME_W = 8;  // events = warps per CTA (gen/emit.py::W_EVENTS: the item tables are laid out for it)
 
-// rows [begin, end) for all W events of the CTA: item = (row, event), event fastest.  The row of the NEXT iteration is
-// fetched before the current one is executed (the table is constant: its latency stays off the dependent chain); the
-// loop is unrolled by two with the rows in alternating registers, so that no register copy waits on the fetch.
-__device__ __forceinline__ void run_row(const uint4 q, double* sm, double mass) {
-  MeRow r;
-  r.x = q.x; r.y = q.y; r.z = q.z; r.w = q.w;
-  me_run_row(r, sm, mass);
-}
-// `first` holds this thread's first row of the stage on entry (fetched during the previous stage) and of the NEXT
-// stage on return (stages are multiples of 32 rows, so that row is end + t / W): its latency hides behind the barrier
-// and the dot products in between.
-template <int W>
-__device__ __forceinline__ void run_rows(const uint4* __restrict__ tab, int begin, int end, int n_rows, double* smem, int ev_stride,
-                                         double mass, uint4& first) {
-  const int t = threadIdx.x;
-  const int ev = t % W;
-  double* sm = smem + ev * ev_stride;
-  int row = begin + t / W;
-  uint4 a = first;
-  first = __ldg(tab + min(end + t / W, n_rows));
-  if (row >= end) return;
-#pragma unroll 1
-  for (;;) {
-    const uint4 b = __ldg(tab + min(row + 32, n_rows));
-    run_row(a, sm, mass);
-    row += 32;
-    if (row >= end) break;
-    a = __ldg(tab + min(row + 32, n_rows));
-    run_row(b, sm, mass);
-    row += 32;
-    if (row >= end) break;
+// J parked in tensor memory: warp w owns lanes 32 (w % 4) .. +31 and the column block w / 4
+template <class P> struct JPark {
+  static constexpr bool ON = P::N_ROUNDS > 1;
+  static constexpr int REGS = 4 * P::N_FLOW;                      // 32-bit columns per warp
+  static constexpr int COLS = tmem_cols((ME_W / 4) * REGS);       // allocation: a power of two >= 32
+  static __device__ __forceinline__ uint32_t addr(uint32_t base) {
+    const int warp = threadIdx.x >> 5;
+    return base + (static_cast<uint32_t>(32 * (warp & 3)) << 16) + (warp >> 2) * REGS;
   }
-}
+  static __device__ __forceinline__ void park(uint32_t base, const double* jr, const double* ji) {
+    uint32_t r[REGS];
+#pragma unroll
+    for (int f = 0; f < P::N_FLOW; ++f) {
+      r[4 * f] = __double2loint(jr[f]); r[4 * f + 1] = __double2hiint(jr[f]);
+      r[4 * f + 2] = __double2loint(ji[f]); r[4 * f + 3] = __double2hiint(ji[f]);
+    }
+    tmem_store<REGS>(addr(base), r);
+  }
+  static __device__ __forceinline__ void unpark(uint32_t base, double* jr, double* ji) {
+    uint32_t r[REGS];
+    tmem_load<REGS>(addr(base), r);
+#pragma unroll
+    for (int f = 0; f < P::N_FLOW; ++f) {
+      jr[f] = __hiloint2double(r[4 * f + 1], r[4 * f]);
+      ji[f] = __hiloint2double(r[4 * f + 3], r[4 * f + 2]);
+    }
+  }
+};
 
-// |M|^2 of the W events whose momenta sit at the head of each event slice ([n_ext][4]).  Returns, on every lane of
+// |M|^2 of the 8 events whose momenta sit at the head of each event slice ([n_ext][4]).  Returns, on every lane of
 // warp w, the helicity- and colour-summed, averaged value of event w.  hel_out (optional, global [N_HEL], per warp)
-// receives each helicity combination's share.
-template <class P, int W>
-__device__ __forceinline__ double cta_me2(double* smem, double mass, double scale, double* hel_out) {
+// receives each helicity combination's share.  tmem: base address of the CTA's tensor-memory allocation.
+template <class P>
+__device__ __forceinline__ double cta_me2(double* smem, double mass, double scale, double* hel_out, uint32_t tmem) {
   constexpr int STRIDE = EventSmem<P>::DOUBLES;
+  constexpr int W = ME_W;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const uint4* tab = reinterpret_cast<const uint4*>(Tables<P>::tasks());
-  // a5: subset momenta / denominators and external wavefunctions, items = (subset or leg, event)
+  // a5: subset momenta / denominators and external wavefunctions, work = (subset or leg, event)
   {
     const int t = threadIdx.x, ev = t % W;
     double* mom_s = smem + ev * STRIDE;
-    me_phase0(t / W, 32, mom_s + 4 * P::N_EXT, mom_s, P::N_EXT, P::N_SUB, Tables<P>::masks(), Tables<P>::kind(),
-              Tables<P>::massive(), Tables<P>::ext_off(), mass);
+    me_phase0(t / W, 32, mom_s + 4 * P::N_EXT, mom_s, P::N_EXT, P::N_SUB, d_masks, d_kind, d_massive, d_extoff, mass);
   }
-  cta_sync<W>();
+  __syncthreads();
   double* base = smem + 4 * P::N_EXT;  // event e's scratch = base + e * STRIDE
   static_assert(P::N_HEL_EVAL <= 32, "one helicity combination per lane");
   double jr[P::N_FLOW], ji[P::N_FLOW];
-#pragma unroll
-  for (int f = 0; f < P::N_FLOW; ++f) { jr[f] = 0.0; ji[f] = 0.0; }
   const double* my = base + warp * STRIDE;
-  int row = 0;
-  uint4 first = __ldg(tab + threadIdx.x / W);
-  // ONE copy of the row interpreter and one of each round's dot products in the instruction stream: the phase loop
-  // must stay rolled (unrolled it is > 600 KB of SASS and the kernel starves on instruction fetch)
+  double* sm_e = base + (lane % W) * STRIDE;   // items: lane = local variant j x event
+  const int j = lane / W;
+  int it = 0;
+  // ONE copy of the item interpreter and one of each round's dot products in the instruction stream
 #pragma unroll 1
-  for (int p = 0; p < P::N_PHASES; ++p) {
-    const int end = P::phase_end(p);
-    run_rows<W>(tab, row, end, P::N_ROWS, base, STRIDE, mass, first);
-    row = end;
-    cta_sync<W>();
-    const int r = P::phase_dots(p);
+  for (int p = 0; p < P::N_STAGES; ++p) {
+    const int end = P::stage_end(p);
+#pragma unroll 1
+    for (int i = it + warp; i < end; i += W) me_run_item(c_items[i], c_members, j, sm_e, mass);
+    it = end;
+    __syncthreads();
+    const int r = P::stage_dots(p);
     if (r >= 0) {
+      // J is defined here on every path (zero in the first round, un-parked afterwards): dead during the items
+      if (r == 0) {
+#pragma unroll
+        for (int f = 0; f < P::N_FLOW; ++f) { jr[f] = 0.0; ji[f] = 0.0; }
+      } else if (JPark<P>::ON) {
+        JPark<P>::unpark(tmem, jr, ji);
+      }
       if (lane < P::N_HEL_EVAL) P::dots(r, my, lane, jr, ji);
-      cta_sync<W>();
+      if (JPark<P>::ON && r + 1 < P::N_ROUNDS) JPark<P>::park(tmem, jr, ji);
+      if (r + 1 < P::N_ROUNDS) __syncthreads();   // the next round's items overwrite the round region
     }
   }
   double v = (lane < P::N_HEL_EVAL) ? P::colour(jr, ji) : 0.0;
@@ -134,27 +138,26 @@ __device__ __forceinline__ double cta_me2(double* smem, double mass, double scal
   return 2.0 * v * scale;
 }
 
-// W events per CTA (blockDim.x = 32 W); persistent grid, batches of W consecutive events.  MADME_OCC_WARPS is the number
-// of resident warps per SM the register allocation is bounded for (8 -> up to 255 registers, 12 -> 168).
-#ifndef MADME_OCC_WARPS
-#define MADME_OCC_WARPS 8
-#endif
-template <class P, int W>
-__global__ void __launch_bounds__(32 * W, (MADME_OCC_WARPS + W - 1) / W) me_eval_kernel(const double* __restrict__ momenta, double* __restrict__ me2,
-                                                         double* __restrict__ me2_hel, long long n_ev, double mass, double scale) {
+// 8 events per CTA (blockDim.x = 256); persistent grid, batches of 8 consecutive events.
+template <class P>
+__global__ void __launch_bounds__(32 * ME_W, 1) me_eval_kernel(const double* __restrict__ momenta, double* __restrict__ me2,
+                                                              double* __restrict__ me2_hel, long long n_ev, double mass, double scale) {
   extern __shared__ __align__(16) double smem[];
   constexpr int STRIDE = EventSmem<P>::DOUBLES;
+  constexpr int W = ME_W;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const uint32_t tmem = JPark<P>::ON ? tmem_alloc<JPark<P>::COLS>() : 0u;
   const long long n_batches = (n_ev + W - 1) / W;
   for (long long b = blockIdx.x; b < n_batches; b += gridDim.x) {
     // events past the end repeat the last one (computed, not stored)
     const long long ev = min(b * W + warp, n_ev - 1);
     if (lane < 4 * P::N_EXT) smem[warp * STRIDE + lane] = momenta[ev * (4 * P::N_EXT) + lane];
-    cta_sync<W>();
-    const double r = cta_me2<P, W>(smem, mass, scale, (me2_hel && b * W + warp < n_ev) ? me2_hel + ev * P::N_HEL : nullptr);
+    __syncthreads();
+    const double r = cta_me2<P>(smem, mass, scale, (me2_hel && b * W + warp < n_ev) ? me2_hel + ev * P::N_HEL : nullptr, tmem);
     if (lane == 0 && me2 && b * W + warp < n_ev) me2[ev] = r;
-    cta_sync<W>();
+    __syncthreads();
   }
+  if (JPark<P>::ON) tmem_free<JPark<P>::COLS>(tmem);
 }
 
 }  // namespace madme

@@ -1,9 +1,8 @@
 // me_tasks.cuh — per-event scratch layout and the table-driven cooperative steps of me_eval.
 //
-// One warp owns one event ("parallelized in the event axis"; the 32 lanes of the warp are
-// 32 helicity combinations of that event — SURVEY.md §7 "hard parts", option B).  The event's
-// wavefunctions live in a private slice of SHARED MEMORY and never touch HBM: that is the paper's
-// memory-footprint point taken to its limit.
+// A CTA works on W events at a time ("parallelized in the event axis").  An event's wavefunctions live in
+// a private slice of SHARED MEMORY and never touch HBM: that is the paper's memory-footprint point (PAPER.md:9,
+// 62-64) taken to its limit.
 //
 // Scratch layout of one event (doubles), produced by gen/emit.py for each process:
 //   subset blocks  : 8 doubles per used leg subset S:  K_S[4], 1/K_S^2, 1/(K_S^2 - m_t^2), pad, pad
@@ -16,28 +15,36 @@
 //   Leg 0 is fixed at helicity +1 (parity: |M(-h)|^2 = |M(h)|^2, the sum is doubled at the end), so
 //   variant index v = sum_k b_{l_k} 2^k over the legs l_0 < l_1 < ... of S OTHER THAN LEG 0, b = 0 for helicity -1,
 //   1 for +1, and nv = 2^(number of those legs).
-//   The first BASE_DOUBLES hold what every round reads (subset blocks, external wavefunctions, the currents that feed
-//   other currents); the rest is the ROUND region, reused by successive rounds of leg splits (gen/emit.py).
+//   Only what somebody reads is stored: the first BASE_DOUBLES hold what every round reads (subset blocks, external
+//   wavefunctions, the currents that feed other currents); the rest is the ROUND region, reused by successive rounds
+//   of leg splits, and holds the operands of the round's propagator-cut dot products (gen/emit.py).
 //
 // The steps:
 //   a5  me_phase0      : K_S and propagator denominators for every subset, external wavefunctions
-//   a6  me_run_row     : off-shell currents and their combinations, one (object, variant) task per thread, stage by stage
+//   a6  me_run_item    : one ITEM = up to 4 colour-ordered currents over one leg set, for one helicity variant per
+//                        lane: the bare vertices of the Feynman subdiagrams that enter them are evaluated in registers
+//                        and summed with their {+-1, +-i} coefficients, the common propagator is applied once per sum
 //   a7-a10             : generated straight-line code (csrc/generated/*.inc: dots, colour), one helicity per lane
 #pragma once
 #include "helas.cuh"
 
 namespace madme {
 
-// One task = one (object, helicity variant), encoded in 128 bits so that a lane fetches its task with one load:
-//   x: out | a << 16                      (offsets in doubles into the event's scratch)
-//   y: b   | c << 16
-//   z: ksub_out | ksub_a << 8 | ksub_b << 16 | op << 24 | massive << 27 | open << 28      (ksub = subset index)
-//   w: n_members << 16 | phase codes (2 bits each) << 20                                    (OP_COMBO)
-// OP_VVVV writes the three colour terms of a four-gluon current: out, (z >> 8) & 0xffff and w & 0xffff.
-// OP_COMBO: out = sum_j i^{k_j} member_j with members (a, b, c, and a fourth in z & 0xffff).  Rows come in groups of
-// one op (padded with OP_NOP to multiples of 4 rows), groups in stages; a barrier separates stages.
-struct MeRow { unsigned x, y, z, w; };
-enum MeOp { OP_FFV_ROW = 0, OP_FFV_COL = 1, OP_FFV_VEC = 2, OP_VVV = 3, OP_VVVV = 4, OP_COMBO = 5, OP_NOP = 7 };
+// One item (16 B), warp-uniform:
+//   w0: n_members | n_out << 8 | kind << 12 | massive << 15 | nv << 16 | vbase << 24
+//   w1: first_member | ksub_out << 16                      (ksub = subset index: block at sm + 8 ksub)
+//   w2: out0 | out1 << 16,  w3: out2 | out3 << 16          (offsets in doubles into the event's scratch, variant 0)
+// One member (32 B) = one bare vertex:
+//   w0: op | ksub_a << 8 | ksub_b << 16
+//   w1: a | b << 16,   w2: c | vmap_c << 16,   w3: vmap_a | vmap_b << 16
+//        (vmap: 4 bits per local variant j: which variant of the argument enters variant vbase + j of the outputs)
+//   w4: codes of term 0 | codes of term 1 << 12,   w5: codes of term 2
+//        (3 bits per accumulator: 4 + k adds i^k x; terms 1, 2 exist for the four-gluon vertex only)
+struct MeItem { unsigned w0, w1, w2, w3; };
+struct MeMember { unsigned w[8]; };
+enum MeOp { OP_SLASH_ROW = 0, OP_SLASH_COL = 1, OP_FFV_VEC = 2, OP_VVV = 3, OP_VVVV = 4 };
+enum MeKind { KIND_VEC = 0, KIND_ROW = 1, KIND_COL = 2, KIND_OPEN = 3 };
+constexpr int ME_NSLOT = 4;
 
 constexpr int ME_WF_STRIDE = 16;  // doubles between the components of a stored wavefunction (one 128-byte line)
 ME_HD wf4 ld_wf(const double* p) {
@@ -109,76 +116,92 @@ ME_HD void me_phase0(int idx, int step, double* sm, const double* mom, int n_ext
   }
 }
 
-// i^k x
-ME_HD cplx times_ik(cplx x, int k) {
-  const double re = (k & 1) ? -x.im : x.re, im = (k & 1) ? x.re : x.im;
-  return mk((k & 2) ? -re : re, (k & 2) ? -im : im);
-}
-
-// acc += i^k x for a stored wavefunction: i^k = cr + i ci with cr, ci in {0, +-1} assembled from the bits of k (no
-// int->double conversion, no select cascade), then four FMAs per component
-ME_HD void combo_add(wf4& acc, const double* p, int k) {
-  const wf4 x = ld_wf(p);
-#if defined(__CUDA_ARCH__)
-  const int one = 0x3FF00000 | ((k & 2) << 30);  // high word of +1.0 (k = 0, 1) or -1.0 (k = 2, 3)
-  const double cr = __hiloint2double((k & 1) ? 0 : one, 0), ci = __hiloint2double((k & 1) ? one : 0, 0);
-#else
-  const double sgn = (k & 2) ? -1.0 : 1.0, cr = (k & 1) ? 0.0 : sgn, ci = (k & 1) ? sgn : 0.0;
-#endif
-  for (int c = 0; c < 4; ++c) {
-    acc.c[c].re = fma(cr, x.c[c].re, fma(-ci, x.c[c].im, acc.c[c].re));
-    acc.c[c].im = fma(cr, x.c[c].im, fma(ci, x.c[c].re, acc.c[c].im));
-  }
-}
-
-// a6: one task
-ME_HD void me_run_row(const MeRow r, double* sm, double mass) {
-  const int op = (r.z >> 24) & 7;
-  if (op == OP_NOP) return;
-  const int out = r.x & 0xffff;
-  const wf4 A = ld_wf(sm + (r.x >> 16));
-  if (op == OP_COMBO) {
-    // colour-ordered combination of currents over the same legs (same variant); members 2 and 3 are optional
-    const int n = (r.w >> 16) & 15;
-    wf4 acc = A;  // the first member always enters with coefficient 1
-    combo_add(acc, sm + (r.y & 0xffff), (r.w >> 22) & 3);
-    if (n > 2) combo_add(acc, sm + (r.y >> 16), (r.w >> 24) & 3);
-    if (n > 3) combo_add(acc, sm + (r.z & 0xffff), (r.w >> 26) & 3);
-    st_wf(sm + out, acc);
-    return;
-  }
-  const wf4 B = ld_wf(sm + (r.y & 0xffff));
-  const double* ks = sm + 8 * (r.z & 0xff);
-  const bool massive = (r.z >> 27) & 1;
-  const bool open = (r.z >> 28) & 1;  // the current stops at its vertex: no propagator (U side of a propagator cut)
-  const double m = massive ? mass : 0.0;
-  const double invk2 = open ? 1.0 : ks[4];
-  // open and propagated rows sit in different groups (gen/emit.py), so these branches are warp-uniform
-  if (op == OP_FFV_ROW) {
-    const wf4 x = slash_row(A, B);
-    if (open) st_wf(sm + out, x);
-    else st_wf(sm + out, prop_row(ld_k(ks), -1.0, m, massive ? ks[5] : ks[4], x));
-  } else if (op == OP_FFV_COL) {
-    const wf4 x = slash_col(B, A);
-    if (open) st_wf(sm + out, x);
-    else st_wf(sm + out, prop_col(ld_k(ks), 1.0, m, massive ? ks[5] : ks[4], x));
-  } else if (op == OP_FFV_VEC) {
-    st_wf(sm + out, ffv_vec(A, B, invk2));
-  } else if (op == OP_VVV) {
-    st_wf(sm + out, vvv_vec(A, ld_k(sm + 8 * ((r.z >> 8) & 0xff)), B, ld_k(sm + 8 * ((r.z >> 16) & 0xff)), invk2));
+// acc += i^k x  (k warp-uniform: a four-way branch, eight additions)
+ME_HD void acc_add(wf4& acc, const wf4& x, int k) {
+  if (k == 0) {
+    for (int c = 0; c < 4; ++c) { acc.c[c].re += x.c[c].re; acc.c[c].im += x.c[c].im; }
+  } else if (k == 2) {
+    for (int c = 0; c < 4; ++c) { acc.c[c].re -= x.c[c].re; acc.c[c].im -= x.c[c].im; }
+  } else if (k == 1) {
+    for (int c = 0; c < 4; ++c) { acc.c[c].re -= x.c[c].im; acc.c[c].im += x.c[c].re; }
   } else {
-    const wf4 C = ld_wf(sm + (r.y >> 16));
-    wf4 t1, t2, t3;
-    vvvv_vec(A, B, C, invk2, t1, t2, t3);
-    st_wf(sm + out, t1);
-    st_wf(sm + ((r.z >> 8) & 0xffff), t2);
-    st_wf(sm + (r.w & 0xffff), t3);
+    for (int c = 0; c < 4; ++c) { acc.c[c].re += x.c[c].im; acc.c[c].im -= x.c[c].re; }
+  }
+}
+// the term x enters accumulator s with i^(code & 3) if bit 2 of its 3-bit code is set
+ME_HD void acc_term(wf4 (&acc)[ME_NSLOT], const wf4& x, unsigned codes) {
+#if defined(__CUDA_ARCH__)
+#pragma unroll
+#endif
+  for (int s = 0; s < ME_NSLOT; ++s) {
+    const unsigned c = (codes >> (3 * s)) & 7u;
+    if (c & 4u) acc_add(acc[s], x, static_cast<int>(c & 3u));
   }
 }
 
-// rows [begin, end) of one stage, 32 lanes at a time (host emulation and reference semantics of the device loop)
-ME_HD void me_run_rows(int lane, double* sm, const MeRow* tab, int begin, int end, double mass) {
-  for (int i = begin + lane; i < end; i += 32) me_run_row(tab[i], sm, mass);
+// a6: one item for local variant j (0 .. VPI-1) of one event (scratch at sm)
+ME_HD void me_run_item(const MeItem H, const MeMember* __restrict__ members, int j, double* __restrict__ sm, double mass) {
+  const int n_mem = H.w0 & 0xff;
+  const int nv = (H.w0 >> 16) & 0xff, v = static_cast<int>(H.w0 >> 24) + j;
+  if (n_mem == 0 || v >= nv) return;
+  const int n_out = (H.w0 >> 8) & 0xf, kind = (H.w0 >> 12) & 7;
+  const int sh = 4 * j;
+  wf4 acc[ME_NSLOT];
+  for (int s = 0; s < ME_NSLOT; ++s)
+    for (int c = 0; c < 4; ++c) acc[s].c[c] = mk(0.0, 0.0);
+  const MeMember* m = members + (H.w1 & 0xffff);
+#if defined(__CUDA_ARCH__)
+#pragma unroll 1
+#endif
+  for (int i = 0; i < n_mem; ++i, ++m) {
+    const unsigned w0 = m->w[0], w1 = m->w[1], w3 = m->w[3], w4 = m->w[4];
+    const int op = w0 & 0xff;
+    const wf4 A = ld_wf(sm + (w1 & 0xffff) + 2 * ((w3 >> sh) & 15u));
+    const wf4 B = ld_wf(sm + (w1 >> 16) + 2 * ((w3 >> (16 + sh)) & 15u));
+    if (op == OP_SLASH_ROW) {
+      acc_term(acc, slash_row(A, B), w4);
+    } else if (op == OP_SLASH_COL) {
+      acc_term(acc, slash_col(B, A), w4);
+    } else if (op == OP_FFV_VEC) {
+      acc_term(acc, ffv_vec_bare(A, B), w4);
+    } else if (op == OP_VVV) {
+      acc_term(acc, vvv_vec_bare(A, ld_k(sm + 8 * ((w0 >> 8) & 0xff)), B, ld_k(sm + 8 * ((w0 >> 16) & 0xff))), w4);
+    } else {
+      const unsigned w2 = m->w[2];
+      const wf4 C = ld_wf(sm + (w2 & 0xffff) + 2 * ((w2 >> (16 + sh)) & 15u));
+      wf4 t1, t2, t3;
+      vvvv_vec_bare(A, B, C, t1, t2, t3);
+      acc_term(acc, t1, w4);
+      acc_term(acc, t2, w4 >> 12);
+      acc_term(acc, t3, m->w[5]);
+    }
+  }
+  // the common propagator, once per colour-ordered current
+  const double* ks = sm + 8 * (H.w1 >> 16);
+  const unsigned outs[ME_NSLOT] = {H.w2 & 0xffff, H.w2 >> 16, H.w3 & 0xffff, H.w3 >> 16};
+  if (kind == KIND_OPEN) {
+    for (int s = 0; s < ME_NSLOT; ++s)
+      if (s < n_out) st_wf(sm + outs[s] + 2 * v, acc[s]);
+  } else if (kind == KIND_VEC) {
+    const double f = ks[4];
+    for (int s = 0; s < ME_NSLOT; ++s)
+      if (s < n_out) {
+        wf4 y;
+        for (int c = 0; c < 4; ++c) y.c[c] = f * acc[s].c[c];
+        st_wf(sm + outs[s] + 2 * v, y);
+      }
+  } else {
+    const bool massive = (H.w0 >> 15) & 1;
+    const double mm = massive ? mass : 0.0, f = massive ? ks[5] : ks[4];
+    const vec4 K = ld_k(ks);
+    if (kind == KIND_ROW) {
+      for (int s = 0; s < ME_NSLOT; ++s)
+        if (s < n_out) st_wf(sm + outs[s] + 2 * v, prop_row(K, -1.0, mm, f, acc[s]));
+    } else {
+      for (int s = 0; s < ME_NSLOT; ++s)
+        if (s < n_out) st_wf(sm + outs[s] + 2 * v, prop_col(K, 1.0, mm, f, acc[s]));
+    }
+  }
 }
 
 }  // namespace madme

@@ -1,6 +1,6 @@
 // proc_eval.cu — me_eval for ONE process: compiled once per process with -DMADME_PROC=<process> (build.py).
-// W (events = warps per CTA) is a run-time choice among the compiled instances; MADME_WARPS overrides it — the
-// threads-per-block scan of PAPER.md:78-84 (Fig. 3) is repeated with it.
+// A CTA is 8 warps = 8 events (me_kernel.cuh); the events-per-CTA scan of PAPER.md:78-84 (Fig. 3) was done on the
+// round-1 kernel (profiles/r1_block_size_scan.md).
 #include "common.cuh"
 #include "me_kernel.cuh"
 
@@ -15,17 +15,21 @@ namespace madme {
 namespace MADME_CAT(tu_, MADME_PROC, _e) {
 using P = MADME_PROC;
 
-template <int W> int geom(int* regs, int* ctas) {
+int geom(me_handle* h) {
   cudaFuncAttributes fa;
-  CU(cudaFuncGetAttributes(&fa, me_eval_kernel<P, W>));
-  const int bytes = W * EventSmem<P>::DOUBLES * 8;
-  if (cudaFuncSetAttribute(me_eval_kernel<P, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) != cudaSuccess) {
-    (void)cudaGetLastError();
-    *ctas = 0;
-    return ME_OK;
-  }
-  *regs = fa.numRegs;
-  CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas, me_eval_kernel<P, W>, 32 * W, bytes));
+  CU(cudaFuncGetAttributes(&fa, me_eval_kernel<P>));
+  const int bytes = ME_W * EventSmem<P>::DOUBLES * 8;
+  CU(cudaFuncSetAttribute(me_eval_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  int ctas = 0;
+  CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas, me_eval_kernel<P>, 32 * ME_W, bytes));
+  if (ctas < 1) return fail(ME_ECUDA, "me_eval kernel does not fit on an SM%s%s");
+  // tensor memory: 512 columns per SM shared by the resident CTAs
+  if (JPark<P>::ON && ctas * JPark<P>::COLS > 512) ctas = 512 / JPark<P>::COLS;
+  h->warps = ME_W;
+  h->regs = fa.numRegs;
+  h->ctas_per_sm = ctas;
+  h->smem_bytes = bytes;
+  h->grid = h->sms * ctas;
   return ME_OK;
 }
 
@@ -39,41 +43,13 @@ int fill(me_handle* h) {
   int dev = 0;
   CU(cudaGetDevice(&dev));
   CU(cudaDeviceGetAttribute(&h->sms, cudaDevAttrMultiProcessorCount, dev));
-  const int cand[4] = {1, 2, 4, 8};
-  int regs[4] = {0, 0, 0, 0}, ctas[4] = {0, 0, 0, 0}, rc;
-  if ((rc = geom<1>(&regs[0], &ctas[0])) || (rc = geom<2>(&regs[1], &ctas[1])) || (rc = geom<4>(&regs[2], &ctas[2])) ||
-      (rc = geom<8>(&regs[3], &ctas[3])))
-    return rc;
-  int pick = -1;
-  const char* env = getenv("MADME_WARPS");
-  if (env) {
-    for (int k = 0; k < 4; ++k)
-      if (atoi(env) == cand[k] && ctas[k] > 0) pick = k;
-    if (pick < 0) return fail(ME_EINVAL, "MADME_WARPS must be 1, 2, 4 or 8 (and fit on an SM)%s%s");
-  } else {
-    // most resident warps per SM; ties go to the larger CTA (fuller lanes in the current stages)
-    int best = 0;
-    for (int k = 0; k < 4; ++k)
-      if (cand[k] * ctas[k] >= best && ctas[k] > 0) { best = cand[k] * ctas[k]; pick = k; }
-    if (pick < 0) return fail(ME_ECUDA, "me_eval kernel does not fit on an SM%s%s");
-  }
-  h->warps = cand[pick];
-  h->regs = regs[pick];
-  h->ctas_per_sm = ctas[pick];
-  h->smem_bytes = h->warps * EventSmem<P>::DOUBLES * 8;
-  h->grid = h->sms * h->ctas_per_sm;
-  return ME_OK;
+  return geom(h);
 }
 
 int eval(me_handle* h, const double* mom, double* me2, double* hel, long long n, cudaStream_t s) {
-  const long long need = (n + h->warps - 1) / h->warps;
-  const int grid = static_cast<int>(need < h->grid ? need : h->grid), T = 32 * h->warps;
-  switch (h->warps) {
-    case 1: me_eval_kernel<P, 1><<<grid, T, h->smem_bytes, s>>>(mom, me2, hel, n, h->mass, h->scale); break;
-    case 2: me_eval_kernel<P, 2><<<grid, T, h->smem_bytes, s>>>(mom, me2, hel, n, h->mass, h->scale); break;
-    case 4: me_eval_kernel<P, 4><<<grid, T, h->smem_bytes, s>>>(mom, me2, hel, n, h->mass, h->scale); break;
-    default: me_eval_kernel<P, 8><<<grid, T, h->smem_bytes, s>>>(mom, me2, hel, n, h->mass, h->scale); break;
-  }
+  const long long need = (n + ME_W - 1) / ME_W;
+  const int grid = static_cast<int>(need < h->grid ? need : h->grid);
+  me_eval_kernel<P><<<grid, 32 * ME_W, h->smem_bytes, s>>>(mom, me2, hel, n, h->mass, h->scale);
   CU(cudaGetLastError());
   return ME_OK;
 }

@@ -13,15 +13,13 @@ namespace madme {
 namespace MADME_CAT(tu_, MADME_PROC, _v) {
 using P = MADME_PROC;
 
-template <int W> int launch(me_handle* h, const VegasArgs& a, double* f, unsigned long long* idx, int words, cudaStream_t s) {
-  static bool prepared = false;
-  if (!prepared) {
-    CU(cudaFuncSetAttribute(vegas_integrand_kernel<P, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_bytes));
-    prepared = true;
-  }
+int integrand(me_handle* h, const VegasArgs& a, double* f, unsigned long long* idx, int words, cudaStream_t s) {
+  constexpr int W = ME_W;
+  CU(cudaFuncSetAttribute(vegas_integrand_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_bytes));
   int per_sm = 0;
-  CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, vegas_integrand_kernel<P, W>, 32 * W, h->smem_bytes));
+  CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, vegas_integrand_kernel<P>, 32 * W, h->smem_bytes));
   if (per_sm < 1) return fail(ME_ECUDA, "vegas_integrand kernel does not fit on an SM%s%s");
+  if (JPark<P>::ON && per_sm * JPark<P>::COLS > 512) per_sm = 512 / JPark<P>::COLS;
   const long long need = (a.n_ev + 32 * W - 1) / (32 * W), full = static_cast<long long>(h->sms) * per_sm;
   const int grid = static_cast<int>(need < full ? need : full);
   const long long stage_len = static_cast<long long>(grid) * 32 * W * (4 * (P::N_EXT - 2) + 4);
@@ -32,18 +30,9 @@ template <int W> int launch(me_handle* h, const VegasArgs& a, double* f, unsigne
     CU(cudaMalloc(&h->vegas_stage, sizeof(double) * stage_len));
     h->vegas_stage_len = stage_len;
   }
-  vegas_integrand_kernel<P, W><<<grid, 32 * W, h->smem_bytes, s>>>(a, f, idx, words, h->vegas_stage);
+  vegas_integrand_kernel<P><<<grid, 32 * W, h->smem_bytes, s>>>(a, f, idx, words, h->vegas_stage);
   CU(cudaGetLastError());
   return ME_OK;
-}
-
-int integrand(me_handle* h, const VegasArgs& a, double* f, unsigned long long* idx, int words, cudaStream_t s) {
-  switch (h->warps) {
-    case 1: return launch<1>(h, a, f, idx, words, s);
-    case 2: return launch<2>(h, a, f, idx, words, s);
-    case 4: return launch<4>(h, a, f, idx, words, s);
-    default: return launch<8>(h, a, f, idx, words, s);
-  }
 }
 
 const ProcOps ops = {nullptr, nullptr, integrand};

@@ -12,11 +12,11 @@ namespace madme {
 // L2) so that the CTA then evaluates |M|^2 of exactly the surviving events, W at a time, whatever warp generated them;
 // cut events cost no matrix element.  Output per event: f (8 B) and the D bin indices packed one byte each
 // (n_bins <= 255) into idx_out[ev][ceil(D/8)].
-template <class P, int W>
-__global__ void __launch_bounds__(32 * W) vegas_integrand_kernel(VegasArgs a, double* __restrict__ f_out,
+template <class P>
+__global__ void __launch_bounds__(32 * ME_W, 1) vegas_integrand_kernel(VegasArgs a, double* __restrict__ f_out,
                                                                  unsigned long long* __restrict__ idx_out, int idx_words,
                                                                  double* __restrict__ stage_all) {
-  constexpr int NF = P::N_EXT - 2;
+  constexpr int NF = P::N_EXT - 2, W = ME_W;
   constexpr int STRIDE = EventSmem<P>::DOUBLES;
   constexpr int SLOT = 4 * NF + 4;  // final momenta, weight, event index, beam energy, pad
   extern __shared__ __align__(16) double smem[];
@@ -24,6 +24,7 @@ __global__ void __launch_bounds__(32 * W) vegas_integrand_kernel(VegasArgs a, do
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   double* mom_s = smem + warp * STRIDE;
   double* stage = stage_all + static_cast<long long>(blockIdx.x) * (32 * W) * SLOT;
+  const uint32_t tmem = JPark<P>::ON ? tmem_alloc<JPark<P>::COLS>() : 0u;
   const long long n_batches = (a.n_ev + 32 * W - 1) / (32 * W);
   for (long long b = blockIdx.x; b < n_batches; b += gridDim.x) {
     const long long ev = (b * W + warp) * 32 + lane;
@@ -92,13 +93,14 @@ __global__ void __launch_bounds__(32 * W) vegas_integrand_kernel(VegasArgs a, do
       const double e_beam = s[4 * NF + 2];
       if (lane < 8) mom_s[lane] = (lane == 0 || lane == 3 || lane == 4) ? e_beam : (lane == 7 ? -e_beam : 0.0);
       else if (lane < 8 + 4 * NF) mom_s[lane] = s[lane - 8];
-      cta_sync<W>();
-      const double r = cta_me2<P, W>(smem, a.mass, a.scale, nullptr);
+      __syncthreads();
+      const double r = cta_me2<P>(smem, a.mass, a.scale, nullptr, tmem);
       if (valid && lane == 0) f_out[__double_as_longlong(s[4 * NF + 1])] = s[4 * NF] * r;
-      cta_sync<W>();
+      __syncthreads();
     }
     __syncthreads();  // the staging area and warp_count are reused by the next batch
   }
+  if (JPark<P>::ON) tmem_free<JPark<P>::COLS>(tmem);
 }
 
 }  // namespace madme

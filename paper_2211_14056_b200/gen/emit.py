@@ -2,14 +2,19 @@
 
 Output: paper_2211_14056_b200/csrc/generated/<process>.inc — a struct with
   * the scratch layout of one event: a BASE region (subset momenta, external wavefunctions, the currents that
-    feed other currents) and one ROUND region that successive rounds reuse,
-  * one table of 128-bit task rows (me_tasks.cuh::MeRow) in execution order: the base currents level by level,
-    then for every round the open / propagated currents of its leg splits and their colour-ordered combinations,
+    feed other currents) and one ROUND region that successive rounds reuse.  Only objects that somebody READS are
+    stored: the feeds and the two operands of every propagator-cut dot product;
+  * a table of ITEMS (me_tasks.cuh::MeItem / MeMember).  One item = up to NSLOT colour-ordered currents over one leg
+    set (the operands of the dot products of one leg split, or one feed), for VPI helicity variants.  Its MEMBERS
+    are the bare vertices of the Feynman subdiagrams that enter those currents; they are evaluated in registers, summed
+    with their {+-1, +-i} coefficients into the item's accumulators, the common propagator is applied ONCE to each
+    sum and only the sums are stored.  (Round 1 stored every member and summed them in separate combination rows:
+    444 of 1 041 rows were load-add-store.)  Items are warp-uniform: the 32 lanes are VPI variants x W events;
   * per round, straight-line code `dots(r, sm, h, jr, ji)` for ONE helicity combination (one lane): the
     propagator-cut dot products of the round's leg splits, accumulated straight into the colour-flow vector J
     (steps a7-a8), and `colour(jr, ji)` = J^dagger CF J (step a9).
-A round is: tasks -> barrier -> combinations -> barrier -> dots -> barrier; J stays in registers across rounds, so an
-event needs BASE + max(ROUND) doubles of shared memory, not the sum over all leg splits.
+A round is: items -> barrier -> dots -> barrier; J is carried across rounds (registers, parked in tensor memory while
+the next round's items run), so an event needs BASE + max(ROUND) doubles of shared memory.
 The file is `__host__ __device__` so tests/ can run it on the CPU for debugging.
 
 Run `python -m paper_2211_14056_b200.gen.emit` to regenerate all processes (done by build()).
@@ -18,23 +23,25 @@ import os
 
 from .diagrams import PROCESSES, Program
 
-OPCODE = {"FFV_ROW": 0, "FFV_COL": 1, "FFV_VEC": 2, "VVV": 3, "VVVV1": 4}
-OP_COMBO, OP_NOP = 5, 7
 HERE = os.path.dirname(os.path.abspath(__file__))
 OUT_DIR = os.path.join(os.path.dirname(HERE), "csrc", "generated")
-N_ROUNDS = int(os.environ.get("MADME_GEN_ROUNDS", "4"))   # shared-memory footprint knob (see Layout)
-GROUP_PAD = int(os.environ.get("MADME_GEN_GROUP_PAD", "4"))   # rows of one op come in multiples of this (a CTA of 8 events maps 4 rows x 8 events on a warp)
+NSLOT = 4            # accumulators (colour-ordered currents) per item
+W_EVENTS = 8         # events per CTA = warps per CTA
+VPI = 32 // W_EVENTS  # helicity variants per item (lanes = VPI variants x W_EVENTS events)
+# shared-memory budget: doubles per event so that W_EVENTS events fit in the 227 KB a CTA can own
+SMEM_BUDGET_DOUBLES = int(os.environ.get("MADME_GEN_SMEM_DOUBLES", str((232448 // (8 * W_EVENTS)) - 32 - 16)))
+N_ROUNDS = int(os.environ.get("MADME_GEN_ROUNDS", "0"))   # 0: the fewest rounds that fit the budget
 
-# fp64 operation counts of the routines in csrc/helas.cuh as written (FMA = 2, add/mul = 1; complex mul = 1 mul +
-# 1 fma per component = 6, complex fma = 8).  (propagated, open) forms.
-FLOPS = {
-    "FFV_ROW": (8 + 4 * 14 + 2 + 4 * 24 + 8, 8 + 4 * 14),      # slash (4 cadd + 4 (cmul + cfma)) + (Kslash + m) x f
-    "FFV_COL": (8 + 4 * 14 + 2 + 4 * 24 + 8, 8 + 4 * 14),
-    "FFV_VEC": (8 * 6 + 12 * 2 + 8, 8 * 6 + 12 * 2 + 8),
-    "VVV": (12 + 14 * 3 + 4 * 20, 12 + 14 * 3 + 4 * 20),
-    "VVVV": (3 * 30 + 6 + 4 * 24, 3 * 30 + 6 + 4 * 24),
-    "DOT": 4 * 8, "EXT": 45,
-}
+OP_SLASH_ROW, OP_SLASH_COL, OP_FFV_VEC, OP_VVV, OP_VVVV = range(5)
+KIND_VEC, KIND_ROW, KIND_COL, KIND_OPEN = range(4)
+UNIT_OP = {"FFV_ROW": OP_SLASH_ROW, "FFV_COL": OP_SLASH_COL, "FFV_VEC": OP_FFV_VEC, "VVV": OP_VVV, "VVVV": OP_VVVV}
+
+# fp64 operation counts of the routines in csrc/helas.cuh / me_tasks.cuh as written (FMA = 2, add/mul = 1; complex
+# mul = 6, complex fma = 8, real x complex fma = 4)
+FLOPS_UNIT = {OP_SLASH_ROW: 64, OP_SLASH_COL: 64, OP_FFV_VEC: 72, OP_VVV: 150, OP_VVVV: 186}
+FLOPS_ACC = 8                                   # acc += i^k x
+FLOPS_FIN = {KIND_VEC: 8, KIND_ROW: 66, KIND_COL: 66, KIND_OPEN: 0}
+FLOPS_DOT, FLOPS_EXT = 4 * 8, 45
 
 
 def bits_of(legs):
@@ -51,29 +58,48 @@ def variant_index(sub_legs, sup_legs, v):
     return r
 
 
+class Unit:
+    """One bare vertex evaluation: a Feynman subdiagram's last vertex without its propagator.  A four-gluon vertex
+    yields three terms (its three colour x Lorentz structures) from one evaluation."""
+
+    def __init__(self, op, args):
+        self.op, self.args = op, args
+        self.codes = [[0] * NSLOT for _ in range(3)]     # [term][slot] -> 0 | 4 + k  (coefficient i^k)
+
+
+class Task:
+    def __init__(self, outputs):
+        self.outputs = outputs          # stored objects (ids), <= NSLOT
+        self.units = []
+
+
 class Layout:
-    """Where every object of one event lives.  A leg split = (legs of the open side U | the rest); all objects that
-    only serve one split (its open currents, its top-level propagated currents, the combinations of both sides)
-    live in the round region while that split's round is processed."""
+    """Where every STORED object of one event lives, and the items that compute them.  A leg split = (legs of the
+    open side U | the rest); the operands of a split's dot products live in the round region while that split's
+    round is processed."""
 
     def __init__(self, P, n_rounds):
         self.P = P
         objs = P.used_objects()
         self.objs = objs
         all_legs = tuple(range(P.n))
-        subsets = sorted({o.legs for o in objs}, key=lambda s: (len(s), s))
-        self.subsets = subsets
-        self.sub_index = {s: i for i, s in enumerate(subsets)}
-        feeds = set()                      # objects that are inputs of vertex tasks
+        feeds = set()                      # objects that are inputs of vertices
         for o in objs:
             if o.op != "COMBO":
                 feeds.update(o.args)
+        dot_ops = set()
+        for (_, u, c, _, _) in P.dots:
+            dot_ops.update((u, c))
         self.base = [o for o in objs if o.op == "EXT" or o.id in feeds]
         base_ids = {o.id for o in self.base}
-        # split of every other object: U side -> its own legs; C side -> the complement
+        self.stored = [o for o in objs if o.id in base_ids or o.id in dot_ops]
+        subsets = sorted({o.legs for o in objs}, key=lambda s: (len(s), s))
+        self.subsets = subsets
+        self.sub_index = {s: i for i, s in enumerate(subsets)}
+        # split of every stored object outside the base: U side -> its own legs; C side -> the complement
         u_sets = {P.objs[d[1]].legs for d in P.dots}
         self.split_of = {}
-        for o in objs:
+        for o in self.stored:
             if o.id in base_ids:
                 continue
             comp = tuple(l for l in all_legs if l not in o.legs)
@@ -81,7 +107,7 @@ class Layout:
             assert self.split_of[o.id] in u_sets, o.legs
         self.splits = sorted(u_sets, key=lambda s: (len(s), s))
         size = {s: 0 for s in self.splits}
-        for o in objs:
+        for o in self.stored:
             if o.id in self.split_of:
                 size[self.split_of[o.id]] += 8 * self.nv(o)
         bins = [[0, []] for _ in range(max(1, min(n_rounds, len(self.splits))))]
@@ -95,7 +121,7 @@ class Layout:
         # Fixed-stride storage: a GROUP is 4 lines of 128 B (one line per wavefunction component); an object with nv
         # variants owns nv consecutive 16-byte slots (aligned to nv) in each line, so component c of variant v sits at
         # double offset  group*64 + c*16 + (slot+v)*2 : the four component loads of a wavefunction are ONE address plus
-        # the immediates 0, 128, 256, 384 bytes, whatever nv is.
+        # the immediates 0, 128, 256, 384 bytes, whatever nv is.  Objects with more than 8 variants take whole groups.
         start = 8 * len(subsets)
         start = ((start + 15) // 16) * 16
         self.off = {}
@@ -104,7 +130,7 @@ class Layout:
             groups = []          # free slot bitmaps
             for o in sorted(obj_list, key=lambda o: (-self.nv(o), o.id)):
                 nv = self.nv(o)
-                assert nv <= 8
+                assert nv <= 8, "objects with more than 8 helicity variants need a wider storage group"
                 for gi, used in enumerate(groups):
                     slot = next((s0 for s0 in range(0, 8, nv) if not any(used[s0:s0 + nv])), None)
                     if slot is not None:
@@ -121,32 +147,177 @@ class Layout:
         self.base_doubles = base_end
         tmax = base_end
         for r in range(len(self.rounds)):
-            tmax = max(tmax, allocate([o for o in objs if o.id in self.split_of and self.round_of[self.split_of[o.id]] == r], base_end))
+            tmax = max(tmax, allocate(self.round_objs(r), base_end))
         self.smem_doubles = tmax
 
     def nv(self, o):
         return 1 << len(bits_of(o.legs))
 
     def round_objs(self, r):
-        return [o for o in self.objs if o.id in self.split_of and self.round_of[self.split_of[o.id]] == r]
+        return [o for o in self.stored if o.id in self.split_of and self.round_of[self.split_of[o.id]] == r]
+
+    # ---- tasks -------------------------------------------------------------------------------------------------
+    def members_of(self, o):
+        """[(member object, coefficient)] of a stored object: a combination's members, or the object itself."""
+        P = self.P
+        if o.op == "COMBO":
+            return [(P.objs[a], c) for a, c in zip(o.args, P.combo_coefs[o.id])]
+        return [(o, 1)]
+
+    @staticmethod
+    def unit_key(m):
+        return ("VVVV" if m.op.startswith("VVVV") else m.op, m.args)
+
+    def make_tasks(self, outputs):
+        """Tasks (<= NSLOT outputs each) for stored objects over ONE leg set with one propagator flag."""
+        outputs = sorted(outputs, key=lambda o: o.id)
+        keys = {o.id: {self.unit_key(m) for m, _ in self.members_of(o)} for o in outputs}
+        tasks, left = [], list(outputs)
+        while left:
+            grp = [left.pop(0)]
+            have = set(keys[grp[0].id])
+            while left and len(grp) < NSLOT:
+                best = max(left, key=lambda o: (len(keys[o.id] & have), -len(keys[o.id] - have), -o.id))
+                left.remove(best)
+                grp.append(best)
+                have |= keys[best.id]
+            t = Task(grp)
+            units = {}
+            for s, o in enumerate(grp):
+                for m, coef in self.members_of(o):
+                    assert m.legs == o.legs and m.prop == o.prop and m.type == o.type
+                    k = self.unit_key(m)
+                    if k not in units:
+                        units[k] = Unit(UNIT_OP[k[0]], m.args)
+                        t.units.append(units[k])
+                    term = int(m.op[4]) - 1 if m.op.startswith("VVVV") else 0
+                    assert units[k].codes[term][s] == 0
+                    units[k].codes[term][s] = 4 + {1: 0, 1j: 1, -1: 2, -1j: 3}[coef]
+            tasks.append(t)
+        return tasks
+
+    def task_flops(self, t):
+        o = t.outputs[0]
+        kind = self.kind_of(o)
+        f = sum(FLOPS_UNIT[u.op] + FLOPS_ACC * sum(1 for term in u.codes for c in term if c) for u in t.units)
+        return f + FLOPS_FIN[kind] * len(t.outputs)
+
+    def kind_of(self, o):
+        if not o.prop:
+            return KIND_OPEN
+        return {"V": KIND_VEC, "O": KIND_ROW, "I": KIND_COL}[o.type[0]]
+
+
+def pick_rounds(P):
+    if N_ROUNDS:
+        return Layout(P, N_ROUNDS)
+    for n in range(1, 17):
+        L = Layout(P, n)
+        if 4 * P.n + L.smem_doubles <= SMEM_BUDGET_DOUBLES or n >= len(L.splits):
+            return L
+    return L
 
 
 def emit_process(name, n_rounds=None):
     P = Program(name)
     assert all(t.op.startswith("DOT") for t in P.terms), "every diagram must be a propagator-cut contraction"
-    L = Layout(P, N_ROUNDS if n_rounds is None else n_rounds)
+    L = Layout(P, n_rounds) if n_rounds else pick_rounds(P)
     n = P.n
     nf = len(P.flow_perms)
     W = []
     w = W.append
     s = P.summary()
+
+    # ---- items ---------------------------------------------------------------------------------------------------
+    members = []          # 8-word records
+    items = []            # 4-word records, in execution order (stage by stage, interleaved over the W_EVENTS warps)
+    stage_end, stage_dots = [], []
+    cur_flops = 0
+    n_tasks = n_units = 0
+    sub_i = lambda legs: L.sub_index[legs]
+
+    def massive_of(o):
+        return 1 if (o.type[0] in "OI" and P.legs[[l for l in o.legs if P.legs[l].kind >= 2][0]].massive) else 0
+
+    def add_stage(task_list, dots_round):
+        """Items of the tasks, balanced over the warps by estimated cost (longest first), then interleaved so that
+        warp w runs items w, w + W_EVENTS, ... of the stage."""
+        nonlocal cur_flops, n_tasks, n_units
+        pending = []
+        for t in task_list:
+            o = t.outputs[0]
+            nv = L.nv(o)
+            n_tasks += 1
+            n_units += len(t.units)
+            cur_flops += L.task_flops(t) * nv
+            for vbase in range(0, nv, VPI):
+                pending.append((L.task_flops(t), t, vbase))
+        pending.sort(key=lambda x: -x[0])
+        queues = [[0, []] for _ in range(W_EVENTS)]
+        for cost, t, vbase in pending:
+            q = min(queues, key=lambda x: x[0])
+            q[0] += cost
+            q[1].append((t, vbase))
+        depth = max(len(q[1]) for q in queues) if pending else 0
+        for k in range(depth):
+            for q in queues:
+                if k < len(q[1]):
+                    items.append(encode_item(*q[1][k]))
+                else:
+                    items.append((0, 0, 0, 0))
+        stage_end.append(len(items))
+        stage_dots.append(dots_round)
+
+    def encode_item(t, vbase):
+        o = t.outputs[0]
+        nv = L.nv(o)
+        first = len(members)
+        for u in t.units:
+            args = [P.objs[a] for a in u.args]
+            offs, vmaps = [], []
+            for a in args:
+                assert a.id in L.off, "a vertex argument must be a stored object"
+                offs.append(L.off[a.id])
+                vm = 0
+                for j in range(VPI):
+                    if vbase + j < nv:
+                        vm |= variant_index(a.legs, o.legs, vbase + j) << (4 * j)
+                vmaps.append(vm)
+            while len(offs) < 3:
+                offs.append(0)
+                vmaps.append(0)
+            assert max(offs) < 65536
+            ks = [sub_i(a.legs) for a in args[:2]]
+            code = lambda term: sum(c << (3 * sl) for sl, c in enumerate(u.codes[term]))
+            members.append((u.op | (ks[0] << 8) | (ks[1] << 16), offs[0] | (offs[1] << 16), offs[2] | (vmaps[2] << 16),
+                            vmaps[0] | (vmaps[1] << 16), code(0) | (code(1) << 12), code(2), 0, 0))
+        outs = [L.off[x.id] for x in t.outputs] + [0] * NSLOT
+        assert first < 65536 and len(t.units) < 256 and nv < 256
+        w0 = len(t.units) | (len(t.outputs) << 8) | (L.kind_of(o) << 12) | (massive_of(o) << 15) | (nv << 16) | (vbase << 24)
+        return (w0, first | (sub_i(o.legs) << 16), outs[0] | (outs[1] << 16), outs[2] | (outs[3] << 16))
+
+    for lev in sorted({len(o.legs) for o in L.base if o.op != "EXT"}):
+        tasks = []
+        for o in L.base:
+            if len(o.legs) == lev and o.op != "EXT":
+                tasks += L.make_tasks([o])
+        add_stage(tasks, -1)
+    for r in range(len(L.rounds)):
+        cells = {}
+        for o in L.round_objs(r):
+            cells.setdefault((o.legs, o.prop), []).append(o)
+        tasks = []
+        for key in sorted(cells):
+            tasks += L.make_tasks(cells[key])
+        add_stage(tasks, r)
+
     w("// GENERATED by paper_2211_14056_b200/gen/emit.py — do not edit; regenerate with")
     w("//   python -m paper_2211_14056_b200.gen.emit")
     w("// process %s: %d Feynman diagrams (%d with a 4-gluon vertex), %d colour-pure terms, %d colour flows"
       % (name, s["n_diagrams"], s["n_diagrams_4g"], s["n_terms"], s["n_flows"]))
     w("// (SURVEY.md §8 table; PAPER.md:57-58 Table 1 pins 16 and 123 through 36 = 16+4x5, 267 = 123+4x36)")
-    w("// evaluation: %d off-shell currents, %d colour-ordered combinations and %d propagator-cut dot products per"
-      % (s["n_currents"], s["n_combos"], s["n_dots"]))
+    w("// evaluation: %d stored currents computed by %d tasks from %d bare vertices, %d propagator-cut dot products per"
+      % (sum(1 for o in L.stored if o.op != "EXT"), n_tasks, n_units, s["n_dots"]))
     w("// helicity combination over %d leg splits in %d rounds; %d of %d combinations evaluated (parity, leg 0 at +1)"
       % (len(L.splits), len(L.rounds), 1 << (n - 1), 1 << n))
     w("#pragma once")
@@ -162,79 +333,6 @@ def emit_process(name, n_rounds=None):
       % (P.cf_den, P.avg, 2 * (n - 2)))
     w("  static constexpr bool QED = %s;" % ("true" if P.coupling == "ee" else "false"))
 
-    # ---- the task table --------------------------------------------------------------------------------------
-    rows = []
-    cur_flops = 0
-    lg = lambda nv: {1: 0, 2: 1, 4: 2, 8: 3, 16: 4, 32: 5}[nv]
-    sub_i = lambda o: L.sub_index[o.legs]
-
-    def pad(mult):
-        while len(rows) % mult:
-            rows.append((0, 0, OP_NOP << 24, 0))
-
-    def add_tasks(objs):
-        nonlocal cur_flops
-        for opn, prop in [(a, b) for a in ("FFV_ROW", "FFV_COL", "FFV_VEC", "VVV", "VVVV1") for b in (True, False)]:
-            for o in objs:
-                if o.op != opn or o.prop != prop:   # open and propagated currents in separate groups: uniform branches
-                    continue
-                args = [P.objs[a] for a in o.args]
-                nv = L.nv(o)
-                sibs = []
-                if opn == "VVVV1":
-                    sibs = [x for x in L.objs if x.op in ("VVVV2", "VVVV3") and x.args == o.args and x.legs == o.legs and x.prop == o.prop]
-                    sibs.sort(key=lambda x: x.op)
-                    assert len(sibs) == 2
-                massive = 1 if (o.type[0] in "OI" and P.legs[[l for l in o.legs if P.legs[l].kind >= 2][0]].massive) else 0
-                for v in range(nv):
-                    offs = [L.off[a.id] + 2 * variant_index(a.legs, o.legs, v) for a in args] + [0]
-                    assert max(offs) < 65536 and L.off[o.id] + 2 * v < 65536
-                    x = (L.off[o.id] + 2 * v) | (offs[0] << 16)
-                    y = offs[1] | ((offs[2] if len(args) > 2 else 0) << 16)
-                    flags = (OPCODE[opn] << 24) | (massive << 27) | ((0 if o.prop else 1) << 28)
-                    if sibs:   # four-gluon current: no argument momenta needed; the two sibling outputs take their place
-                        z = sub_i(o) | ((L.off[sibs[0].id] + 2 * v) << 8) | flags
-                        wv = L.off[sibs[1].id] + 2 * v
-                        assert L.off[sibs[0].id] + 2 * v < 65536
-                    else:
-                        z = sub_i(o) | (sub_i(args[0]) << 8) | (sub_i(args[1]) << 16) | flags
-                        wv = 0
-                    rows.append((x, y, z, wv))
-                    cur_flops += FLOPS["VVVV" if opn == "VVVV1" else opn][0 if o.prop else 1]
-            pad(GROUP_PAD)
-        pad(32)
-
-    def add_combos(objs):
-        nonlocal cur_flops
-        for o in objs:
-            if o.op != "COMBO":
-                continue
-            coefs = P.combo_coefs[o.id]
-            assert len(coefs) <= 4 and coefs[0] == 1
-            nv = L.nv(o)
-            for v in range(nv):
-                m = [L.off[a] + 2 * v for a in o.args] + [0, 0, 0]
-                k = [{1: 0, 1j: 1, -1: 2, -1j: 3}[zc] for zc in coefs] + [0, 0, 0]
-                x = (L.off[o.id] + 2 * v) | (m[0] << 16)
-                y = m[1] | (m[2] << 16)
-                z = m[3] | (OP_COMBO << 24)
-                wv = (len(coefs) << 16) | (k[1] << 22) | (k[2] << 24) | (k[3] << 26)
-                rows.append((x, y, z, wv))
-                cur_flops += 8 * (len(coefs) - 1)
-        pad(32)
-
-    base_ends = []
-    for lev in sorted({len(o.legs) for o in L.base if o.op != "EXT"}):
-        add_tasks([o for o in L.base if len(o.legs) == lev and o.op != "EXT"])
-        base_ends.append(len(rows))
-    raw_ends, combo_ends = [], []
-    for r in range(len(L.rounds)):
-        ro = L.round_objs(r)
-        add_tasks(ro)
-        raw_ends.append(len(rows))
-        add_combos(ro)
-        combo_ends.append(len(rows))
-
     def table_fn(fname, vals):
         w("  static ME_HD int %s(int i) {" % fname)
         w("    switch (i) {")
@@ -244,23 +342,20 @@ def emit_process(name, n_rounds=None):
         w("    }")
         w("  }")
 
-    # phases: rows up to phase_end(p), barrier, then (if phase_dots(p) >= 0) the dot products of that round, barrier
-    ph_end = list(base_ends)
-    ph_dots = [-1] * len(base_ends)
-    for r in range(len(L.rounds)):
-        if raw_ends[r] > (ph_end[-1] if ph_end else 0) and combo_ends[r] > raw_ends[r]:
-            ph_end.append(raw_ends[r])
-            ph_dots.append(-1)
-        ph_end.append(combo_ends[r])
-        ph_dots.append(r)
-    w("  static constexpr int N_ROWS = %d, N_ROUNDS = %d, N_PHASES = %d;" % (len(rows), len(L.rounds), len(ph_end)))
-    w("  // phase p: task rows up to phase_end(p), barrier, then the dot products of round phase_dots(p) (if >= 0), barrier")
-    table_fn("phase_end", ph_end)
-    table_fn("phase_dots", ph_dots)
-    w("#define %s_TASK_TABLE { \\" % name.upper())
-    for r4 in rows:
+    w("  static constexpr int N_ITEMS = %d, N_MEMBERS = %d, N_ROUNDS = %d, N_STAGES = %d, N_TASKS = %d, N_UNITS = %d;"
+      % (len(items), len(members), len(L.rounds), len(stage_end), n_tasks, n_units))
+    w("  // stage p: items up to stage_end(p) (warp w takes items w, w + %d, ...), barrier, then the dot products of round" % W_EVENTS)
+    w("  // stage_dots(p) (if >= 0), barrier")
+    table_fn("stage_end", stage_end)
+    table_fn("stage_dots", stage_dots)
+    w("#define %s_ITEM_TABLE { \\" % name.upper())
+    for r4 in items:
         w("  {%du,%du,%du,%du}, \\" % r4)
-    w("  {0u,0u,%du,0u} }" % (OP_NOP << 24))
+    w("  {0u,0u,0u,0u} }")
+    w("#define %s_MEMBER_TABLE { \\" % name.upper())
+    for r8 in members:
+        w("  {{%du,%du,%du,%du,%du,%du,%du,%du}}, \\" % r8)
+    w("  {{0u,0u,0u,0u,0u,0u,0u,0u}} }")
     w("#define %s_SUB_MASKS { %s }" % (name.upper(), ",".join(str(sum(1 << l for l in sub)) for sub in L.subsets)))
     w("#define %s_LEG_KIND { %s }" % (name.upper(), ",".join(str(leg.kind) for leg in P.legs)))
     w("#define %s_LEG_MASSIVE { %s }" % (name.upper(), ",".join("1" if leg.massive else "0" for leg in P.legs)))
@@ -297,7 +392,7 @@ def emit_process(name, n_rounds=None):
                 for (f, uu, c, z, kind) in dots:
                     if uu == u:
                         w("            dot_acc<%d, %s>(jr[%d], ji[%d], u, c%d);" % (zcode[z], "true" if kind == "V" else "false", f, f, c))
-                        amp_flops += FLOPS["DOT"]
+                        amp_flops += FLOPS_DOT
                 w("          }")
             w("        }")
         w("      } break;")
@@ -336,10 +431,10 @@ def emit_process(name, n_rounds=None):
         col_flops += 2
     w("    return " + " + ".join(expr) + ";")
     w("  }")
-    ext_flops = FLOPS["EXT"] * 2 * n
+    ext_flops = FLOPS_EXT * 2 * n
     nh = 1 << (n - 1)
     per_event = ext_flops + cur_flops + nh * (amp_flops + col_flops)
-    w("  // nominal fp64 flops per event as emitted (FMA = 2): externals %d + currents and combinations %d + %d helicities x"
+    w("  // nominal fp64 flops per event as emitted (FMA = 2): externals %d + currents %d + %d helicities x"
       % (ext_flops, cur_flops, nh))
     w("  // (dot products %d + colour %d)" % (amp_flops, col_flops))
     w("  static constexpr double FLOPS_PER_EVENT = %d.0;" % per_event)

@@ -1,5 +1,5 @@
 // TEST-ONLY harness: runs the GENERATED matrix-element programs (csrc/generated/*.inc, csrc/helas.cuh,
-// csrc/me_tasks.cuh) on the CPU by emulating the 32 lanes of a warp one after the other.  It exists so the
+// csrc/me_tasks.cuh) on the CPU by emulating the lanes of a warp one after the other.  It exists so the
 // generator's diagram / colour / phase logic and the vertex routines can be checked against the oracle in the
 // `-m "not gpu"` suite, where no GPU is available.  It is compiled by tests/test_generated_host.py with g++ and
 // is NOT part of the product library: libmadme.so has no CPU path.
@@ -16,7 +16,8 @@ using namespace madme;
 template <class P> struct Tables;
 #define DEF_TABLES(P, U)                                        \
   template <> struct Tables<P> {                                \
-    static const MeRow* tasks() { static const MeRow t[] = U##_TASK_TABLE; return t; }  \
+    static const MeItem* items() { static const MeItem t[] = U##_ITEM_TABLE; return t; }        \
+    static const MeMember* members() { static const MeMember t[] = U##_MEMBER_TABLE; return t; } \
     static const int* masks() { static const int t[] = U##_SUB_MASKS; return t; }       \
     static const int* kind() { static const int t[] = U##_LEG_KIND; return t; }         \
     static const int* massive() { static const int t[] = U##_LEG_MASSIVE; return t; }   \
@@ -27,8 +28,10 @@ DEF_TABLES(gg_ttx, GG_TTX)
 DEF_TABLES(gg_ttxg, GG_TTXG)
 DEF_TABLES(gg_ttxgg, GG_TTXGG)
 
-template <class P> void rows(double* sm, int begin, int end, double mass) {
-  for (int lane = 0; lane < 32; ++lane) me_run_rows(lane, sm, Tables<P>::tasks(), begin, end, mass);
+// items [begin, end) of one stage for ONE event: the device runs them with lanes = (local variant j, event)
+template <class P> void items(double* sm, int begin, int end, double mass) {
+  for (int it = begin; it < end; ++it)
+    for (int j = 0; j < 4; ++j) me_run_item(Tables<P>::items()[it], Tables<P>::members(), j, sm, mass);
 }
 
 template <class P> void eval(const double* mom, double* me2, long long n, double mass, double coupling, double* per_hel) {
@@ -40,12 +43,12 @@ template <class P> void eval(const double* mom, double* me2, long long n, double
     for (int lane = 0; lane < 32; ++lane)
       me_phase0(lane, 32, sm.data(), mom + e * 4 * P::N_EXT, P::N_EXT, P::N_SUB, Tables<P>::masks(), Tables<P>::kind(),
                 Tables<P>::massive(), Tables<P>::ext_off(), mass);
-    int row = 0;
+    int it = 0;
     std::vector<double> jr(P::N_HEL_EVAL * P::N_FLOW, 0.0), ji(P::N_HEL_EVAL * P::N_FLOW, 0.0);
-    for (int p = 0; p < P::N_PHASES; ++p) {
-      rows<P>(sm.data(), row, P::phase_end(p), mass);
-      row = P::phase_end(p);
-      const int r = P::phase_dots(p);
+    for (int p = 0; p < P::N_STAGES; ++p) {
+      items<P>(sm.data(), it, P::stage_end(p), mass);
+      it = P::stage_end(p);
+      const int r = P::stage_dots(p);
       if (r >= 0)
         for (int h = 0; h < P::N_HEL_EVAL; ++h) P::dots(r, sm.data(), h, &jr[h * P::N_FLOW], &ji[h * P::N_FLOW]);
     }
