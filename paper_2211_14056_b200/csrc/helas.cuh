@@ -302,4 +302,22 @@ template <int K, bool MINK> ME_HD void dot_acc(double& jr, double& ji, const wf4
   cacc<MINK ? ((K + 2) & 3) : K>(jr, ji, u.c[3], c.c[3]);
 }
 
+// the same contraction as a value (a U . C pair that feeds several colour flows is contracted once) ...
+template <bool MINK> ME_HD cplx dot_val(const wf4& u, const wf4& c) {
+  cplx t = u.c[0] * c.c[0];
+  if (MINK) {
+    t = cfms(u.c[1], c.c[1], t); t = cfms(u.c[2], c.c[2], t); t = cfms(u.c[3], c.c[3], t);
+  } else {
+    t = cfma(u.c[1], c.c[1], t); t = cfma(u.c[2], c.c[2], t); t = cfma(u.c[3], c.c[3], t);
+  }
+  return t;
+}
+// ... and J += i^K t
+template <int K> ME_HD void jadd(double& jr, double& ji, cplx t) {
+  if (K == 0) { jr += t.re; ji += t.im; }
+  else if (K == 2) { jr -= t.re; ji -= t.im; }
+  else if (K == 1) { jr -= t.im; ji += t.re; }
+  else { jr += t.im; ji -= t.re; }
+}
+
 }  // namespace madme

@@ -90,7 +90,9 @@ template <class P>
 __device__ __forceinline__ double cta_me2(double* smem, double mass, double scale, double* hel_out, uint32_t tmem) {
   constexpr int STRIDE = EventSmem<P>::DOUBLES;
   constexpr int W = ME_W;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  // the warp index through a shuffle: the compiler then knows it is warp-uniform, so the item loop (table reads, op
+  // and coefficient decoding, branches) runs on the uniform datapath
+  const int lane = threadIdx.x & 31, warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
   // a5: subset momenta / denominators and external wavefunctions, work = (subset or leg, event)
   {
     const int t = threadIdx.x, ev = t % W;

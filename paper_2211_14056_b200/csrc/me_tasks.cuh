@@ -38,8 +38,8 @@ namespace madme {
 //   w0: op | ksub_a << 8 | ksub_b << 16
 //   w1: a | b << 16,   w2: c | vmap_c << 16,   w3: vmap_a | vmap_b << 16
 //        (vmap: 4 bits per local variant j: which variant of the argument enters variant vbase + j of the outputs)
-//   w4: codes of term 0 | codes of term 1 << 12,   w5: codes of term 2
-//        (3 bits per accumulator: 4 + k adds i^k x; terms 1, 2 exist for the four-gluon vertex only)
+//   w4: code of term 0 | code of term 1 << 9 | code of term 2 << 18      (see acc_term; terms 1, 2 exist for the
+//        four-gluon vertex only)
 struct MeItem { unsigned w0, w1, w2, w3; };
 struct MeMember { unsigned w[8]; };
 enum MeOp { OP_SLASH_ROW = 0, OP_SLASH_COL = 1, OP_FFV_VEC = 2, OP_VVV = 3, OP_VVVV = 4 };
@@ -116,26 +116,38 @@ ME_HD void me_phase0(int idx, int step, double* sm, const double* mom, int n_ext
   }
 }
 
-// acc += i^k x  (k warp-uniform: a four-way branch, eight additions)
-ME_HD void acc_add(wf4& acc, const wf4& x, int k) {
-  if (k == 0) {
-    for (int c = 0; c < 4; ++c) { acc.c[c].re += x.c[c].re; acc.c[c].im += x.c[c].im; }
-  } else if (k == 2) {
-    for (int c = 0; c < 4; ++c) { acc.c[c].re -= x.c[c].re; acc.c[c].im -= x.c[c].im; }
-  } else if (k == 1) {
-    for (int c = 0; c < 4; ++c) { acc.c[c].re -= x.c[c].im; acc.c[c].im += x.c[c].re; }
-  } else {
-    for (int c = 0; c < 4; ++c) { acc.c[c].re += x.c[c].im; acc.c[c].im -= x.c[c].re; }
-  }
-}
-// the term x enters accumulator s with i^(code & 3) if bit 2 of its 3-bit code is set
-ME_HD void acc_term(wf4 (&acc)[ME_NSLOT], const wf4& x, unsigned codes) {
+// A term x of a bare vertex enters the item's accumulators as  acc_s += e_s (i^b x),  e_s in {0, +1, -1}: its 9-bit code
+// is  b | sign_0 << 1 | sign_1 << 3 | sign_2 << 5 | sign_3 << 7  with sign 0 none, 1 plus, 2 minus (gen/emit.py:
+// Task.solve_phases).  Everything here is warp-uniform; the only branches are on b and on "more than two currents".
+ME_HD double sign_of(unsigned code2) {   // 0 -> 0.0, 1 -> +1.0, 2 -> -1.0
 #if defined(__CUDA_ARCH__)
-#pragma unroll
+  return __hiloint2double(static_cast<int>((code2 ? 0x3FF00000u : 0u) | ((code2 & 2u) << 30)), 0);
+#else
+  return code2 == 0 ? 0.0 : (code2 == 1 ? 1.0 : -1.0);
 #endif
-  for (int s = 0; s < ME_NSLOT; ++s) {
-    const unsigned c = (codes >> (3 * s)) & 7u;
-    if (c & 4u) acc_add(acc[s], x, static_cast<int>(c & 3u));
+}
+ME_HD void acc_plain(wf4& acc, const wf4& x, double e) {
+  for (int c = 0; c < 4; ++c) { acc.c[c].re = fma(e, x.c[c].re, acc.c[c].re); acc.c[c].im = fma(e, x.c[c].im, acc.c[c].im); }
+}
+ME_HD void acc_times_i(wf4& acc, const wf4& x, double e) {
+  for (int c = 0; c < 4; ++c) { acc.c[c].re = fma(-e, x.c[c].im, acc.c[c].re); acc.c[c].im = fma(e, x.c[c].re, acc.c[c].im); }
+}
+ME_HD void acc_term(wf4 (&acc)[ME_NSLOT], const wf4& x, unsigned code, bool wide) {
+  const double e0 = sign_of((code >> 1) & 3u), e1 = sign_of((code >> 3) & 3u);
+  if (code & 1u) {
+    acc_times_i(acc[0], x, e0);
+    acc_times_i(acc[1], x, e1);
+    if (wide) {
+      acc_times_i(acc[2], x, sign_of((code >> 5) & 3u));
+      acc_times_i(acc[3], x, sign_of((code >> 7) & 3u));
+    }
+  } else {
+    acc_plain(acc[0], x, e0);
+    acc_plain(acc[1], x, e1);
+    if (wide) {
+      acc_plain(acc[2], x, sign_of((code >> 5) & 3u));
+      acc_plain(acc[3], x, sign_of((code >> 7) & 3u));
+    }
   }
 }
 
@@ -145,35 +157,49 @@ ME_HD void me_run_item(const MeItem H, const MeMember* __restrict__ members, int
   const int nv = (H.w0 >> 16) & 0xff, v = static_cast<int>(H.w0 >> 24) + j;
   if (n_mem == 0 || v >= nv) return;
   const int n_out = (H.w0 >> 8) & 0xf, kind = (H.w0 >> 12) & 7;
+  const bool wide = n_out > 2;
   const int sh = 4 * j;
   wf4 acc[ME_NSLOT];
   for (int s = 0; s < ME_NSLOT; ++s)
     for (int c = 0; c < 4; ++c) acc[s].c[c] = mk(0.0, 0.0);
   const MeMember* m = members + (H.w1 & 0xffff);
+  // the operands of member i + 1 are fetched before member i is evaluated
+  unsigned w0 = m->w[0], w2 = m->w[2], w4 = m->w[4];
+  wf4 A, B;
+  {
+    const unsigned w1 = m->w[1], w3 = m->w[3];
+    A = ld_wf(sm + (w1 & 0xffff) + 2 * ((w3 >> sh) & 15u));
+    B = ld_wf(sm + (w1 >> 16) + 2 * ((w3 >> (16 + sh)) & 15u));
+  }
 #if defined(__CUDA_ARCH__)
 #pragma unroll 1
 #endif
-  for (int i = 0; i < n_mem; ++i, ++m) {
-    const unsigned w0 = m->w[0], w1 = m->w[1], w3 = m->w[3], w4 = m->w[4];
-    const int op = w0 & 0xff;
-    const wf4 A = ld_wf(sm + (w1 & 0xffff) + 2 * ((w3 >> sh) & 15u));
-    const wf4 B = ld_wf(sm + (w1 >> 16) + 2 * ((w3 >> (16 + sh)) & 15u));
+  for (int i = 0; i < n_mem; ++i) {
+    const unsigned c0 = w0, c2 = w2, c4 = w4;
+    const wf4 a = A, b = B;
+    if (i + 1 < n_mem) {
+      ++m;
+      const unsigned w1 = m->w[1], w3 = m->w[3];
+      w0 = m->w[0]; w2 = m->w[2]; w4 = m->w[4];
+      A = ld_wf(sm + (w1 & 0xffff) + 2 * ((w3 >> sh) & 15u));
+      B = ld_wf(sm + (w1 >> 16) + 2 * ((w3 >> (16 + sh)) & 15u));
+    }
+    const int op = c0 & 0xff;
     if (op == OP_SLASH_ROW) {
-      acc_term(acc, slash_row(A, B), w4);
+      acc_term(acc, slash_row(a, b), c4 & 0x1ffu, wide);
     } else if (op == OP_SLASH_COL) {
-      acc_term(acc, slash_col(B, A), w4);
+      acc_term(acc, slash_col(b, a), c4 & 0x1ffu, wide);
     } else if (op == OP_FFV_VEC) {
-      acc_term(acc, ffv_vec_bare(A, B), w4);
+      acc_term(acc, ffv_vec_bare(a, b), c4 & 0x1ffu, wide);
     } else if (op == OP_VVV) {
-      acc_term(acc, vvv_vec_bare(A, ld_k(sm + 8 * ((w0 >> 8) & 0xff)), B, ld_k(sm + 8 * ((w0 >> 16) & 0xff))), w4);
+      acc_term(acc, vvv_vec_bare(a, ld_k(sm + 8 * ((c0 >> 8) & 0xff)), b, ld_k(sm + 8 * ((c0 >> 16) & 0xff))), c4 & 0x1ffu, wide);
     } else {
-      const unsigned w2 = m->w[2];
-      const wf4 C = ld_wf(sm + (w2 & 0xffff) + 2 * ((w2 >> (16 + sh)) & 15u));
+      const wf4 C = ld_wf(sm + (c2 & 0xffff) + 2 * ((c2 >> (16 + sh)) & 15u));
       wf4 t1, t2, t3;
-      vvvv_vec_bare(A, B, C, t1, t2, t3);
-      acc_term(acc, t1, w4);
-      acc_term(acc, t2, w4 >> 12);
-      acc_term(acc, t3, m->w[5]);
+      vvvv_vec_bare(a, b, C, t1, t2, t3);
+      acc_term(acc, t1, c4 & 0x1ffu, wide);
+      acc_term(acc, t2, (c4 >> 9) & 0x1ffu, wide);
+      acc_term(acc, t3, (c4 >> 18) & 0x1ffu, wide);
     }
   }
   // the common propagator, once per colour-ordered current

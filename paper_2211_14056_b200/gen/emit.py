@@ -39,7 +39,7 @@ UNIT_OP = {"FFV_ROW": OP_SLASH_ROW, "FFV_COL": OP_SLASH_COL, "FFV_VEC": OP_FFV_V
 # fp64 operation counts of the routines in csrc/helas.cuh / me_tasks.cuh as written (FMA = 2, add/mul = 1; complex
 # mul = 6, complex fma = 8, real x complex fma = 4)
 FLOPS_UNIT = {OP_SLASH_ROW: 64, OP_SLASH_COL: 64, OP_FFV_VEC: 72, OP_VVV: 150, OP_VVVV: 186}
-FLOPS_ACC = 8                                   # acc += i^k x
+FLOPS_ACC = 16                                  # acc += (+-1 | 0) x: one FMA per real component
 FLOPS_FIN = {KIND_VEC: 8, KIND_ROW: 66, KIND_COL: 66, KIND_OPEN: 0}
 FLOPS_DOT, FLOPS_EXT = 4 * 8, 45
 
@@ -65,12 +65,43 @@ class Unit:
     def __init__(self, op, args):
         self.op, self.args = op, args
         self.codes = [[0] * NSLOT for _ in range(3)]     # [term][slot] -> 0 | 4 + k  (coefficient i^k)
+        self.swap = [0, 0, 0]                            # [term] -> b: the term enters as i^b x   (Task.solve_phases)
+        self.sign = [[0] * NSLOT for _ in range(3)]      # [term][slot] -> 0 none | 1 plus | 2 minus
 
 
 class Task:
     def __init__(self, outputs):
         self.outputs = outputs          # stored objects (ids), <= NSLOT
         self.units = []
+        self.out_phase = [0] * len(outputs)   # a_s: the stored current is i^(-a_s) x the true one
+
+    def solve_phases(self, fixed_zero):
+        """Write every coefficient i^k (slot s, term m) as i^(a_s) (-1)^(n_sm) i^(b_m) with a_s, b_m in {0, 1}: the
+        term is rotated once (b_m), enters the accumulators with a SIGN only, and the phase a_s of a stored current
+        is absorbed by the dot products that read it.  fixed_zero: a_s = 0 (the current feeds vertices)."""
+        import itertools
+        ns = len(self.outputs)
+        rows = [(u, k) for u in self.units for k in range(3) if any(u.codes[k])]
+        choices = [tuple([0] * ns)] if fixed_zero else itertools.product((0, 1), repeat=ns)
+        for a in choices:
+            sol = {}
+            for u, k in rows:
+                bs = {((c & 1) ^ a[sl]) for sl, c in enumerate(u.codes[k]) if c}
+                if len(bs) > 1:
+                    break
+                sol[(id(u), k)] = bs.pop()
+            else:
+                self.out_phase = list(a)
+                for u, k in rows:
+                    b = sol[(id(u), k)]
+                    u.swap[k] = b
+                    for sl, c in enumerate(u.codes[k]):
+                        if c:
+                            n2 = ((c & 3) - a[sl] - b) % 4
+                            assert n2 in (0, 2)
+                            u.sign[k][sl] = 1 if n2 == 0 else 2       # 1: +, 2: -
+                return True
+        return False
 
 
 class Layout:
@@ -168,7 +199,7 @@ class Layout:
     def unit_key(m):
         return ("VVVV" if m.op.startswith("VVVV") else m.op, m.args)
 
-    def make_tasks(self, outputs):
+    def make_tasks(self, outputs, fixed_zero=False):
         """Tasks (<= NSLOT outputs each) for stored objects over ONE leg set with one propagator flag."""
         outputs = sorted(outputs, key=lambda o: o.id)
         keys = {o.id: {self.unit_key(m) for m, _ in self.members_of(o)} for o in outputs}
@@ -193,13 +224,20 @@ class Layout:
                     term = int(m.op[4]) - 1 if m.op.startswith("VVVV") else 0
                     assert units[k].codes[term][s] == 0
                     units[k].codes[term][s] = 4 + {1: 0, 1j: 1, -1: 2, -1j: 3}[coef]
-            tasks.append(t)
+            if t.solve_phases(fixed_zero):
+                tasks.append(t)
+            else:       # no common rotation: one current per task always works
+                assert len(grp) > 1
+                for o in grp:
+                    tasks += self.make_tasks([o], fixed_zero)
         return tasks
 
     def task_flops(self, t):
         o = t.outputs[0]
         kind = self.kind_of(o)
-        f = sum(FLOPS_UNIT[u.op] + FLOPS_ACC * sum(1 for term in u.codes for c in term if c) for u in t.units)
+        # every term visits accumulators 0, 1 (and 2, 3 of items with more than two currents)
+        nacc = 2 if len(t.outputs) <= 2 else 4
+        f = sum(FLOPS_UNIT[u.op] + FLOPS_ACC * nacc * sum(1 for term in u.codes if any(term)) for u in t.units)
         return f + FLOPS_FIN[kind] * len(t.outputs)
 
     def kind_of(self, o):
@@ -239,6 +277,8 @@ def emit_process(name, n_rounds=None):
     def massive_of(o):
         return 1 if (o.type[0] in "OI" and P.legs[[l for l in o.legs if P.legs[l].kind >= 2][0]].massive) else 0
 
+    out_phase = {}        # stored object id -> a: true current = i^a x stored current
+
     def add_stage(task_list, dots_round):
         """Items of the tasks, balanced over the warps by estimated cost (longest first), then interleaved so that
         warp w runs items w, w + W_EVENTS, ... of the stage."""
@@ -247,6 +287,8 @@ def emit_process(name, n_rounds=None):
         for t in task_list:
             o = t.outputs[0]
             nv = L.nv(o)
+            for x, a in zip(t.outputs, t.out_phase):
+                out_phase[x.id] = a
             n_tasks += 1
             n_units += len(t.units)
             cur_flops += L.task_flops(t) * nv
@@ -288,9 +330,9 @@ def emit_process(name, n_rounds=None):
                 vmaps.append(0)
             assert max(offs) < 65536
             ks = [sub_i(a.legs) for a in args[:2]]
-            code = lambda term: sum(c << (3 * sl) for sl, c in enumerate(u.codes[term]))
+            code = lambda term: u.swap[term] | (sum(c << (2 * sl) for sl, c in enumerate(u.sign[term])) << 1)
             members.append((u.op | (ks[0] << 8) | (ks[1] << 16), offs[0] | (offs[1] << 16), offs[2] | (vmaps[2] << 16),
-                            vmaps[0] | (vmaps[1] << 16), code(0) | (code(1) << 12), code(2), 0, 0))
+                            vmaps[0] | (vmaps[1] << 16), code(0) | (code(1) << 9) | (code(2) << 18), 0, 0, 0))
         outs = [L.off[x.id] for x in t.outputs] + [0] * NSLOT
         assert first < 65536 and len(t.units) < 256 and nv < 256
         w0 = len(t.units) | (len(t.outputs) << 8) | (L.kind_of(o) << 12) | (massive_of(o) << 15) | (nv << 16) | (vbase << 24)
@@ -300,7 +342,7 @@ def emit_process(name, n_rounds=None):
         tasks = []
         for o in L.base:
             if len(o.legs) == lev and o.op != "EXT":
-                tasks += L.make_tasks([o])
+                tasks += L.make_tasks([o], fixed_zero=True)
         add_stage(tasks, -1)
     for r in range(len(L.rounds)):
         cells = {}
@@ -389,10 +431,21 @@ def emit_process(name, n_rounds=None):
                 w("          const wf4 c%d = %s;" % (c, ldw(c)))
             for u in sorted({d[1] for d in dots}):
                 w("          { const wf4 u = %s;" % ldw(u))
+                by_c = {}
                 for (f, uu, c, z, kind) in dots:
-                    if uu == u:
-                        w("            dot_acc<%d, %s>(jr[%d], ji[%d], u, c%d);" % (zcode[z], "true" if kind == "V" else "false", f, f, c))
+                    if uu == u:     # the phases i^a of the stored operands go into the dot product's phase
+                        by_c.setdefault((c, kind), []).append((f, (zcode[z] + out_phase.get(u, 0) + out_phase.get(c, 0)) % 4))
+                for (c, kind), fl in sorted(by_c.items()):
+                    mink = "true" if kind == "V" else "false"
+                    if len(fl) == 1:
+                        w("            dot_acc<%d, %s>(jr[%d], ji[%d], u, c%d);" % (fl[0][1], mink, fl[0][0], fl[0][0], c))
                         amp_flops += FLOPS_DOT
+                    else:   # one contraction feeds several colour flows: computed once, added with each flow's phase
+                        w("            { const cplx t = dot_val<%s>(u, c%d);" % (mink, c))
+                        for f, zc in fl:
+                            w("              jadd<%d>(jr[%d], ji[%d], t);" % (zc, f, f))
+                        w("            }")
+                        amp_flops += FLOPS_DOT - 4 + 2 * len(fl)
                 w("          }")
             w("        }")
         w("      } break;")
