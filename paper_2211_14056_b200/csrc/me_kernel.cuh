@@ -52,7 +52,8 @@ template <class P> struct EventSmem {
   static constexpr int DOUBLES = ((RAW + 13) / 16) * 16 + 2;
 };
 
-constexpr int ME_W = 8;  // events = warps per CTA (gen/emit.py::W_EVENTS: the item tables are laid out for it)
+constexpr int ME_W = 8;  // events per CTA (gen/emit.py::W_EVENTS: the item tables are laid out for it); a CTA has P::N_WARPS >= ME_W
+                         // warps: all of them run items, the first ME_W own one event each in the dot stages
 
 // J parked in tensor memory: warp w owns lanes 32 (w % 4) .. +31 and the column block w / 4
 template <class P> struct JPark {
@@ -97,7 +98,7 @@ __device__ __forceinline__ double cta_me2(double* smem, double mass, double scal
   {
     const int t = threadIdx.x, ev = t % W;
     double* mom_s = smem + ev * STRIDE;
-    me_phase0(t / W, 32, mom_s + 4 * P::N_EXT, mom_s, P::N_EXT, P::N_SUB, d_masks, d_kind, d_massive, d_extoff, mass);
+    me_phase0(t / W, 4 * P::N_WARPS, mom_s + 4 * P::N_EXT, mom_s, P::N_EXT, P::N_SUB, d_masks, d_kind, d_massive, d_extoff, mass);
   }
   __syncthreads();
   double* base = smem + 4 * P::N_EXT;  // event e's scratch = base + e * STRIDE
@@ -107,28 +108,33 @@ __device__ __forceinline__ double cta_me2(double* smem, double mass, double scal
   double* sm_e = base + (lane % W) * STRIDE;   // items: lane = local variant j x event
   const int j = lane / W;
   int it = 0;
-  // ONE copy of the item interpreter and one of each round's dot products in the instruction stream
+  // ONE copy of the item interpreter and one of each round's dot products in the instruction stream.  Warp w runs
+  // items w, w + N_WARPS, ... of a stage: the generator balanced them by cost (a shared work counter was measured
+  // and lost 4 %, profiles/r2_me_eval_summary.md).
 #pragma unroll 1
   for (int p = 0; p < P::N_STAGES; ++p) {
     const int end = P::stage_end(p);
 #pragma unroll 1
-    for (int i = it + warp; i < end; i += W) me_run_item(c_items[i], c_members, j, sm_e, mass);
+    for (int i = it + warp; i < end; i += P::N_WARPS) me_run_item(c_items[i], c_members, j, sm_e, mass);
     it = end;
     __syncthreads();
     const int r = P::stage_dots(p);
     if (r >= 0) {
       // J is defined here on every path (zero in the first round, un-parked afterwards): dead during the items
-      if (r == 0) {
+      if (P::N_WARPS == W || warp < W) {   // helper warps (>= W), if any, only run items
+        if (r == 0) {
 #pragma unroll
-        for (int f = 0; f < P::N_FLOW; ++f) { jr[f] = 0.0; ji[f] = 0.0; }
-      } else if (JPark<P>::ON) {
-        JPark<P>::unpark(tmem, jr, ji);
+          for (int f = 0; f < P::N_FLOW; ++f) { jr[f] = 0.0; ji[f] = 0.0; }
+        } else if (JPark<P>::ON) {
+          JPark<P>::unpark(tmem, jr, ji);
+        }
+        if (lane < P::N_HEL_EVAL) P::dots(r, my, lane, jr, ji);
+        if (JPark<P>::ON && r + 1 < P::N_ROUNDS) JPark<P>::park(tmem, jr, ji);
       }
-      if (lane < P::N_HEL_EVAL) P::dots(r, my, lane, jr, ji);
-      if (JPark<P>::ON && r + 1 < P::N_ROUNDS) JPark<P>::park(tmem, jr, ji);
       if (r + 1 < P::N_ROUNDS) __syncthreads();   // the next round's items overwrite the round region
     }
   }
+  if (P::N_WARPS > W && warp >= W) return 0.0;
   double v = (lane < P::N_HEL_EVAL) ? P::colour(jr, ji) : 0.0;
   if (hel_out && lane < P::N_HEL_EVAL) {  // full index: leg 0 at +1 is bit 0; the parity partner has every helicity flipped
     const int hf = (lane << 1) | 1;
@@ -140,9 +146,9 @@ __device__ __forceinline__ double cta_me2(double* smem, double mass, double scal
   return 2.0 * v * scale;
 }
 
-// 8 events per CTA (blockDim.x = 256); persistent grid, batches of 8 consecutive events.
+// 8 events per CTA (blockDim.x = 32 P::N_WARPS); persistent grid, batches of 8 consecutive events.
 template <class P>
-__global__ void __launch_bounds__(32 * ME_W, 1) me_eval_kernel(const double* __restrict__ momenta, double* __restrict__ me2,
+__global__ void __launch_bounds__(32 * P::N_WARPS, 1) me_eval_kernel(const double* __restrict__ momenta, double* __restrict__ me2,
                                                               double* __restrict__ me2_hel, long long n_ev, double mass, double scale) {
   extern __shared__ __align__(16) double smem[];
   constexpr int STRIDE = EventSmem<P>::DOUBLES;
@@ -153,10 +159,10 @@ __global__ void __launch_bounds__(32 * ME_W, 1) me_eval_kernel(const double* __r
   for (long long b = blockIdx.x; b < n_batches; b += gridDim.x) {
     // events past the end repeat the last one (computed, not stored)
     const long long ev = min(b * W + warp, n_ev - 1);
-    if (lane < 4 * P::N_EXT) smem[warp * STRIDE + lane] = momenta[ev * (4 * P::N_EXT) + lane];
+    if ((P::N_WARPS == W || warp < W) && lane < 4 * P::N_EXT) smem[warp * STRIDE + lane] = momenta[ev * (4 * P::N_EXT) + lane];
     __syncthreads();
     const double r = cta_me2<P>(smem, mass, scale, (me2_hel && b * W + warp < n_ev) ? me2_hel + ev * P::N_HEL : nullptr, tmem);
-    if (lane == 0 && me2 && b * W + warp < n_ev) me2[ev] = r;
+    if ((P::N_WARPS == W || warp < W) && lane == 0 && me2 && b * W + warp < n_ev) me2[ev] = r;
     __syncthreads();
   }
   if (JPark<P>::ON) tmem_free<JPark<P>::COLS>(tmem);

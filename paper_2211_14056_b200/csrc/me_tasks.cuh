@@ -5,7 +5,8 @@
 // 62-64) taken to its limit.
 //
 // Scratch layout of one event (doubles), produced by gen/emit.py for each process:
-//   subset blocks  : 8 doubles per used leg subset S:  K_S[4], 1/K_S^2, 1/(K_S^2 - m_t^2), pad, pad
+//   subset blocks  : 8 doubles per used leg subset S:  K_S[4], the propagator denominator 1/(K_S^2 - m^2) of the currents
+//                    over S (m = m_t on the massive quark line, else 0; only where a propagated current exists), pads
 //   wavefunctions  : object o over the leg set S has one helicity variant per combination of the helicities of
 //                    ITS OWN legs ("helicity recycling").  Storage is in GROUPS of 4 lines x 128 B, one line per
 //                    component; o owns nv consecutive 16-byte slots of each line:
@@ -80,30 +81,33 @@ ME_HD vec4 ld_k(const double* p) {
 }
 
 // a5: subset momenta + denominators, external wavefunctions.  `mom` = this event's [n_ext][4] (E,px,py,pz),
-// physical momenta; legs 0,1 incoming.  sub_masks[s] = bitmask of legs of subset s (block s at sm + 8 s).
+// physical momenta; legs 0,1 incoming.  sub_masks[s] = bitmask of legs of subset s (block s at sm + 8 s) | flags << 16:
+// flag 1 = some propagated current lives on S (the denominator is needed), flag 2 = that line is massive.
 // Work items idx, idx + step, ... (subsets, then legs) of ONE event.
 ME_HD void me_phase0(int idx, int step, double* sm, const double* mom, int n_ext, int n_sub, const int* sub_masks,
                      const int* leg_kind, const int* leg_massive, const int* ext_off, double mass) {
+  // rolled: this runs once per event and must not crowd the instruction cache of the item and dot stages
+#if defined(__CUDA_ARCH__)
+#pragma unroll 1
+#endif
   for (int s = idx; s < n_sub; s += step) {
     const int m = sub_masks[s];
     double K[4] = {0.0, 0.0, 0.0, 0.0};
-    int cnt = 0;
     for (int l = 0; l < n_ext; ++l)
       if ((m >> l) & 1) {
         const double sg = (l < 2) ? 1.0 : -1.0;  // all-incoming convention
         for (int i = 0; i < 4; ++i) K[i] = fma(sg, mom[4 * l + i], K[i]);
-        ++cnt;
       }
     double* o = sm + 8 * s;
     for (int i = 0; i < 4; ++i) o[i] = K[i];
-    if (cnt > 1) {
+    if ((m >> 16) & 1) {
       const double k2 = fma(K[0], K[0], -fma(K[1], K[1], fma(K[2], K[2], K[3] * K[3])));
-      o[4] = 1.0 / k2;
-      o[5] = 1.0 / fma(-mass, mass, k2);
-    } else {
-      o[4] = 0.0; o[5] = 0.0;
+      o[4] = 1.0 / (((m >> 17) & 1) ? fma(-mass, mass, k2) : k2);
     }
   }
+#if defined(__CUDA_ARCH__)
+#pragma unroll 1
+#endif
   for (int l = idx; l < n_ext; l += step) {
     wf4 w[2];
     external_wavefunction(leg_kind[l], mom + 4 * l, leg_massive[l] ? mass : 0.0, w);
@@ -218,7 +222,7 @@ ME_HD void me_run_item(const MeItem H, const MeMember* __restrict__ members, int
       }
   } else {
     const bool massive = (H.w0 >> 15) & 1;
-    const double mm = massive ? mass : 0.0, f = massive ? ks[5] : ks[4];
+    const double mm = massive ? mass : 0.0, f = ks[4];
     const vec4 K = ld_k(ks);
     if (kind == KIND_ROW) {
       for (int s = 0; s < ME_NSLOT; ++s)

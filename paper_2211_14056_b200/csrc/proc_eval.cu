@@ -21,7 +21,7 @@ int geom(me_handle* h) {
   const int bytes = ME_W * EventSmem<P>::DOUBLES * 8;
   CU(cudaFuncSetAttribute(me_eval_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
   int ctas = 0;
-  CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas, me_eval_kernel<P>, 32 * ME_W, bytes));
+  CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas, me_eval_kernel<P>, 32 * P::N_WARPS, bytes));
   if (ctas < 1) return fail(ME_ECUDA, "me_eval kernel does not fit on an SM%s%s");
   // tensor memory: 512 columns per SM shared by the resident CTAs
   if (JPark<P>::ON && ctas * JPark<P>::COLS > 512) ctas = 512 / JPark<P>::COLS;
@@ -49,7 +49,7 @@ int fill(me_handle* h) {
 int eval(me_handle* h, const double* mom, double* me2, double* hel, long long n, cudaStream_t s) {
   const long long need = (n + ME_W - 1) / ME_W;
   const int grid = static_cast<int>(need < h->grid ? need : h->grid);
-  me_eval_kernel<P><<<grid, 32 * ME_W, h->smem_bytes, s>>>(mom, me2, hel, n, h->mass, h->scale);
+  me_eval_kernel<P><<<grid, 32 * P::N_WARPS, h->smem_bytes, s>>>(mom, me2, hel, n, h->mass, h->scale);
   CU(cudaGetLastError());
   return ME_OK;
 }

@@ -14,7 +14,7 @@ namespace MADME_CAT(tu_, MADME_PROC, _v) {
 using P = MADME_PROC;
 
 int integrand(me_handle* h, const VegasArgs& a, double* f, unsigned long long* idx, int words, cudaStream_t s) {
-  constexpr int W = ME_W;
+  constexpr int W = P::N_WARPS;   // threads per CTA = 32 W, each generates one event per batch
   CU(cudaFuncSetAttribute(vegas_integrand_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem_bytes));
   int per_sm = 0;
   CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, vegas_integrand_kernel<P>, 32 * W, h->smem_bytes));

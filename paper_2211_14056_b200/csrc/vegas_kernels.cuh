@@ -6,28 +6,28 @@
 
 namespace madme {
 
-// Fused integrand.  A CTA of W warps takes 32 W consecutive events: every thread generates one event (Philox -> Vegas
+// Fused integrand.  A CTA of NW warps takes 32 NW consecutive events: every thread generates one event (Philox -> Vegas
 // map -> RAMBO -> cuts).  The survivors are COMPACTED across the CTA (ballot + prefix sum) into a small per-CTA staging
 // area (final-state momenta, weight, event index: 32 W x (4 n_final + 2) doubles of global memory that never leaves
 // L2) so that the CTA then evaluates |M|^2 of exactly the surviving events, W at a time, whatever warp generated them;
 // cut events cost no matrix element.  Output per event: f (8 B) and the D bin indices packed one byte each
 // (n_bins <= 255) into idx_out[ev][ceil(D/8)].
 template <class P>
-__global__ void __launch_bounds__(32 * ME_W, 1) vegas_integrand_kernel(VegasArgs a, double* __restrict__ f_out,
+__global__ void __launch_bounds__(32 * P::N_WARPS, 1) vegas_integrand_kernel(VegasArgs a, double* __restrict__ f_out,
                                                                  unsigned long long* __restrict__ idx_out, int idx_words,
                                                                  double* __restrict__ stage_all) {
-  constexpr int NF = P::N_EXT - 2, W = ME_W;
+  constexpr int NF = P::N_EXT - 2, W = ME_W, NW = P::N_WARPS;
   constexpr int STRIDE = EventSmem<P>::DOUBLES;
   constexpr int SLOT = 4 * NF + 4;  // final momenta, weight, event index, beam energy, pad
   extern __shared__ __align__(16) double smem[];
-  __shared__ int warp_count[W];
+  __shared__ int warp_count[NW];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   double* mom_s = smem + warp * STRIDE;
-  double* stage = stage_all + static_cast<long long>(blockIdx.x) * (32 * W) * SLOT;
+  double* stage = stage_all + static_cast<long long>(blockIdx.x) * (32 * NW) * SLOT;
   const uint32_t tmem = JPark<P>::ON ? tmem_alloc<JPark<P>::COLS>() : 0u;
-  const long long n_batches = (a.n_ev + 32 * W - 1) / (32 * W);
+  const long long n_batches = (a.n_ev + 32 * NW - 1) / (32 * NW);
   for (long long b = blockIdx.x; b < n_batches; b += gridDim.x) {
-    const long long ev = (b * W + warp) * 32 + lane;
+    const long long ev = (b * NW + warp) * 32 + lane;
     const bool live = ev < a.n_ev;
     {
       double p[NF][4], y[VEGAS_MAX_DIM], x[VEGAS_MAX_DIM];
@@ -85,14 +85,16 @@ __global__ void __launch_bounds__(32 * ME_W, 1) vegas_integrand_kernel(VegasArgs
     }
     int n_pass = 0;
 #pragma unroll
-    for (int k = 0; k < W; ++k) n_pass += warp_count[k];
+    for (int k = 0; k < NW; ++k) n_pass += warp_count[k];
     __syncthreads();  // staging writes visible to the CTA
     for (int first = 0; first < n_pass; first += W) {
-      const bool valid = first + warp < n_pass;
+      const bool valid = (NW == W || warp < W) && first + warp < n_pass;   // warps >= W only help with the items
       const double* s = stage + (valid ? first + warp : 0) * SLOT;  // idle warps re-evaluate slot 0 (finite input, not stored)
       const double e_beam = s[4 * NF + 2];
-      if (lane < 8) mom_s[lane] = (lane == 0 || lane == 3 || lane == 4) ? e_beam : (lane == 7 ? -e_beam : 0.0);
-      else if (lane < 8 + 4 * NF) mom_s[lane] = s[lane - 8];
+      if (NW == W || warp < W) {
+        if (lane < 8) mom_s[lane] = (lane == 0 || lane == 3 || lane == 4) ? e_beam : (lane == 7 ? -e_beam : 0.0);
+        else if (lane < 8 + 4 * NF) mom_s[lane] = s[lane - 8];
+      }
       __syncthreads();
       const double r = cta_me2<P>(smem, a.mass, a.scale, nullptr, tmem);
       if (valid && lane == 0) f_out[__double_as_longlong(s[4 * NF + 1])] = s[4 * NF] * r;

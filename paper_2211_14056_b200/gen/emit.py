@@ -28,6 +28,8 @@ OUT_DIR = os.path.join(os.path.dirname(HERE), "csrc", "generated")
 NSLOT = 4            # accumulators (colour-ordered currents) per item
 W_EVENTS = 8         # events per CTA = warps per CTA
 VPI = 32 // W_EVENTS  # helicity variants per item (lanes = VPI variants x W_EVENTS events)
+N_WARPS = int(os.environ.get("MADME_GEN_WARPS", "8"))
+DYNAMIC = False      # True: items listed longest first for a shared work counter (measured, lost 4 %; the kernel uses the fixed map)   # warps per CTA: W_EVENTS own an event in the dot stages, all run items
 # shared-memory budget: doubles per event so that W_EVENTS events fit in the 227 KB a CTA can own
 SMEM_BUDGET_DOUBLES = int(os.environ.get("MADME_GEN_SMEM_DOUBLES", str((232448 // (8 * W_EVENTS)) - 32 - 16)))
 N_ROUNDS = int(os.environ.get("MADME_GEN_ROUNDS", "0"))   # 0: the fewest rounds that fit the budget
@@ -295,18 +297,22 @@ def emit_process(name, n_rounds=None):
             for vbase in range(0, nv, VPI):
                 pending.append((L.task_flops(t), t, vbase))
         pending.sort(key=lambda x: -x[0])
-        queues = [[0, []] for _ in range(W_EVENTS)]
-        for cost, t, vbase in pending:
-            q = min(queues, key=lambda x: x[0])
-            q[0] += cost
-            q[1].append((t, vbase))
-        depth = max(len(q[1]) for q in queues) if pending else 0
-        for k in range(depth):
-            for q in queues:
-                if k < len(q[1]):
-                    items.append(encode_item(*q[1][k]))
-                else:
-                    items.append((0, 0, 0, 0))
+        if DYNAMIC:     # handed out through a shared counter, longest first
+            for cost, t, vbase in pending:
+                items.append(encode_item(t, vbase))
+        else:
+            queues = [[0, []] for _ in range(N_WARPS)]
+            for cost, t, vbase in pending:
+                q = min(queues, key=lambda x: x[0])
+                q[0] += cost
+                q[1].append((t, vbase))
+            depth = max(len(q[1]) for q in queues) if pending else 0
+            for k in range(depth):
+                for q in queues:
+                    if k < len(q[1]):
+                        items.append(encode_item(*q[1][k]))
+                    else:
+                        items.append((0, 0, 0, 0))
         stage_end.append(len(items))
         stage_dots.append(dots_round)
 
@@ -386,7 +392,8 @@ def emit_process(name, n_rounds=None):
 
     w("  static constexpr int N_ITEMS = %d, N_MEMBERS = %d, N_ROUNDS = %d, N_STAGES = %d, N_TASKS = %d, N_UNITS = %d;"
       % (len(items), len(members), len(L.rounds), len(stage_end), n_tasks, n_units))
-    w("  // stage p: items up to stage_end(p) (warp w takes items w, w + %d, ...), barrier, then the dot products of round" % W_EVENTS)
+    w("  static constexpr int N_WARPS = %d;" % N_WARPS)
+    w("  // stage p: items up to stage_end(p) (warp w takes items w, w + %d, ...), barrier, then the dot products of round" % N_WARPS)
     w("  // stage_dots(p) (if >= 0), barrier")
     table_fn("stage_end", stage_end)
     table_fn("stage_dots", stage_dots)
@@ -398,7 +405,11 @@ def emit_process(name, n_rounds=None):
     for r8 in members:
         w("  {{%du,%du,%du,%du,%du,%du,%du,%du}}, \\" % r8)
     w("  {{0u,0u,0u,0u,0u,0u,0u,0u}} }")
-    w("#define %s_SUB_MASKS { %s }" % (name.upper(), ",".join(str(sum(1 << l for l in sub)) for sub in L.subsets)))
+    sub_flags = {sub: 0 for sub in L.subsets}     # 1: a propagated current lives on the subset, 2: on the massive line
+    for o in L.stored:
+        if o.op != "EXT" and o.prop:
+            sub_flags[o.legs] |= 1 | (2 * massive_of(o))
+    w("#define %s_SUB_MASKS { %s }" % (name.upper(), ",".join(str(sum(1 << l for l in sub) | (sub_flags[sub] << 16)) for sub in L.subsets)))
     w("#define %s_LEG_KIND { %s }" % (name.upper(), ",".join(str(leg.kind) for leg in P.legs)))
     w("#define %s_LEG_MASSIVE { %s }" % (name.upper(), ",".join("1" if leg.massive else "0" for leg in P.legs)))
     ext_off = [L.off[o.id] for o in L.objs if o.op == "EXT"]
