@@ -29,6 +29,7 @@ NSLOT = 4            # accumulators (colour-ordered currents) per item
 W_EVENTS = 8         # events per CTA = warps per CTA
 VPI = 32 // W_EVENTS  # helicity variants per item (lanes = VPI variants x W_EVENTS events)
 N_WARPS = int(os.environ.get("MADME_GEN_WARPS", "8"))
+DOTS_C_PER_U = N_WARPS > W_EVENTS
 DYNAMIC = False      # True: items listed longest first for a shared work counter (measured, lost 4 %; the kernel uses the fixed map)   # warps per CTA: W_EVENTS own an event in the dot stages, all run items
 # shared-memory budget: doubles per event so that W_EVENTS events fit in the 227 KB a CTA can own
 SMEM_BUDGET_DOUBLES = int(os.environ.get("MADME_GEN_SMEM_DOUBLES", str((232448 // (8 * W_EVENTS)) - 32 - 16)))
@@ -438,8 +439,9 @@ def emit_process(name, n_rounds=None):
         for legs in split_list:
             dots = by_split[legs]
             w("        {  // split %s | rest: %d dot products" % ("".join(str(l) for l in legs), len(dots)))
-            for c in sorted({d[2] for d in dots}):
-                w("          const wf4 c%d = %s;" % (c, ldw(c)))
+            if not DOTS_C_PER_U:
+                for c in sorted({d[2] for d in dots}):
+                    w("          const wf4 c%d = %s;" % (c, ldw(c)))
             for u in sorted({d[1] for d in dots}):
                 w("          { const wf4 u = %s;" % ldw(u))
                 by_c = {}
@@ -448,6 +450,8 @@ def emit_process(name, n_rounds=None):
                         by_c.setdefault((c, kind), []).append((f, (zcode[z] + out_phase.get(u, 0) + out_phase.get(c, 0)) % 4))
                 for (c, kind), fl in sorted(by_c.items()):
                     mink = "true" if kind == "V" else "false"
+                    if DOTS_C_PER_U:     # one C operand live at a time (register budget of CTAs with helper warps)
+                        w("            { const wf4 c%d = %s;" % (c, ldw(c)))
                     if len(fl) == 1:
                         w("            dot_acc<%d, %s>(jr[%d], ji[%d], u, c%d);" % (fl[0][1], mink, fl[0][0], fl[0][0], c))
                         amp_flops += FLOPS_DOT
@@ -457,6 +461,8 @@ def emit_process(name, n_rounds=None):
                             w("              jadd<%d>(jr[%d], ji[%d], t);" % (zc, f, f))
                         w("            }")
                         amp_flops += FLOPS_DOT - 4 + 2 * len(fl)
+                    if DOTS_C_PER_U:
+                        w("            }")
                 w("          }")
             w("        }")
         w("      } break;")
