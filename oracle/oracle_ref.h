@@ -17,6 +17,11 @@
  *   - the Vegas grid-update details (alpha = 1.5, 3-point smoothing): a READING,
  *     pinned only by closed-form integrals and fixed-point/quantile properties.
  *   - sigma(gg -> ttbar gg): "parity unpinned" against the outside world (no published value).
+ * vegas_integrand_ref (flux 1/(2 s_hat), W_ps, jac, the pb conversion, Theta) and vegas_iterate_ref (I, sigma^2,
+ * refinement, iteration counter) ARE pinned since round 2: the total cross section sigma(gg -> t tbar) at
+ * sqrt(s_hat) = 1 TeV from vegas_iterate_ref against the 1-D quadrature of the pinned closed form x beta/(16 pi) x
+ * 1/(2 s_hat) (and the textbook total cross section as a check of the quadrature), and the iteration's I, sigma^2 and
+ * refined grid recomputed by hand from its per-event f (tests/test_oracle_vegas.py).
  */
 #ifndef ORACLE_REF_H
 #define ORACLE_REF_H

@@ -84,8 +84,9 @@ CASES = [((0.0, 0.0), 100.0), ((173.0, 173.0), 1000.0), ((173.0, 173.0, 0.0), 10
 @pytest.mark.parametrize("ps_mode", [0, 1])
 @pytest.mark.parametrize("masses,sqrt_s", CASES)
 def test_rambo_conservation_and_mass_shell(masses, sqrt_s, ps_mode):
-    """SURVEY §8(c) G1 pins: sum p = (sqrt_s,0,0,0), p_i^2 = m_i^2 (1e-12 s typical; 1e-9 s worst case of the
-    ill-conditioned near-parallel configurations of classic RAMBO), incoming legs (sqrt_s/2)(1,0,0,+-1)."""
+    """SURVEY §8(c) G1 pins: sum p = (sqrt_s,0,0,0), p_i^2 = m_i^2 to 1e-12 s on EVERY event (the cancellation-free
+    boost of DESIGN.md R-G1b; the textbook form reached only 1e-9 on near-parallel pairs), incoming legs
+    (sqrt_s/2)(1,0,0,+-1)."""
     n = len(masses)
     if ps_mode == 1 and n < 3:
         pytest.skip("diet RAMBO needs n >= 3 here")
@@ -95,13 +96,41 @@ def test_rambo_conservation_and_mass_shell(masses, sqrt_s, ps_mode):
     tot = mom[:, 2:].sum(1)
     tot[:, 0] -= sqrt_s
     dev = np.abs(tot).max(1) / sqrt_s
-    assert np.median(dev) < 1e-14 and dev.max() < 1e-9
+    assert np.median(dev) < 1e-14 and dev.max() < 1e-12
     m2 = mdot(mom[:, 2:], mom[:, 2:])
     devm = np.abs(m2 - np.array(masses) ** 2).max(1) / sqrt_s ** 2
-    assert np.median(devm) < 1e-14 and devm.max() < 1e-9
+    assert np.median(devm) < 1e-14 and devm.max() < 1e-12
     assert np.all(mom[:, 2:, 0] > 0) and np.all(w > 0)
     assert np.array_equal(mom[:, 0], np.tile([sqrt_s / 2, 0, 0, sqrt_s / 2], (20000, 1)))
     assert np.array_equal(mom[:, 1], np.tile([sqrt_s / 2, 0, 0, -sqrt_s / 2], (20000, 1)))
+
+
+def test_rambo_classic_equals_textbook_boost_at_generic_points():
+    """DESIGN.md R-G1b rewrote the conformal boost of classic RAMBO in a cancellation-free form; this compares it with
+    SURVEY §8(c) G1 written out literally (numpy): q_i from (c, phi, -ln(r3 r4)), Q = sum q, M = sqrt(Q^2), b = -Q/M,
+    gamma = Q0/M, a = 1/(1+gamma), x = sqrt(s)/M, p0 = x (gamma q0 + b.q), p = x (q + b q0 + a (b.q) b).  At generic
+    points (M not tiny against Q0) the two agree to rounding."""
+    for n in (2, 3, 4, 6):
+        u = ref.philox_uniform(77, 0, 0, 4 * n, 4000)
+        rs = 1000.0
+        mom, _ = ref.rambo_generate(u, rs, [0.0] * n, 0)
+        r = u.reshape(-1, n, 4)
+        c, phi, q0 = 2 * r[..., 0] - 1, 2 * math.pi * r[..., 1], -np.log(r[..., 2] * r[..., 3])
+        st = np.sqrt(1 - c * c)
+        q = np.stack([q0, q0 * st * np.cos(phi), q0 * st * np.sin(phi), q0 * c], -1)
+        Q = q.sum(1)
+        M = np.sqrt(Q[:, 0] ** 2 - (Q[:, 1:] ** 2).sum(1))
+        b = -Q[:, 1:] / M[:, None]
+        gam = Q[:, 0] / M
+        a = 1 / (1 + gam)
+        x = rs / M
+        bq = (b[:, None, :] * q[..., 1:]).sum(-1)
+        p0 = x[:, None] * (gam[:, None] * q[..., 0] + bq)
+        pv = x[:, None, None] * (q[..., 1:] + b[:, None, :] * q[..., 0:1] + (a[:, None] * bq)[..., None] * b[:, None, :])
+        want = np.concatenate([p0[..., None], pv], -1)
+        generic = M / Q[:, 0] > 0.2          # the textbook form itself loses digits when Q is nearly light-like
+        assert generic.sum() > 2000
+        assert np.max(np.abs(mom[generic, 2:] - want[generic])) < 1e-12 * rs
 
 
 def test_rambo_massless_weight_closed_form():

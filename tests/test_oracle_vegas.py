@@ -135,3 +135,75 @@ def test_hadronic_mode_factorises_into_pinned_pieces():
     nz = want != 0
     assert np.max(np.abs(f[nz] / want[nz] - 1)) < 1e-12
     assert abs(sums[0] / f.sum() - 1) < 1e-12 and sums[2] == nz.sum()
+
+
+# ---- the physics integrand and the iteration driver ------------------------------
+def _sigma_gg_ttx_quadrature(sqrt_s, m, alpha_s, n_nodes=96):
+    """sigma(gg -> t tbar) at fixed sqrt(s_hat) from pieces pinned elsewhere: the closed-form |M|^2 of config 1
+    (tests/helpers.py, pinned against the definition tier in test_oracle_me.py) integrated over the two-body phase
+    space d Phi_2 = beta/(16 pi) d cos(theta) (total beta/(8 pi): test_rambo_two_body_massive_weight) times the
+    flux 1/(2 s_hat) and the conversion 0.3893793721e9 pb GeV^2."""
+    from tests.helpers import closed_form_gg_ttx
+    s = sqrt_s * sqrt_s
+    beta = math.sqrt(1 - 4 * m * m / s)
+    c, wq = np.polynomial.legendre.leggauss(n_nodes)
+    e, p = sqrt_s / 2, beta * sqrt_s / 2
+    st = np.sqrt(1 - c * c)
+    mom = np.zeros((n_nodes, 4, 4))
+    mom[:, 0] = [e, 0, 0, e]
+    mom[:, 1] = [e, 0, 0, -e]
+    mom[:, 2, 0], mom[:, 2, 1], mom[:, 2, 3] = e, p * st, p * c
+    mom[:, 3, 0], mom[:, 3, 1], mom[:, 3, 3] = e, -p * st, -p * c
+    integral = (wq * closed_form_gg_ttx(mom, alpha_s, m)).sum()
+    return 0.3893793721e9 / (2 * s) * beta / (16 * math.pi) * integral
+
+
+def test_total_cross_section_gg_ttx_pins_the_integrand_normalisation():
+    """Pins flux 1/(2 s_hat), W_ps, jac, the conversion constant and |M|^2 TOGETHER through vegas_iterate_ref itself
+    (VERDICT r1 'parity unpinned' item): sigma(gg -> t tbar, sqrt(s_hat) = 1 TeV, no cuts) from three oracle Vegas
+    iterations (classic RAMBO, D = 8) against the 1-D quadrature above; the textbook total cross section
+    pi alpha_s^2/(3 s)[(1 + rho + rho^2/16) ln((1+beta)/(1-beta)) - beta (7/4 + 31 rho/16)] is a second, independent
+    check of the quadrature (it is verified here, not trusted)."""
+    from paper_2211_14056_b200.workloads import PARAMS
+    rs, m, a_s = 1000.0, PARAMS["m_top"], PARAMS["alpha_s"]
+    quad = _sigma_gg_ttx_quadrature(rs, m, a_s)
+    assert abs(_sigma_gg_ttx_quadrature(rs, m, a_s, 48) / quad - 1) < 1e-12      # the quadrature has converged
+    s = rs * rs
+    rho, beta = 4 * m * m / s, math.sqrt(1 - 4 * m * m / s)
+    book = math.pi * a_s ** 2 / (3 * s) * ((1 + rho + rho ** 2 / 16) * math.log((1 + beta) / (1 - beta))
+                                           - beta * (7 / 4 + 31 * rho / 16)) * 0.3893793721e9
+    assert abs(book / quad - 1) < 1e-10
+    me = ref.MatrixElementRef("gg_ttx")
+    g = ref.GridRef(8, 50, 1.5, seed=11, ps_mode=0)
+    res = [me.vegas_iterate(g, rs, 150000) for _ in range(3)]
+    I = np.array([r["integral"] for r in res])
+    var = np.array([r["variance"] for r in res])
+    for Ij, vj in zip(I, var):      # every iteration is an unbiased estimate
+        assert abs(Ij - quad) < 4.5 * math.sqrt(vj)
+    comb, sig = (I / var).sum() / (1 / var).sum(), (1 / var).sum() ** -0.5
+    assert sig / comb < 3e-3 and abs(comb - quad) < 4 * sig
+    assert all(r["n_pass"] == 150000 for r in res)      # no cuts: every event contributes
+    # a wrong flux (1/(2 sqrt(s)), 1/s, 1/(4 s)), a dropped 2 pi or a missing conversion would be off by >= 2x
+    assert abs(comb / quad - 1) < 0.01
+
+
+def test_vegas_iterate_ref_by_hand():
+    """vegas_iterate_ref itself: I = (1/N) sum f, sigma^2 = [(1/N) sum f^2 - I^2]/(N-1)
+    recomputed by hand from the per-event f of the same iteration (vegas_integrand_ref, pinned above), the grid
+    refined with exactly the accumulated S_{d,i}, the iteration counter advanced (so the next call draws new points)."""
+    me = ref.MatrixElementRef("gg_ttx")
+    for n in (2, 7, 1000):
+        g = ref.GridRef(8, 50, 1.5, seed=5, ps_mode=0)
+        g2 = ref.GridRef(8, 50, 1.5, seed=5, ps_mode=0)
+        sums, f = me.vegas_integrand(g2, 1000.0, 0, n, want_f=True)
+        r = me.vegas_iterate(g, 1000.0, n)
+        I = math.fsum(f) / n
+        var = (math.fsum(f * f) / n - I * I) / (n - 1)
+        assert abs(r["integral"] / I - 1) < 1e-14 and abs(r["variance"] / var - 1) < 1e-10 * max(1, I * I / (var * n))
+        assert abs(r["sum_w"] / math.fsum(f) - 1) < 1e-14 and abs(r["sum_w2"] / math.fsum(f * f) - 1) < 1e-14
+        assert r["n_pass"] == n and g.iteration == 1 and g2.iteration == 0
+        want_edges = ref.vegas_refine(g2.edges, sums[3:].reshape(8, 50), 1.5)
+        assert np.array_equal(g.edges, want_edges)
+        # the second iteration uses the refined grid and a new random stream
+        r2 = me.vegas_iterate(g, 1000.0, n)
+        assert g.iteration == 2 and r2["integral"] != r["integral"]
