@@ -13,7 +13,11 @@
  *   - "dev" pointers are device (HBM) pointers, 16-byte aligned; "host" pointers are host memory.
  *     The caller owns every data buffer and keeps it alive until the stream work completed.
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All calls are
- *     asynchronous on `stream`, except vegas_iterate, which synchronises once to return its scalars.
+ *     asynchronous on `stream`, except vegas_iterate / vegas_finish, which synchronise once to return their scalars.
+ *   - a handle belongs to the device that was current in me_init (calls switch to it and back) and owns scratch
+ *     that its vegas_* calls share: use one handle from ONE stream at a time (one handle per stream otherwise).
+ *   - allocation: me_init and me_reserve allocate; no other call allocates, frees or synchronises behind the
+ *     caller's back (vegas_integrand beyond the reserved size fails with ME_EINVAL).
  *   - units: GeV.  Momenta are (E, px, py, pz), metric (+,-,-,-); legs 0,1 are the incoming partons
  *     along +z / -z, legs 2.. the final state in the order of the process name.
  *   - fp64 throughout (BASELINE.json:metric), Philox words are uint32.
@@ -63,14 +67,21 @@ typedef struct {
 
 /* me_init — select the generated kernel of `process` and fix its parameters.
  * process: "epem_mupmum" (e+ e- -> mu- mu+), "gg_ttx", "gg_ttxg", "gg_ttxgg" (BASELINE.json:configs[0-3]).
- * Allocates the handle and a small device scratch (reduction partials) — no per-call allocation later. */
+ * Allocates the handle and the fixed-size device scratch of the Vegas path (reduction partials, the survivor staging
+ * of the fused integrand: about 25 MB, independent of the event count). */
 int me_init(const char* process, const me_params* params, me_handle** out);
 void me_free(me_handle* h);
+/* me_reserve — size the per-event scratch of vegas_integrand / vegas_iterate / vegas_unweight (the integrand values
+ * and their packed bin indices, 32 bytes per event, plus 8 bytes per 256 events) for calls of up to max_events
+ * events.  Grows only (a smaller request is a no-op); synchronises the device when it has to replace a buffer. */
+int me_reserve(me_handle* h, long long max_events);
 int me_n_external(const me_handle* h);
 int me_n_final(const me_handle* h);
 /* what: 0 Feynman diagrams, 1 colour-pure amplitude terms, 2 diagrams with a 4-gluon vertex, 3 colour flows,
  * 4 helicity combinations, 5 off-shell currents, 6 shared-memory bytes per event, 7 events (warps) per CTA,
- * 8 registers per thread of the me_eval kernel, 9 resident CTAs per SM, 10 SM count. */
+ * 8 registers per thread of the me_eval kernel, 9 resident CTAs per SM, 10 SM count, 11 events reserved by
+ * me_reserve, 12 the handle's device ordinal, 13 address of the per-event scratch (to check that calls do not
+ * reallocate). */
 long long me_info(const me_handle* h, int what);
 /* nominal fp64 flops per event of the emitted program (real add or mul = 1, FMA = 2) */
 double me_flops_per_event(const me_handle* h);
@@ -117,6 +128,32 @@ int vegas_integrand(me_handle* h, const vegas_grid* g, double sqrt_s, long long 
 /* vegas_iterate — one full iteration over events [0, n_ev): integrand, result, grid refinement in place
  * (all on the device), ++g->iteration.  result: HOST.  Synchronises `stream` once. */
 int vegas_iterate(me_handle* h, vegas_grid* g, double sqrt_s, long long n_ev, vegas_result* result, void* stream);
+
+/* vegas_combine — the one exchange of a sharded iteration: sums[j] = parts[0][j] + parts[1][j] + ...
+ * in that FIXED order (reproducible whatever the arrival order).  parts: dev [n_parts][n_out], sums: dev [n_out]. */
+int vegas_combine(const double* parts, int n_parts, int n_out, double* sums, void* stream);
+/* vegas_finish — step 3 of SURVEY.md 8(c) G7 from the accumulated sums of n_total events:
+ * I = sums[0]/N, sigma^2 = [sums[1]/N - I^2]/(N-1), n_pass = sums[2].  sums: dev [>= 3]; result: HOST.
+ * Synchronises `stream` once. */
+int vegas_finish(const double* sums, long long n_total, vegas_result* result, void* stream);
+
+/* Unweighted events — the step behind the path.
+ * vegas_max_weight: *w_max (dev [1]) = max_e f[e] over f dev [n_ev].
+ * vegas_unweight: hit-or-miss on the weights f (dev [n_ev]) of events [first_event, first_event + n_ev) of iteration
+ * `iteration`: event e is kept iff f > 0 and u_e w_max < f, u_e = the Philox uniform of counter (event lo, event hi,
+ * 0x7fffffff, iteration), words 0-1 — a counter word no phase-space dimension uses, so the decision is independent
+ * of the event's kinematics and reproducible under any sharding.  accepted: dev int64 [n_ev] receives the GLOBAL
+ * indices of the kept events in ascending order; counts: dev int64 [2] = (number kept, number with f > w_max, which
+ * are always kept and signal that w_max was too small). */
+int vegas_max_weight(const double* f, long long n_ev, double* w_max, void* stream);
+int vegas_unweight(me_handle* h, const double* f, long long n_ev, double w_max, uint64_t seed, uint64_t iteration,
+                   long long first_event, long long* accepted, long long* counts, void* stream);
+/* vegas_generate — the kinematics of LISTED events of iteration g->iteration on grid g (the grid the weights were
+ * computed with, i.e. before its refinement): Philox -> Vegas map -> RAMBO for event_ids dev int64 [n].
+ * momenta: dev [n][n_ext][4] (partonic centre-of-mass frame); weights: dev [n] = jac W_ps C/(2 s_hat) (times the
+ * toy densities in ps_mode 2): the event weight without |M|^2 and cuts. */
+int vegas_generate(me_handle* h, const vegas_grid* g, double sqrt_s, const long long* event_ids, long long n,
+                   double* momenta, double* weights, void* stream);
 
 /* fp64_peak_probe — a register-resident DFMA chain on every SM (8 independent accumulators per thread):
  * runs n_iter x 8 x 256 DFMA per thread on `stream`; returns the thread-DFMA count in *n_dfma (host).

@@ -234,4 +234,62 @@ int vegas_iterate_ref(me_handle_ref* h, vegas_grid_ref* g, double sqrt_s, long l
   return 0;
 }
 
+// Unweighted events ("the step behind the path").  Hit-or-miss: event e of the iteration is kept iff
+// f_e > 0 and u_e w_max < f_e, with u_e the Philox uniform of counter (event lo, event hi, 0x7fffffff, iteration),
+// words 0-1 — a pair index no phase-space dimension reaches (D <= 24 uses pair indices 0..11), so the decision is
+// independent of the kinematics.  accepted: global indices in ascending order; counts = (kept, f > w_max).
+int vegas_unweight_ref(const double* f, long long n_ev, double w_max, uint64_t seed, uint64_t iteration, long long first_event,
+                       long long* accepted, long long* counts) {
+  if (!counts || n_ev < 0 || !(w_max > 0) || (n_ev > 0 && (!f || !accepted))) return -1;
+  counts[0] = counts[1] = 0;
+  const uint32_t key[2] = {uint32_t(seed), uint32_t(seed >> 32)};
+  for (long long e = 0; e < n_ev; ++e) {
+    if (f[e] > w_max) counts[1] += 1;
+    if (!(f[e] > 0)) continue;
+    const uint64_t ev = uint64_t(first_event + e);
+    const uint32_t ctr[4] = {uint32_t(ev), uint32_t(ev >> 32), 0x7fffffffu, uint32_t(iteration)};
+    uint32_t o[4];
+    philox4x32_10(ctr, key, o);
+    const uint64_t bits = (uint64_t(o[0]) << 32 | o[1]) >> 11;
+    const double u = (double(bits) + 0.5) * (1.0 / 9007199254740992.0);
+    if (u * w_max < f[e]) accepted[counts[0]++] = first_event + e;
+  }
+  return 0;
+}
+
+// The kinematics of listed events of iteration g->iteration on grid g: momenta [n][n_ext][4] (partonic centre-of-mass
+// frame, incoming legs filled in) and weights jac W_ps C/(2 s_hat) (times the toy densities in ps_mode 2) — the
+// integrand of vegas_integrand_ref without |M|^2 and without the cuts.
+int vegas_generate_ref(me_handle_ref* h, const vegas_grid_ref* g, double sqrt_s, const long long* ids, long long n, double* momenta,
+                       double* weights) {
+  if (!h || !g || n < 0 || (n > 0 && (!ids || !momenta || !weights)) || h->P.qed) return -1;
+  const int nf = h->P.n_ext - 2, D = g->n_dim, nb = g->n_bins;
+  if (D != (g->ps_mode == 0 ? 4 * nf : g->ps_mode == 1 ? 3 * nf - 4 : 3 * nf - 2)) return -4;
+  std::vector<double> masses(nf);
+  double msum = 0;
+  for (int i = 0; i < nf; ++i) { masses[i] = h->P.mass[2 + i]; msum += masses[i]; }
+  const double conv = 0.3893793721e9;
+  std::vector<int> idx(D);
+  for (long long k = 0; k < n; ++k) {
+    double y[4 * NMAX_FINAL], x[4 * NMAX_FINAL];
+    double* mom = momenta + k * 4 * (nf + 2);
+    philox_uniforms(g->seed, uint64_t(g->iteration), uint64_t(ids[k]), D, y);
+    const double jac = vegas_map_point(g->edges, D, nb, y, x, idx.data());
+    if (g->ps_mode == 2) {
+      const double rs_hat = std::sqrt(x[0] * x[1]) * sqrt_s;
+      if (rs_hat > msum) {
+        weights[k] = jac * toy_gluon_density(x[0]) * toy_gluon_density(x[1]) * rambo_event(x + 2, rs_hat, masses.data(), nf, 1, mom) /
+                     (2.0 * rs_hat * rs_hat) * conv;
+      } else {
+        weights[k] = 0;
+        for (int i = 0; i < 4 * (nf + 2); ++i) mom[i] = 0;
+        mom[0] = mom[3] = mom[4] = 0.5 * rs_hat; mom[7] = -0.5 * rs_hat;
+      }
+    } else {
+      weights[k] = jac * rambo_event(x, sqrt_s, masses.data(), nf, g->ps_mode, mom) / (2.0 * sqrt_s * sqrt_s) * conv;
+    }
+  }
+  return 0;
+}
+
 }  // extern "C"

@@ -93,6 +93,12 @@ int vegas_integrand_ref(me_handle_ref* h, const vegas_grid_ref* g, double sqrt_s
 /* one full iteration on events [0, n_ev): integrand, result, refine g->edges in place, ++g->iteration */
 int vegas_iterate_ref(me_handle_ref* h, vegas_grid_ref* g, double sqrt_s, long long n_ev, vegas_result_ref* result);
 
+/* unweighted events: hit-or-miss on f with a dedicated Philox counter word; kinematics of listed events */
+int vegas_unweight_ref(const double* f, long long n_ev, double w_max, uint64_t seed, uint64_t iteration, long long first_event,
+                       long long* accepted, long long* counts);
+int vegas_generate_ref(me_handle_ref* h, const vegas_grid_ref* g, double sqrt_s, const long long* ids, long long n, double* momenta,
+                       double* weights);
+
 #ifdef __cplusplus
 }
 #endif

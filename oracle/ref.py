@@ -62,6 +62,10 @@ def lib():
                                              C.c_void_p, C.c_void_p]
         _lib.vegas_iterate_ref.argtypes = [C.c_void_p, C.POINTER(VegasGrid), C.c_double, C.c_longlong,
                                            C.POINTER(VegasResult)]
+        _lib.vegas_unweight_ref.argtypes = [C.c_void_p, C.c_longlong, C.c_double, C.c_uint64, C.c_uint64, C.c_longlong,
+                                            C.c_void_p, C.c_void_p]
+        _lib.vegas_generate_ref.argtypes = [C.c_void_p, C.POINTER(VegasGrid), C.c_double, C.c_void_p, C.c_longlong,
+                                            C.c_void_p, C.c_void_p]
         _lib.oracle_set_threads_ref.argtypes = [C.c_int]
         _lib.oracle_set_threads_ref.restype = None
     return _lib
@@ -171,11 +175,28 @@ class MatrixElementRef:
         assert rc == 0, rc
         return (sums, f) if want_f else sums
 
+    def vegas_generate(self, grid, sqrt_s, ids):
+        ids = np.ascontiguousarray(ids, dtype=np.int64)
+        mom = np.empty((len(ids), lib().me_n_external_ref(self._h), 4))
+        w = np.empty(len(ids))
+        rc = lib().vegas_generate_ref(self._h, C.byref(grid.c), sqrt_s, _p(ids), len(ids), _p(mom), _p(w))
+        assert rc == 0, rc
+        return mom, w
+
     def vegas_iterate(self, grid, sqrt_s, n_ev):
         res = VegasResult()
         rc = lib().vegas_iterate_ref(self._h, C.byref(grid.c), sqrt_s, n_ev, C.byref(res))
         assert rc == 0, rc
         return dict(integral=res.integral, variance=res.variance, sum_w=res.sum_w, sum_w2=res.sum_w2, n_pass=res.n_pass)
+
+
+def vegas_unweight(f, w_max, seed, iteration, first_event=0):
+    """Hit-or-miss: returns (accepted global event indices, ascending; number of f > w_max)."""
+    f = _f64(f)
+    acc = np.empty(len(f), dtype=np.int64)
+    counts = np.zeros(2, dtype=np.int64)
+    assert lib().vegas_unweight_ref(_p(f), len(f), float(w_max), seed, iteration, first_event, _p(acc), _p(counts)) == 0
+    return acc[:counts[0]].copy(), int(counts[1])
 
 
 class GridRef:

@@ -39,9 +39,10 @@ class VegasResultC(C.Structure):
 
 
 # every symbol include/madme.h declares (tests check that the library exports exactly these)
-SYMBOLS = ["me_init", "me_free", "me_n_external", "me_n_final", "me_info", "me_flops_per_event", "me_eval",
+SYMBOLS = ["me_init", "me_free", "me_reserve", "me_n_external", "me_n_final", "me_info", "me_flops_per_event", "me_eval",
            "me_eval_helicities", "philox_uniform", "rambo_generate", "apply_cuts", "vegas_map", "vegas_refine",
-           "vegas_integrand", "vegas_iterate", "fp64_peak_probe", "me_last_error"]
+           "vegas_integrand", "vegas_iterate", "vegas_combine", "vegas_finish", "vegas_max_weight", "vegas_unweight",
+           "vegas_generate", "fp64_peak_probe", "me_last_error"]
 
 
 def lib():
@@ -57,6 +58,7 @@ def lib():
     L.me_init.argtypes = [C.c_char_p, C.POINTER(MeParams), C.POINTER(vp)]
     L.me_free.argtypes = [vp]
     L.me_free.restype = None
+    L.me_reserve.argtypes = [vp, ll]
     L.me_n_external.argtypes = [vp]
     L.me_n_final.argtypes = [vp]
     L.me_info.argtypes = [vp, i32]
@@ -72,6 +74,11 @@ def lib():
     L.vegas_refine.argtypes = [vp, i32, i32, vp, dbl, vp]
     L.vegas_integrand.argtypes = [vp, C.POINTER(VegasGridC), dbl, ll, ll, vp, vp, vp]
     L.vegas_iterate.argtypes = [vp, C.POINTER(VegasGridC), dbl, ll, C.POINTER(VegasResultC), vp]
+    L.vegas_combine.argtypes = [vp, i32, i32, vp, vp]
+    L.vegas_finish.argtypes = [vp, ll, C.POINTER(VegasResultC), vp]
+    L.vegas_max_weight.argtypes = [vp, ll, vp, vp]
+    L.vegas_unweight.argtypes = [vp, vp, ll, dbl, u64, u64, ll, vp, vp, vp]
+    L.vegas_generate.argtypes = [vp, C.POINTER(VegasGridC), dbl, vp, ll, vp, vp, vp]
     L.fp64_peak_probe.argtypes = [ll, vp, C.POINTER(dbl), vp]
     L.me_last_error.restype = C.c_char_p
     _lib = L
@@ -119,6 +126,18 @@ def me_init(process, params):
 
 def me_free(h):
     h.__del__()
+
+
+def me_reserve(h, max_events):
+    """Size the handle's per-event Vegas scratch (32 B/event) for calls of up to max_events events.  The C calls
+    never allocate; this binding's vegas_* functions call me_reserve for you when they see a larger batch than
+    reserved — call it yourself to decide when that allocation happens."""
+    _check(lib().me_reserve(h.ptr, int(max_events)))
+
+
+def _reserved(h, n_ev):
+    if n_ev > int(lib().me_info(h.ptr, 11)):
+        me_reserve(h, n_ev)
 
 
 def me_info(h, what):
@@ -220,6 +239,7 @@ def vegas_integrand(h, grid, sqrt_s, first_event, n_ev, want_f=False, stream=Non
     n_out = 3 + grid.c.n_dim * grid.c.n_bins
     sums = torch.empty(n_out, dtype=torch.float64, device=grid.edges.device)
     f = torch.empty(n_ev, dtype=torch.float64, device=grid.edges.device) if want_f else None
+    _reserved(h, n_ev)
     _check(lib().vegas_integrand(h.ptr, C.byref(grid.c), float(sqrt_s), first_event, n_ev, _dev(sums, torch.float64, "sums"),
                                  _dev(f, torch.float64, "f") if want_f else None, _stream(stream)))
     return sums, f
@@ -227,8 +247,57 @@ def vegas_integrand(h, grid, sqrt_s, first_event, n_ev, want_f=False, stream=Non
 
 def vegas_iterate(h, grid, sqrt_s, n_ev, stream=None):
     r = VegasResultC()
+    _reserved(h, n_ev)
     _check(lib().vegas_iterate(h.ptr, C.byref(grid.c), float(sqrt_s), n_ev, C.byref(r), _stream(stream)))
+    return _result(r)
+
+
+def _result(r):
     return dict(integral=r.integral, variance=r.variance, sum_w=r.sum_w, sum_w2=r.sum_w2, n_pass=r.n_pass)
+
+
+def vegas_combine(parts, stream=None):
+    """parts: cuda f64 [n_parts, n_out] -> their sum in fixed order, cuda f64 [n_out]."""
+    n_parts, n_out = parts.shape
+    sums = torch.empty(n_out, dtype=torch.float64, device=parts.device)
+    _check(lib().vegas_combine(_dev(parts, torch.float64, "parts"), n_parts, n_out, _dev(sums, torch.float64, "sums"), _stream(stream)))
+    return sums
+
+
+def vegas_finish(sums, n_total, stream=None):
+    r = VegasResultC()
+    _check(lib().vegas_finish(_dev(sums, torch.float64, "sums"), int(n_total), C.byref(r), _stream(stream)))
+    return _result(r)
+
+
+def vegas_max_weight(f, stream=None):
+    """f: cuda f64 [n_ev] -> cuda f64 [1], max f."""
+    out = torch.empty(1, dtype=torch.float64, device=f.device)
+    _check(lib().vegas_max_weight(_dev(f, torch.float64, "f"), f.shape[0], _dev(out, torch.float64, "w_max"), _stream(stream)))
+    return out
+
+
+def vegas_unweight(h, f, w_max, seed, iteration, first_event=0, stream=None):
+    """Hit-or-miss on the weights f of events [first_event, first_event + len(f)).  Returns (accepted global event
+    indices in ascending order as a cuda int64 tensor view of length n_kept, n_overweight)."""
+    n_ev = f.shape[0]
+    accepted = torch.empty(n_ev, dtype=torch.int64, device=f.device)
+    counts = torch.empty(2, dtype=torch.int64, device=f.device)
+    _reserved(h, n_ev)
+    _check(lib().vegas_unweight(h.ptr, _dev(f, torch.float64, "f"), n_ev, float(w_max), seed, iteration, first_event,
+                                _dev(accepted, torch.int64, "accepted"), _dev(counts, torch.int64, "counts"), _stream(stream)))
+    c = counts.tolist()      # marshalling: the two counters come back to size the view
+    return accepted[:c[0]], c[1]
+
+
+def vegas_generate(h, grid, sqrt_s, event_ids, stream=None):
+    """Momenta [n, n_ext, 4] and weights (without |M|^2 and cuts) [n] of the listed events of iteration grid.iteration."""
+    n = event_ids.shape[0]
+    momenta = torch.empty((n, h.n_external, 4), dtype=torch.float64, device=event_ids.device)
+    weights = torch.empty(n, dtype=torch.float64, device=event_ids.device)
+    _check(lib().vegas_generate(h.ptr, C.byref(grid.c), float(sqrt_s), _dev(event_ids, torch.int64, "event_ids"), n,
+                                _dev(momenta, torch.float64, "momenta"), _dev(weights, torch.float64, "weights"), _stream(stream)))
+    return momenta, weights
 
 
 def fp64_peak_probe(n_iter, stream=None):
@@ -242,27 +311,21 @@ def fp64_peak_probe(n_iter, stream=None):
 def vegas_iterate_sharded(h, grid, sqrt_s, n_total, group=None, stream=None):
     """One Vegas iteration over `n_total` events split across the ranks of `group`: every rank
     integrates its contiguous event range with the fused kernel (no communication), the per-rank sum vectors
-    (3 + n_dim * n_bins doubles) are all-gathered and added in FIXED rank order, and every rank refines its own copy
-    of the grid from the identical totals — so all ranks hold bit-identical grids and the result does not depend on
-    arrival order.  The exchange is latency-bound (3.2 KB); with backend "nccl" it runs over NVLink, with "gloo" over
-    the host.  Returns the same dict as vegas_iterate, identical on every rank."""
+    (3 + n_dim * n_bins doubles) are all-gathered and added by the library in FIXED rank order (vegas_combine), and
+    every rank refines its own copy of the grid from the identical totals — so all ranks hold bit-identical grids and
+    the result does not depend on arrival order.  The exchange is latency-bound (3.2 KB); with backend "nccl" it runs
+    over NVLink, with "gloo" over the host.  Returns the same dict as vegas_iterate, identical on every rank.
+    Marshalling only: every number is computed by the library."""
     import torch.distributed as dist
-    from .sharding import combine_vegas_sums, strong_shard
+    from .sharding import gather_sums, strong_shard
     rank = dist.get_rank(group) if dist.is_initialized() else 0
     world = dist.get_world_size(group) if dist.is_initialized() else 1
     first, n = strong_shard(rank, world, n_total)
     sums, _ = vegas_integrand(h, grid, sqrt_s, first, n, stream=stream)
     if world > 1:
-        on_host = dist.get_backend(group) == "gloo"
-        mine = sums.cpu() if on_host else sums
-        parts = [torch.empty_like(mine) for _ in range(world)]
-        dist.all_gather(parts, mine, group=group)
-        sums = combine_vegas_sums(parts).to(grid.edges.device)
+        sums = vegas_combine(gather_sums(sums, group), stream=stream)
     n_dim, n_bins = grid.c.n_dim, grid.c.n_bins
-    vegas_refine(grid.edges, sums[3:].reshape(n_dim, n_bins).contiguous(), grid.c.alpha, stream=stream)
-    s = sums[:3].cpu()
-    N = float(n_total)
-    integral = float(s[0]) / N
+    vegas_refine(grid.edges, sums[3:].view(n_dim, n_bins), grid.c.alpha, stream=stream)
+    res = vegas_finish(sums, n_total, stream=stream)
     grid.iteration = grid.iteration + 1
-    return dict(integral=integral, variance=(float(s[1]) / N - integral * integral) / (N - 1.0), sum_w=float(s[0]),
-                sum_w2=float(s[1]), n_pass=int(s[2]))
+    return res

@@ -37,7 +37,10 @@ struct me_handle {
   unsigned gluon_mask;
   // launch geometry of the CTA-per-W-events kernels
   int warps, grid, smem_bytes, regs, ctas_per_sm, sms;
-  // vegas scratch (grown on demand, never shrunk)
+  int device = 0;  // the device that was current in me_init: every call runs there
+  // vegas scratch: per-event buffers sized by me_reserve, fixed-size buffers by me_init; calls never allocate
+  int vegas_grid = 0;  // CTAs of the fused integrand kernel (fixed at me_init)
+  long long* block_counts = nullptr;  // vegas_unweight: accepted events per 256-event block [scratch_ev / 256 + 2]
   double* f_scratch = nullptr;
   unsigned long long* idx_scratch = nullptr;
   long long scratch_ev = 0;
@@ -52,6 +55,7 @@ struct me_handle {
 namespace madme {
 
 struct ProcOps {
+  int (*prepare)(me_handle* h);  // vegas: per-device kernel attribute, launch geometry, staging size (me_init)
   int (*fill)(me_handle* h);  // constants of the generated program + launch geometry
   int (*eval)(me_handle* h, const double* mom, double* me2, double* hel, long long n, cudaStream_t s);
   int (*integrand)(me_handle* h, const VegasArgs& a, double* f, unsigned long long* idx, int words, cudaStream_t s);

@@ -21,6 +21,20 @@ bool have_device() {
 }
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
+// A handle lives on the device that was current in me_init: calls run there and restore the caller's device.
+struct DeviceGuard {
+  int prev = -1;
+  bool ok = true;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; prev = -1; return; }
+    if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+    else if (prev == dev) prev = -1;
+  }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+#define ON_DEVICE_OF(h) DeviceGuard guard__((h)->device); if (!guard__.ok) return fail(ME_ECUDA, "cannot switch to the handle's device%s%s")
+constexpr int VEGAS_MAX_CHUNKS = 1024, VEGAS_MAX_OUT = 512 * VEGAS_RED_PER_THREAD;
+
 // ---- stand-alone phase-space kernels: one event per thread ------------------------------------------------
 __global__ void philox_kernel(unsigned long long seed, unsigned iteration, long long first, int n_dim, double* __restrict__ out,
                               long long n_ev) {
@@ -106,24 +120,126 @@ __global__ void __launch_bounds__(256) dfma_probe_kernel(long long n_iter, doubl
 
 inline int blocks_for(long long n, int threads) { return static_cast<int>((n + threads - 1) / threads); }
 
-int ensure_scratch(me_handle* h, long long n_ev, int idx_words, int n_chunks, int n_out) {
-  if (n_ev > h->scratch_ev) {
-    if (h->f_scratch) cudaFree(h->f_scratch);
-    if (h->idx_scratch) cudaFree(h->idx_scratch);
-    h->f_scratch = nullptr; h->idx_scratch = nullptr; h->scratch_ev = 0;
-    CU(cudaMalloc(&h->f_scratch, sizeof(double) * n_ev));
-    CU(cudaMalloc(&h->idx_scratch, sizeof(unsigned long long) * 2 * n_ev));
-    h->scratch_ev = n_ev;
+// ---- unweighting: hit-or-miss with a dedicated Philox counter word, order-preserving compaction ----
+__device__ __forceinline__ bool unweight_keep(double f, double w_max, unsigned long long seed, unsigned iteration, long long event) {
+  if (!(f > 0.0)) return false;
+  const uint4 w = philox4x32_10(make_uint4(static_cast<uint32_t>(event), static_cast<uint32_t>(static_cast<unsigned long long>(event) >> 32),
+                                           0x7fffffffu, iteration),
+                                make_uint2(static_cast<uint32_t>(seed), static_cast<uint32_t>(seed >> 32)));
+  return philox_u01(w.x, w.y) * w_max < f;
+}
+// pass 1: kept events per 256-event block (+ overweight count); pass 2 (one block): exclusive scan; pass 3: write
+__global__ void __launch_bounds__(256) unweight_count_kernel(const double* __restrict__ f, long long n_ev, double w_max, unsigned long long seed,
+                                                             unsigned iteration, long long first_event, long long* __restrict__ block_counts,
+                                                             unsigned long long* __restrict__ n_over) {
+  const long long e = static_cast<long long>(blockIdx.x) * 256 + threadIdx.x;
+  const double v = e < n_ev ? f[e] : 0.0;
+  const bool keep = e < n_ev && unweight_keep(v, w_max, seed, iteration, first_event + e);
+  const int c = __syncthreads_count(keep);
+  const int o = __syncthreads_count(e < n_ev && v > w_max);
+  if (threadIdx.x == 0) {
+    block_counts[blockIdx.x] = c;
+    if (o) atomicAdd(n_over, static_cast<unsigned long long>(o));   // an integer count: order does not matter
   }
-  (void)idx_words;
-  const long long need = static_cast<long long>(n_chunks) * n_out;
-  if (need > h->partial_len) {
-    if (h->partial) cudaFree(h->partial);
-    h->partial = nullptr; h->partial_len = 0;
-    CU(cudaMalloc(&h->partial, sizeof(double) * need));
-    h->partial_len = need;
+}
+__global__ void __launch_bounds__(1024) unweight_scan_kernel(long long* __restrict__ block_counts, long long n_blocks, long long* __restrict__ counts) {
+  __shared__ long long part[1024];
+  const long long per = (n_blocks + 1023) / 1024, lo = threadIdx.x * per, hi = min(n_blocks, lo + per);
+  long long s = 0;
+  for (long long i = lo; i < hi; ++i) s += block_counts[i];
+  part[threadIdx.x] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    long long run = 0;
+    for (int i = 0; i < 1024; ++i) { const long long t = part[i]; part[i] = run; run += t; }
+    counts[0] = run;
   }
+  __syncthreads();
+  long long run = part[threadIdx.x];
+  for (long long i = lo; i < hi; ++i) { const long long t = block_counts[i]; block_counts[i] = run; run += t; }
+}
+__global__ void __launch_bounds__(256) unweight_write_kernel(const double* __restrict__ f, long long n_ev, double w_max, unsigned long long seed,
+                                                             unsigned iteration, long long first_event, const long long* __restrict__ block_offsets,
+                                                             long long* __restrict__ accepted) {
+  __shared__ int warp_count[8];
+  const long long e = static_cast<long long>(blockIdx.x) * 256 + threadIdx.x;
+  const bool keep = e < n_ev && unweight_keep(f[e], w_max, seed, iteration, first_event + e);
+  const unsigned mask = __ballot_sync(0xffffffffu, keep);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (lane == 0) warp_count[warp] = __popc(mask);
+  __syncthreads();
+  if (keep) {
+    long long pos = block_offsets[blockIdx.x] + __popc(mask & ((1u << lane) - 1u));
+    for (int k = 0; k < warp; ++k) pos += warp_count[k];
+    accepted[pos] = first_event + e;
+  }
+}
+__global__ void max_weight_kernel(const double* __restrict__ f, long long n_ev, double* __restrict__ w_max) {
+  // grid-stride maximum; the maximum does not depend on the order, so one atomic per block is deterministic
+  double m = 0.0;
+  for (long long e = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x; e < n_ev; e += static_cast<long long>(gridDim.x) * blockDim.x)
+    m = fmax(m, f[e]);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0 && m > 0.0)
+    atomicMax(reinterpret_cast<unsigned long long*>(w_max), static_cast<unsigned long long>(__double_as_longlong(m)));  // non-negative doubles order like integers
+}
+
+// the kinematics of listed events (same device functions as the fused integrand)
+template <int NF>
+__global__ void vegas_generate_kernel(VegasArgs a, const long long* __restrict__ ids, long long n, double* __restrict__ mom_out,
+                                      double* __restrict__ wgt_out) {
+  const long long k = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  double p[NF][4], y[VEGAS_MAX_DIM], x[VEGAS_MAX_DIM];
+  philox_fill<VEGAS_MAX_DIM>(a.seed, a.iteration, static_cast<uint64_t>(ids[k]), a.n_dim, y);
+  double jac = 1.0;
+#pragma unroll
+  for (int d = 0; d < VEGAS_MAX_DIM; ++d) {
+    int bin;
+    x[d] = d < a.n_dim ? vegas_map_1d(a.edges + d * (a.n_bins + 1), a.n_bins, y[d], jac, bin) : 0.5;
+  }
+  double w = 0.0, rs = a.sqrt_s;
+  bool ok = true;
+  if (a.ps_mode == 2) {
+    double msum = 0.0;
+#pragma unroll
+    for (int i = 0; i < NF; ++i) msum += a.masses[i];
+    rs = sqrt(x[0] * x[1]) * a.sqrt_s;
+    ok = rs > msum;
+    if (ok) w = jac * toy_gluon_density(x[0]) * toy_gluon_density(x[1]) * rambo_event<NF>(x + 2, rs, a.masses, 1, rambo_volume(NF, rs * rs), p) *
+                (PB_GEV2 / (2.0 * rs * rs));
+  } else {
+    w = jac * rambo_event<NF>(x, a.sqrt_s, a.masses, a.ps_mode, a.w0, p) * a.prefactor;
+  }
+  double* o = mom_out + k * (4 * (NF + 2));
+  const double e = 0.5 * rs;
+  o[0] = e; o[1] = 0.0; o[2] = 0.0; o[3] = e;
+  o[4] = e; o[5] = 0.0; o[6] = 0.0; o[7] = -e;
+#pragma unroll
+  for (int i = 0; i < NF; ++i)
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) o[8 + 4 * i + mu] = ok ? p[i][mu] : 0.0;
+  wgt_out[k] = w;
+}
+
+int check_grid(const me_handle* h, const vegas_grid* g, double sqrt_s, const char* who) {
+  if (h->proc == P_EPEM) return fail(ME_EINVAL, "%s: QCD processes only%s", who);
+  const int nf = h->n_ext - 2, D = g->n_dim, nb = g->n_bins;
+  if (g->ps_mode < 0 || g->ps_mode > 2 || D != (g->ps_mode == 0 ? 4 * nf : g->ps_mode == 1 ? 3 * nf - 4 : 3 * nf - 2))
+    return fail(ME_EDIM, "%s: n_dim must be 4 n_final (ps_mode 0), 3 n_final - 4 (1) or 3 n_final - 2 (2)%s", who);
+  if (D > VEGAS_MAX_DIM || nb < 1 || nb > VEGAS_MAX_BINS || D * nb + 3 > VEGAS_MAX_OUT)
+    return fail(ME_EDIM, "%s: n_bins 1..255 and n_dim*n_bins <= 2045%s", who);
+  if (!(sqrt_s > 2.0 * h->par.m_top)) return fail(ME_EINVAL, "%s: sqrt_s below threshold%s", who);
   return ME_OK;
+}
+void fill_args(const me_handle* h, const vegas_grid* g, double sqrt_s, long long first_event, long long n_ev, VegasArgs& a) {
+  const int nf = h->n_ext - 2;
+  a.edges = g->edges; a.n_dim = g->n_dim; a.n_bins = g->n_bins; a.ps_mode = g->ps_mode; a.seed = g->seed;
+  a.iteration = static_cast<unsigned>(g->iteration); a.first_event = first_event; a.n_ev = n_ev; a.sqrt_s = sqrt_s;
+  a.w0 = rambo_volume(nf, sqrt_s * sqrt_s); a.prefactor = PB_GEV2 / (2.0 * sqrt_s * sqrt_s);
+  for (int i = 0; i < PS_MAX_FINAL; ++i) a.masses[i] = h->masses[i];
+  a.gluon_mask = h->gluon_mask; a.ptj_min = h->par.ptj_min; a.dr_min = h->par.dr_min; a.mass = h->mass; a.scale = h->scale;
 }
 
 }  // namespace
@@ -144,6 +260,7 @@ int me_init(const char* process, const me_params* params, me_handle** out) {
   if (params->w_top != 0.0) return fail(ME_EINVAL, "me_init: w_top must be 0 (no width in propagators)%s%s");
   if (!have_device()) return fail(ME_ENODEV, "me_init: no CUDA device (this library has no CPU path)%s%s");
   me_handle* h = new me_handle();
+  if (cudaGetDevice(&h->device) != cudaSuccess) { delete h; return fail(ME_ECUDA, "me_init: cudaGetDevice failed%s%s"); }
   h->proc = pr;
   h->par = *params;
   h->mass = (pr == P_EPEM) ? 0.0 : params->m_top;
@@ -159,9 +276,22 @@ int me_init(const char* process, const me_params* params, me_handle** out) {
     case P_GGTTG: rc = ops_gg_ttxg_eval()->fill(h); break;
     default: rc = ops_gg_ttxgg_eval()->fill(h); break;
   }
+  if (rc == ME_OK && pr != P_EPEM) {
+    switch (pr) {
+      case P_GGTT: rc = ops_gg_ttx_vegas()->prepare(h); break;
+      case P_GGTTG: rc = ops_gg_ttxg_vegas()->prepare(h); break;
+      default: rc = ops_gg_ttxgg_vegas()->prepare(h); break;
+    }
+  }
   if (rc == ME_OK) {
-    cudaError_t e = cudaMalloc(&h->sums_d, sizeof(double) * (3 + VEGAS_MAX_DIM * VEGAS_MAX_BINS));
+    // the fixed-size scratch of the Vegas path: sums, reduction partials, survivor staging, unweighting counters
+    cudaError_t e = cudaMalloc(&h->sums_d, sizeof(double) * (VEGAS_MAX_OUT + 8));
     if (e == cudaSuccess) e = cudaMallocHost(&h->sums_h, sizeof(double) * 4);
+    if (e == cudaSuccess && pr != P_EPEM) {
+      h->partial_len = static_cast<long long>(VEGAS_MAX_CHUNKS) * VEGAS_MAX_OUT;
+      e = cudaMalloc(&h->partial, sizeof(double) * h->partial_len);
+      if (e == cudaSuccess) e = cudaMalloc(&h->vegas_stage, sizeof(double) * h->vegas_stage_len);
+    }
     if (e != cudaSuccess) rc = cuda_fail(e, "me_init scratch");
   }
   if (rc != ME_OK) { me_free(h); return rc; }
@@ -171,6 +301,8 @@ int me_init(const char* process, const me_params* params, me_handle** out) {
 
 void me_free(me_handle* h) {
   if (!h) return;
+  DeviceGuard guard(h->device);
+  if (h->block_counts) cudaFree(h->block_counts);
   if (h->f_scratch) cudaFree(h->f_scratch);
   if (h->idx_scratch) cudaFree(h->idx_scratch);
   if (h->partial) cudaFree(h->partial);
@@ -178,6 +310,22 @@ void me_free(me_handle* h) {
   if (h->sums_h) cudaFreeHost(h->sums_h);
   if (h->vegas_stage) cudaFree(h->vegas_stage);
   delete h;
+}
+
+int me_reserve(me_handle* h, long long max_events) {
+  if (!h || max_events < 0) return fail(ME_EINVAL, "me_reserve: null handle or negative count%s%s");
+  if (max_events <= h->scratch_ev) return ME_OK;
+  ON_DEVICE_OF(h);
+  CU(cudaDeviceSynchronize());  // earlier work may still use the buffers that are replaced
+  if (h->f_scratch) cudaFree(h->f_scratch);
+  if (h->idx_scratch) cudaFree(h->idx_scratch);
+  if (h->block_counts) cudaFree(h->block_counts);
+  h->f_scratch = nullptr; h->idx_scratch = nullptr; h->block_counts = nullptr; h->scratch_ev = 0;
+  CU(cudaMalloc(&h->f_scratch, sizeof(double) * max_events));
+  CU(cudaMalloc(&h->idx_scratch, sizeof(unsigned long long) * VEGAS_IDX_WORDS * max_events));
+  CU(cudaMalloc(&h->block_counts, sizeof(long long) * (max_events / 256 + 2)));
+  h->scratch_ev = max_events;
+  return ME_OK;
 }
 
 int me_n_external(const me_handle* h) { return h ? h->n_ext : ME_EINVAL; }
@@ -196,6 +344,9 @@ long long me_info(const me_handle* h, int what) {
     case 8: return h->regs;
     case 9: return h->ctas_per_sm;
     case 10: return h->sms;
+    case 11: return h->scratch_ev;
+    case 12: return h->device;
+    case 13: return static_cast<long long>(reinterpret_cast<uintptr_t>(h->f_scratch));
     default: return ME_EINVAL;
   }
 }
@@ -206,7 +357,8 @@ static int eval_common(me_handle* h, const double* momenta, double* me2, double*
   if (n_ev == 0) return ME_OK;  // an empty batch needs no buffers
   if (!momenta || (!me2 && !hel)) return fail(ME_EINVAL, "me_eval: null buffer%s%s");
   if (!aligned16(momenta)) return fail(ME_EINVAL, "me_eval: momenta must be 16-byte aligned%s%s");
-  if (n_ev == 0) return ME_OK;
+  if (!have_device()) return fail(ME_ENODEV, "me_eval: no CUDA device%s%s");
+  ON_DEVICE_OF(h);
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   switch (h->proc) {
     case P_EPEM: return ops_epem_mupmum_eval()->eval(h, momenta, me2, hel, n_ev, s);
@@ -306,28 +458,20 @@ int vegas_refine(double* edges, int n_dim, int n_bins, const double* S, double a
 int vegas_integrand(me_handle* h, const vegas_grid* g, double sqrt_s, long long first_event, long long n_ev, double* sums,
                     double* f_out, void* stream) {
   if (!h || !g || !g->edges || !sums || n_ev < 0 || first_event < 0) return fail(ME_EINVAL, "vegas_integrand: null pointer or negative count%s%s");
-  if (h->proc == P_EPEM) return fail(ME_EINVAL, "vegas_integrand: QCD processes only%s%s");
-  const int nf = h->n_ext - 2, D = g->n_dim, nb = g->n_bins;
-  if (g->ps_mode < 0 || g->ps_mode > 2 || D != (g->ps_mode == 0 ? 4 * nf : g->ps_mode == 1 ? 3 * nf - 4 : 3 * nf - 2))
-    return fail(ME_EDIM, "vegas_integrand: n_dim must be 4 n_final (ps_mode 0), 3 n_final - 4 (1) or 3 n_final - 2 (2)%s%s");
-  if (nb < 1 || nb > VEGAS_MAX_BINS || D * nb + 3 > 512 * VEGAS_RED_PER_THREAD)
-    return fail(ME_EDIM, "vegas_integrand: n_bins 1..255 and n_dim*n_bins <= 2045%s%s");
-  if (!(sqrt_s > 2.0 * h->par.m_top)) return fail(ME_EINVAL, "vegas_integrand: sqrt_s below threshold%s%s");
+  int rc = check_grid(h, g, sqrt_s, "vegas_integrand");
+  if (rc) return rc;
+  if (n_ev > h->scratch_ev) return fail(ME_EINVAL, "vegas_integrand: n_ev exceeds the reserved scratch: call me_reserve(h, n_ev) first%s%s");
+  ON_DEVICE_OF(h);
+  const int D = g->n_dim, nb = g->n_bins;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const int n_out = 3 + D * nb, words = (D + 7) / 8;
   if (n_ev == 0) { CU(cudaMemsetAsync(sums, 0, sizeof(double) * n_out, s)); return ME_OK; }
   // fixed-shape reduction: chunk = ceil(n_ev / 1024) rounded up to a multiple of the tile -> n_chunks <= 1024
-  long long chunk = (n_ev + 1023) / 1024;
+  long long chunk = (n_ev + VEGAS_MAX_CHUNKS - 1) / VEGAS_MAX_CHUNKS;
   chunk = ((chunk + VEGAS_RED_TILE - 1) / VEGAS_RED_TILE) * VEGAS_RED_TILE;
   const int n_chunks = static_cast<int>((n_ev + chunk - 1) / chunk);
-  int rc = ensure_scratch(h, n_ev, words, n_chunks, n_out);
-  if (rc) return rc;
   VegasArgs a;
-  a.edges = g->edges; a.n_dim = D; a.n_bins = nb; a.ps_mode = g->ps_mode; a.seed = g->seed;
-  a.iteration = static_cast<unsigned>(g->iteration); a.first_event = first_event; a.n_ev = n_ev; a.sqrt_s = sqrt_s;
-  a.w0 = rambo_volume(nf, sqrt_s * sqrt_s); a.prefactor = PB_GEV2 / (2.0 * sqrt_s * sqrt_s);
-  for (int i = 0; i < PS_MAX_FINAL; ++i) a.masses[i] = h->masses[i];
-  a.gluon_mask = h->gluon_mask; a.ptj_min = h->par.ptj_min; a.dr_min = h->par.dr_min; a.mass = h->mass; a.scale = h->scale;
+  fill_args(h, g, sqrt_s, first_event, n_ev, a);
   double* f = f_out ? f_out : h->f_scratch;
   switch (h->proc) {
     case P_GGTT: rc = ops_gg_ttx_vegas()->integrand(h, a, f, h->idx_scratch, words, s); break;
@@ -342,22 +486,96 @@ int vegas_integrand(me_handle* h, const vegas_grid* g, double sqrt_s, long long 
   return ME_OK;
 }
 
+int vegas_combine(const double* parts, int n_parts, int n_out, double* sums, void* stream) {
+  if (!parts || !sums || n_parts < 1 || n_out < 1) return fail(ME_EINVAL, "vegas_combine: null pointer or empty input%s%s");
+  if (!have_device()) return fail(ME_ENODEV, "vegas_combine: no CUDA device%s%s");
+  vegas_reduce_final<<<blocks_for(n_out, 128), 128, 0, static_cast<cudaStream_t>(stream)>>>(parts, n_parts, n_out, sums);
+  CU(cudaGetLastError());
+  return ME_OK;
+}
+
+int vegas_finish(const double* sums, long long n_total, vegas_result* result, void* stream) {
+  if (!sums || !result || n_total < 2) return fail(ME_EINVAL, "vegas_finish: null pointer or n_total < 2%s%s");
+  if (!have_device()) return fail(ME_ENODEV, "vegas_finish: no CUDA device%s%s");
+  double host[3];
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  CU(cudaMemcpyAsync(host, sums, sizeof host, cudaMemcpyDeviceToHost, s));
+  CU(cudaStreamSynchronize(s));
+  const double N = static_cast<double>(n_total), I = host[0] / N;
+  result->integral = I;
+  result->variance = (host[1] / N - I * I) / (N - 1.0);
+  result->sum_w = host[0];
+  result->sum_w2 = host[1];
+  result->n_pass = static_cast<long long>(host[2]);
+  return ME_OK;
+}
+
 int vegas_iterate(me_handle* h, vegas_grid* g, double sqrt_s, long long n_ev, vegas_result* result, void* stream) {
   if (!h || !g || !result || n_ev < 2) return fail(ME_EINVAL, "vegas_iterate: null pointer or n_ev < 2%s%s");
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   int rc = vegas_integrand(h, g, sqrt_s, 0, n_ev, h->sums_d, nullptr, s);
   if (rc) return rc;
+  ON_DEVICE_OF(h);
   vegas_refine_kernel<<<1, 32, 0, s>>>(g->edges, g->n_dim, g->n_bins, h->sums_d + 3, g->alpha);
   CU(cudaGetLastError());
-  CU(cudaMemcpyAsync(h->sums_h, h->sums_d, sizeof(double) * 3, cudaMemcpyDeviceToHost, s));
-  CU(cudaStreamSynchronize(s));
-  const double N = static_cast<double>(n_ev), I = h->sums_h[0] / N;
-  result->integral = I;
-  result->variance = (h->sums_h[1] / N - I * I) / (N - 1.0);
-  result->sum_w = h->sums_h[0];
-  result->sum_w2 = h->sums_h[1];
-  result->n_pass = static_cast<long long>(h->sums_h[2]);
+  rc = vegas_finish(h->sums_d, n_ev, result, stream);
+  if (rc) return rc;
   g->iteration += 1;
+  return ME_OK;
+}
+
+int vegas_max_weight(const double* f, long long n_ev, double* w_max, void* stream) {
+  if (!w_max || n_ev < 0 || (n_ev > 0 && !f)) return fail(ME_EINVAL, "vegas_max_weight: null pointer or negative count%s%s");
+  if (!have_device()) return fail(ME_ENODEV, "vegas_max_weight: no CUDA device%s%s");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  CU(cudaMemsetAsync(w_max, 0, sizeof(double), s));
+  if (n_ev == 0) return ME_OK;
+  const int blocks = static_cast<int>(n_ev / 256 + 1 < 1184 ? n_ev / 256 + 1 : 1184);
+  max_weight_kernel<<<blocks, 256, 0, s>>>(f, n_ev, w_max);
+  CU(cudaGetLastError());
+  return ME_OK;
+}
+
+int vegas_unweight(me_handle* h, const double* f, long long n_ev, double w_max, uint64_t seed, uint64_t iteration, long long first_event,
+                   long long* accepted, long long* counts, void* stream) {
+  if (!h || !counts || n_ev < 0 || first_event < 0 || (n_ev > 0 && (!f || !accepted)))
+    return fail(ME_EINVAL, "vegas_unweight: null pointer or negative count%s%s");
+  if (!(w_max > 0.0)) return fail(ME_EINVAL, "vegas_unweight: w_max must be positive%s%s");
+  if (n_ev > h->scratch_ev) return fail(ME_EINVAL, "vegas_unweight: n_ev exceeds the reserved scratch: call me_reserve(h, n_ev) first%s%s");
+  ON_DEVICE_OF(h);
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  CU(cudaMemsetAsync(counts, 0, 2 * sizeof(long long), s));
+  if (n_ev == 0) return ME_OK;
+  const long long n_blocks = (n_ev + 255) / 256;
+  unweight_count_kernel<<<static_cast<unsigned>(n_blocks), 256, 0, s>>>(f, n_ev, w_max, seed, static_cast<unsigned>(iteration), first_event,
+                                                                        h->block_counts, reinterpret_cast<unsigned long long*>(counts + 1));
+  CU(cudaGetLastError());
+  unweight_scan_kernel<<<1, 1024, 0, s>>>(h->block_counts, n_blocks, counts);
+  CU(cudaGetLastError());
+  unweight_write_kernel<<<static_cast<unsigned>(n_blocks), 256, 0, s>>>(f, n_ev, w_max, seed, static_cast<unsigned>(iteration), first_event,
+                                                                        h->block_counts, accepted);
+  CU(cudaGetLastError());
+  return ME_OK;
+}
+
+int vegas_generate(me_handle* h, const vegas_grid* g, double sqrt_s, const long long* event_ids, long long n, double* momenta,
+                   double* weights, void* stream) {
+  if (!h || !g || !g->edges || n < 0 || (n > 0 && (!event_ids || !momenta || !weights)))
+    return fail(ME_EINVAL, "vegas_generate: null pointer or negative count%s%s");
+  int rc = check_grid(h, g, sqrt_s, "vegas_generate");
+  if (rc) return rc;
+  if (n == 0) return ME_OK;
+  ON_DEVICE_OF(h);
+  VegasArgs a;
+  fill_args(h, g, sqrt_s, 0, n, a);
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const int T = 128, B = blocks_for(n, T);
+  switch (h->n_ext - 2) {
+    case 2: vegas_generate_kernel<2><<<B, T, 0, s>>>(a, event_ids, n, momenta, weights); break;
+    case 3: vegas_generate_kernel<3><<<B, T, 0, s>>>(a, event_ids, n, momenta, weights); break;
+    default: vegas_generate_kernel<4><<<B, T, 0, s>>>(a, event_ids, n, momenta, weights); break;
+  }
+  CU(cudaGetLastError());
   return ME_OK;
 }
 

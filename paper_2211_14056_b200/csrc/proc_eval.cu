@@ -54,7 +54,7 @@ int eval(me_handle* h, const double* mom, double* me2, double* hel, long long n,
   return ME_OK;
 }
 
-const ProcOps ops = {fill, eval, nullptr};
+const ProcOps ops = {nullptr, fill, eval, nullptr};
 }  // namespace tu_<process>
 
 const ProcOps* MADME_CAT(ops_, MADME_PROC, _eval)() { return &MADME_CAT(tu_, MADME_PROC, _e)::ops; }

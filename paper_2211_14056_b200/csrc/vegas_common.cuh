@@ -8,6 +8,7 @@
 namespace madme {
 
 constexpr int VEGAS_MAX_DIM = 4 * PS_MAX_FINAL;
+constexpr int VEGAS_IDX_WORDS = (VEGAS_MAX_DIM + 7) / 8;   // bin indices packed one byte per dimension
 constexpr double PB_GEV2 = 0.3893793721e9;  // (hbar c)^2 in pb GeV^2
 
 struct VegasArgs {
@@ -31,7 +32,7 @@ static __global__ void __launch_bounds__(512) vegas_reduce_chunks(const double* 
                                                            int idx_words, int n_dim, int n_bins, long long n_ev, long long chunk,
                                                            double* __restrict__ partial) {
   __shared__ double f_s[VEGAS_RED_TILE];
-  __shared__ unsigned long long idx_s[2 * VEGAS_RED_TILE];
+  __shared__ unsigned long long idx_s[VEGAS_IDX_WORDS * VEGAS_RED_TILE];
   const int n_out = n_dim * n_bins + 3, t = threadIdx.x;
   const long long begin = blockIdx.x * chunk, end = min(n_ev, begin + chunk);
   double acc[VEGAS_RED_PER_THREAD];

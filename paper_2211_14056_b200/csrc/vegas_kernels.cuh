@@ -31,7 +31,7 @@ __global__ void __launch_bounds__(32 * P::N_WARPS, 1) vegas_integrand_kernel(Veg
     const bool live = ev < a.n_ev;
     {
       double p[NF][4], y[VEGAS_MAX_DIM], x[VEGAS_MAX_DIM];
-      unsigned long long packed[2] = {0ull, 0ull};
+      unsigned long long packed[VEGAS_IDX_WORDS] = {};   // one byte per dimension
       bool pass = false;
       double w = 0.0, rs = a.sqrt_s;
       if (live) {

@@ -1,6 +1,7 @@
 """Event-range sharding over ranks: events are independent and event e's random numbers
 depend only on (seed, iteration, e), so rank r of N takes the global event indices [first, first + n) below and the
-union over ranks is the single-GPU stream, whatever N is.  No arithmetic of the method lives here.
+union over ranks is the single-GPU stream, whatever N is.  No arithmetic of the method lives here: the one exchange of
+a sharded Vegas iteration is gathered here and ADDED by the library (vegas_combine, fixed rank order).
 """
 
 
@@ -20,10 +21,15 @@ def strong_shard(rank: int, world: int, total_events: int):
     return first, base + (1 if rank < extra else 0)
 
 
-def combine_vegas_sums(per_rank_sums):
-    """Sum the per-shard (sum f, sum f^2, n_pass, S_{d,i}) vectors in FIXED rank order (reproducible whatever the
-    arrival order): what a multi-GPU vegas_iterate does between vegas_integrand and vegas_refine."""
-    total = None
-    for s in per_rank_sums:
-        total = s.clone() if total is None else total + s
-    return total
+def gather_sums(sums, group=None):
+    """All-gather every rank's (sum f, sum f^2, n_pass, S_{d,i}) vector; returns them stacked in RANK order,
+    [world, n_out], on the device of `sums` (through the host with the gloo backend).  The addition is the library's
+    (vegas_combine): no arithmetic here."""
+    import torch
+    import torch.distributed as dist
+    world = dist.get_world_size(group)
+    on_host = dist.get_backend(group) == "gloo"
+    mine = sums.cpu() if on_host else sums
+    parts = [torch.empty_like(mine) for _ in range(world)]
+    dist.all_gather(parts, mine, group=group)
+    return torch.stack(parts).to(sums.device).contiguous()

@@ -207,3 +207,55 @@ def test_vegas_iterate_ref_by_hand():
         # the second iteration uses the refined grid and a new random stream
         r2 = me.vegas_iterate(g, 1000.0, n)
         assert g.iteration == 2 and r2["integral"] != r["integral"]
+
+
+# ---- unweighted events ------------------------------------------------------------------------
+def test_unweighting_is_hit_or_miss_with_its_own_random_stream():
+    """Pins of vegas_unweight_ref: the uniform comes from Philox counter (event, 0x7fffffff, iteration) — recomputed here
+    from the pinned raw Philox —, the decision is u w_max < f, the accepted list is ascending and reproducible under
+    sharding, overweight events are always kept and counted, and the acceptance rate is <f>/w_max within its binomial
+    error (so the kept events carry unit weight)."""
+    rng = np.random.default_rng(5)
+    n = 40000
+    f = rng.exponential(1.0, n) * (rng.uniform(size=n) < 0.8)        # 20 % cut events with f = 0
+    w_max = 6.0
+    acc, n_over = ref.vegas_unweight(f, w_max, seed=4, iteration=3, first_event=1000)
+    assert n_over == int((f > w_max).sum()) and n_over > 0
+    assert np.all(np.diff(acc) > 0) and acc.min() >= 1000 and acc.max() < 1000 + n
+    keep = np.zeros(n, bool)
+    keep[acc - 1000] = True
+    assert not keep[f == 0].any() and keep[f > w_max].all()
+    for e in list(range(0, 200)) + [n - 1]:                           # the decision, event by event, from raw Philox
+        o = ref.philox_raw([(1000 + e) & 0xffffffff, (1000 + e) >> 32, 0x7fffffff, 3], [4, 0])
+        u = (((int(o[0]) << 32 | int(o[1])) >> 11) + 0.5) / 2 ** 53
+        assert keep[e] == (f[e] > 0 and u * w_max < f[e])
+    p = np.minimum(f / w_max, 1.0)
+    assert abs(keep.sum() - p.sum()) < 5 * math.sqrt((p * (1 - p)).sum())
+    # sharding: two halves with their own first_event give the same list
+    a1, _ = ref.vegas_unweight(f[:n // 2], w_max, 4, 3, 1000)
+    a2, _ = ref.vegas_unweight(f[n // 2:], w_max, 4, 3, 1000 + n // 2)
+    assert np.array_equal(np.concatenate([a1, a2]), acc)
+    # another iteration or seed decides differently; the phase-space uniforms of the event do not enter
+    assert not np.array_equal(ref.vegas_unweight(f, w_max, 4, 2, 1000)[0], acc)
+    assert not np.array_equal(ref.vegas_unweight(f, w_max, 5, 3, 1000)[0], acc)
+
+
+def test_generate_reproduces_the_integrand_kinematics():
+    """vegas_generate_ref(ids) gives the momenta and the |M|^2-free weight of exactly the events vegas_integrand_ref
+    integrates: f_e = weight_e x Theta_e x me2(momenta_e) with the pinned cuts and tier-1 |M|^2 called separately."""
+    from paper_2211_14056_b200.workloads import PARAMS
+    me = ref.MatrixElementRef("gg_ttxg")
+    g = ref.GridRef(5, 50, 1.5, seed=8, ps_mode=1)
+    rng = np.random.default_rng(1)
+    e = np.sort(rng.uniform(size=(5, 51)), axis=1)
+    e[:, 0], e[:, -1] = 0.0, 1.0
+    g.edges[:] = e
+    n = 300
+    sums, f = me.vegas_integrand(g, 1000.0, 40, n, want_f=True)
+    ids = np.arange(40, 40 + n)[::-1].copy()                           # any order, any subset
+    mom, w = me.vegas_generate(g, 1000.0, ids)
+    ok = ref.cuts(mom, (0, 0, 1), PARAMS["ptj_min"], PARAMS["dr_min"]).astype(bool)
+    want = np.where(ok, w * me.eval(mom), 0.0)[::-1]
+    nz = want != 0
+    assert np.array_equal(nz, f != 0) and nz.sum() > 100
+    assert np.max(np.abs(f[nz] / want[nz] - 1)) < 1e-12

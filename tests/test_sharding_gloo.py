@@ -11,7 +11,7 @@ import torch
 import torch.distributed as dist
 import torch.multiprocessing as mp
 
-from paper_2211_14056_b200.sharding import combine_vegas_sums, strong_shard, weak_shard
+from paper_2211_14056_b200.sharding import strong_shard, weak_shard
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
@@ -41,7 +41,9 @@ def _worker(rank, world, port, n_total, q):
     sums = torch.from_numpy(ref.vegas_accumulate(f, idx, 50))
     gathered = [torch.zeros_like(sums) for _ in range(world)]
     dist.all_gather(gathered, sums)
-    total = combine_vegas_sums(gathered)
+    total = gathered[0].clone()      # what vegas_combine does on the device: fixed rank order
+    for part in gathered[1:]:
+        total = total + part
     ms = torch.tensor([10.0 + rank])
     dist.all_reduce(ms, op=dist.ReduceOp.MAX)
     sizes = [torch.zeros(1, dtype=torch.int64) for _ in range(world)]
