@@ -26,9 +26,11 @@ if ROOT not in sys.path:
 METRIC = "gg->ttbar gg |M|^2 events/sec (fp64, 1 B200)"
 UNIT = "events/s"
 NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12  # SMs x DFMA lanes/SM x 2 flop x max SM clock
-# dram__bytes_read.sum + dram__bytes_write.sum of me_eval_kernel<gg_ttxgg, 8> per event, from the ncu --set full capture
-# summarised in profiles/r1_me_eval_summary.md (818.4 MB + 36.9 MB for 4 194 304 events; algorithmic: 200 B/event)
-NCU_DRAM_BYTES_PER_EVENT = {"gg_ttxgg": 203.9}
+# dram__bytes_read.sum + dram__bytes_write.sum of me_eval_kernel<gg_ttxgg> per event, from the ncu --set full capture
+# of the kernel at HEAD summarised in profiles/r2_me_eval_summary.md (817.7 MB + 37.1 MB for 4 194 304 events;
+# algorithmic: 200 B/event)
+NCU_DRAM_BYTES_PER_EVENT = {"gg_ttxgg": 203.8}
+NCU_SUMMARY = "profiles/r2_me_eval_summary.md"
 
 
 class ClockSampler(threading.Thread):
@@ -66,12 +68,16 @@ class ClockSampler(threading.Thread):
                 "reasons": sorted(reasons), "samples": len(self.rows), "power_w_max": max(pw) if pw else None}
 
 
-def oracle_rate(workload, n_sample, first_event=0):
-    """Time the tier-1 oracle, as it stands, on the host cores over n_sample events of the workload's own stream."""
+def oracle_rate(workload, n_sample, first_event=0, blocks=1):
+    """Time the tier-1 oracle, as it stands, on the host cores over n_sample events of the workload's own stream:
+    `blocks` equally spaced runs of consecutive events starting at first_event (blocks = 1: the first n_sample)."""
     import numpy as np
     from oracle import ref
     w = workload
-    r = ref.philox_uniform(w.seed, 0, first_event, w.n_dim, n_sample)
+    per = max(1, n_sample // blocks)
+    gap = max(per, (w.n_events - first_event) // blocks)
+    r = np.concatenate([ref.philox_uniform(w.seed, 0, first_event + b * gap, w.n_dim, per) for b in range(blocks)])
+    n_sample = len(r)
     me = ref.MatrixElementRef(w.process)
     t0 = time.perf_counter()
     mom, wt = ref.rambo_generate(r, w.sqrt_s, w.masses, w.ps_mode)
@@ -114,6 +120,7 @@ def main():
     ap.add_argument("--workload", default="config3", choices=["config3", "config4", "config4_hadronic", "config2", "config1"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-vegas-leg", action="store_true", help="skip the config-4 Vegas integration reported beside config 3")
     args = ap.parse_args()
 
     from paper_2211_14056_b200.workloads import BY_NAME, PARAMS, VEGAS_ALPHA, VEGAS_BINS
@@ -154,7 +161,7 @@ def main():
 
     def step(k, timed):
         if vegas:
-            if world > 1:  # strong-sharded iteration over world * n_ev events with the single 3.2 KB exchange
+            if world > 1:  # strong-sharded iteration over world * n_ev events with the single 3.2 KB exchange (NCCL)
                 return api.vegas_iterate_sharded(h, grid, wl.sqrt_s, n_ev * world)
             return api.vegas_iterate(h, grid, wl.sqrt_s, n_ev)
         api.philox_uniform(wl.seed, k, first, wl.n_dim, n_ev, out=rand)
@@ -194,10 +201,10 @@ def main():
 
     # dominant kernel: me_eval (or the fused integrand), CUDA events on its own stream
     flops_ev = api.me_flops_per_event(h)
-    if vegas:
+    if vegas:   # the roofline is per GPU: this rank's launch evaluated about 1/world of the surviving events
         kern_ms = ms_total / args.steps
-        pass_frac = last["n_pass"] / n_ev
-        flops_launch = flops_ev * last["n_pass"]
+        pass_frac = last["n_pass"] / (n_ev * world)
+        flops_launch = flops_ev * last["n_pass"] / world
     else:
         kern_ms = sum(a.elapsed_time(b) for a, b in me_ms) / len(me_ms)
         pass_frac = float(passed.float().mean().item())
@@ -217,7 +224,7 @@ def main():
     # end to end through the public API with HOST buffers: pinned uniforms in, (me2, weight, pass) out, every step
     e2e = None
     if not vegas:
-        n_e2e = min(n_ev, 1 << 22)
+        n_e2e = n_ev          # the same events per step as the device-resident number
         rand_h = torch.empty((n_e2e, wl.n_dim), dtype=torch.float64).pin_memory()
         rand_h.copy_(rand[:n_e2e])
         me2_h = torch.empty(n_e2e, dtype=torch.float64).pin_memory()
@@ -273,6 +280,38 @@ def main():
         e2e = {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 24,
                "note": "vegas_iterate generates its inputs on the device from the seed; result scalars are read back every step"}
 
+    # config 4 beside the headline: a short extra leg, outside the timed region above — the full
+    # Vegas integration of BASELINE.json:configs[4] (5 iterations of the workload's event count, uniform start)
+    vegas_leg = None
+    if not vegas and world == 1 and wl.name == "config3" and not args.no_vegas_leg:
+        from paper_2211_14056_b200.workloads import VEGAS_ITERATIONS
+        w4 = BY_NAME["config4"]
+        del rand, mom
+        torch.cuda.empty_cache()
+        n4 = args.events or w4.n_events
+        g4 = api.VegasGrid(w4.n_dim, VEGAS_BINS, VEGAS_ALPHA, w4.seed, w4.ps_mode)
+        api.me_reserve(h, n4)
+        api.vegas_iterate(h, api.VegasGrid(w4.n_dim, VEGAS_BINS, VEGAS_ALPHA, w4.seed, w4.ps_mode), w4.sqrt_s, min(n4, 1 << 20))  # warm-up
+        its, evs = [], []
+        for _ in range(VEGAS_ITERATIONS):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            its.append(api.vegas_iterate(h, g4, w4.sqrt_s, n4))
+            b.record(stream)
+            evs.append((a, b))
+        torch.cuda.synchronize()
+        it_ms = [a.elapsed_time(b) for a, b in evs]
+        wts = [1.0 / r["variance"] for r in its]
+        comb = sum(r["integral"] * x for r, x in zip(its, wts)) / sum(wts)
+        chi2 = sum((r["integral"] - comb) ** 2 * x for r, x in zip(its, wts)) / (len(its) - 1)
+        lastv = its[-1]
+        tf = flops_ev * lastv["n_pass"] / (it_ms[-1] * 1e-3) / 1e12
+        vegas_leg = {"workload": "config4 gg_ttxgg D=%d, %d iterations x %d events, uniform start, seed %d" % (w4.n_dim, len(its), n4, w4.seed),
+                     "events_per_s_per_iteration": [n4 / (t * 1e-3) for t in it_ms], "ms_per_iteration": it_ms,
+                     "cut_pass_fraction_last": lastv["n_pass"] / n4, "tflops_last": tf, "frac_of_measured_last": tf / probe_tflops,
+                     "integral_pb_last": lastv["integral"], "sigma_pb_last": lastv["variance"] ** 0.5,
+                     "integral_pb_combined": comb, "sigma_pb_combined": sum(wts) ** -0.5, "chi2_per_dof": chi2}
+
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -281,9 +320,10 @@ def main():
     if not args.no_cpu_baseline and world == 1:
         rate0, _, cores = oracle_rate(wl, 256)
         n_s = int(max(256, min(1 << 16, rate0 * 15.0)))
-        rate, dt, cores = oracle_rate(wl, n_s)
-        cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": "first %d events of %s (Philox seed %d): rambo + cuts + tier-1 |M|^2, %.1f s" % (n_s, wl.name, wl.seed, dt)}
+        rate, dt, cores = oracle_rate(wl, n_s, blocks=64)
+        cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "events_per_s_per_core": rate / max(1, cores),
+               "sample": "%d events of %s (Philox seed %d) in 64 equally spaced runs over the stream: rambo + cuts + tier-1 |M|^2, %.1f s"
+                         % (n_s // 64 * 64, wl.name, wl.seed, dt)}
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "f64", "data": "synthetic",
@@ -298,11 +338,13 @@ def main():
                         "peak_measured_dfma_chain": probe_tflops, "frac_of_measured": achieved / probe_tflops,
                         "flops_per_event": flops_ev, "kernel_ms": kern_ms,
                         "traffic": (NCU_DRAM_BYTES_PER_EVENT[wl.process] * n_ev if (wl.process in NCU_DRAM_BYTES_PER_EVENT and not vegas) else None),
-                        "traffic_unit": "bytes per launch (ncu capture, profiles/r1_me_eval_summary.md)",
+                        "traffic_unit": "bytes per launch (ncu --set full capture of this kernel, %s)" % NCU_SUMMARY,
                         "hbm_gbs_algorithmic": (32 * (nf + 2) + 8) * n_ev / (kern_ms * 1e-3) / 1e9},
            "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "clocks": clocks}
     if vegas:
         out["vegas"] = last
+    elif vegas_leg is not None:
+        out["vegas"] = vegas_leg
     print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()

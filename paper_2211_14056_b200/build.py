@@ -57,6 +57,13 @@ def build(force: bool = False, verbose: bool = False) -> str:
         res = subprocess.run(link, capture_output=True, text=True)
         text += " ".join(link) + "\n" + res.stdout + res.stderr
         failed = res.returncode != 0
+    if not failed:   # the stand-alone measurement programs of csrc/probes (profiles/r2_probes.md), not linked into the library
+        for name in sorted(os.listdir(os.path.join(CSRC, "probes"))):
+            if name.endswith(".cu"):
+                cmd = [NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-o", os.path.join(objdir, name[:-3]), os.path.join(CSRC, "probes", name)]
+                res = subprocess.run(cmd, capture_output=True, text=True)
+                text += " ".join(cmd) + "\n" + res.stdout + res.stderr
+                failed = failed or res.returncode != 0
     log = os.path.join(HERE, "build.log")
     with open(log, "w") as f:
         f.write(text)
