@@ -55,29 +55,32 @@ template <class P> struct EventSmem {
 constexpr int ME_W = 8;  // events per CTA (gen/emit.py::W_EVENTS: the item tables are laid out for it); a CTA has P::N_WARPS >= ME_W
                          // warps: all of them run items, the first ME_W own one event each in the dot stages
 
-// J parked in tensor memory: warp w owns lanes 32 (w % 4) .. +31 and the column block w / 4
+// J in tensor memory: warp w owns TMEM lanes 32 (w % 4) .. +31 and the column block w / 4 (REGS columns: 4 per colour
+// flow it holds).  With P::SPLIT_J an event has TWO warps (w and w + 8, same lanes, neighbouring blocks), each holding
+// the flows of one half; the halves meet once, for J^dagger CF J, by reading the partner's block.
 template <class P> struct JPark {
-  static constexpr bool ON = P::N_ROUNDS > 1;
-  static constexpr int REGS = 4 * P::N_FLOW;                      // 32-bit columns per warp
-  static constexpr int COLS = tmem_cols((ME_W / 4) * REGS);       // allocation: a power of two >= 32
-  static __device__ __forceinline__ uint32_t addr(uint32_t base) {
-    const int warp = threadIdx.x >> 5;
+  static constexpr int NFW = P::SPLIT_J ? P::N_FLOW_HALF : P::N_FLOW;   // flows per warp
+  static constexpr bool ON = P::N_ROUNDS > 1 || P::SPLIT_J;
+  static constexpr int REGS = 4 * NFW;                             // 32-bit columns per warp
+  static constexpr int COLS = tmem_cols((P::N_WARPS / 4) * REGS);  // allocation: a power of two >= 32
+  static __device__ __forceinline__ uint32_t addr(uint32_t base, int warp) {
     return base + (static_cast<uint32_t>(32 * (warp & 3)) << 16) + (warp >> 2) * REGS;
   }
-  static __device__ __forceinline__ void park(uint32_t base, const double* jr, const double* ji) {
+  static __device__ __forceinline__ void park(uint32_t base, int warp, const double* jr, const double* ji) {
     uint32_t r[REGS];
 #pragma unroll
-    for (int f = 0; f < P::N_FLOW; ++f) {
+    for (int f = 0; f < NFW; ++f) {
       r[4 * f] = __double2loint(jr[f]); r[4 * f + 1] = __double2hiint(jr[f]);
       r[4 * f + 2] = __double2loint(ji[f]); r[4 * f + 3] = __double2hiint(ji[f]);
     }
-    tmem_store<REGS>(addr(base), r);
+    tmem_store<REGS>(addr(base, warp), r);
   }
-  static __device__ __forceinline__ void unpark(uint32_t base, double* jr, double* ji) {
-    uint32_t r[REGS];
-    tmem_load<REGS>(addr(base), r);
+  // N flows starting at flow `first` of the block of warp `owner`
+  template <int N> static __device__ __forceinline__ void load(uint32_t base, int owner, int first, double* jr, double* ji) {
+    uint32_t r[4 * N];
+    tmem_load<4 * N>(addr(base, owner) + 4 * first, r);
 #pragma unroll
-    for (int f = 0; f < P::N_FLOW; ++f) {
+    for (int f = 0; f < N; ++f) {
       jr[f] = __hiloint2double(r[4 * f + 1], r[4 * f]);
       ji[f] = __hiloint2double(r[4 * f + 3], r[4 * f + 2]);
     }
@@ -85,15 +88,18 @@ template <class P> struct JPark {
 };
 
 // |M|^2 of the 8 events whose momenta sit at the head of each event slice ([n_ext][4]).  Returns, on every lane of
-// warp w, the helicity- and colour-summed, averaged value of event w.  hel_out (optional, global [N_HEL], per warp)
+// warp w < 8, the helicity- and colour-summed, averaged value of event w.  hel_out (optional, global [N_HEL], per warp)
 // receives each helicity combination's share.  tmem: base address of the CTA's tensor-memory allocation.
 template <class P>
 __device__ __forceinline__ double cta_me2(double* smem, double mass, double scale, double* hel_out, uint32_t tmem) {
   constexpr int STRIDE = EventSmem<P>::DOUBLES;
   constexpr int W = ME_W;
+  constexpr bool SPLIT = P::SPLIT_J;
+  static_assert(!SPLIT || P::N_WARPS == 2 * W, "two warps per event");
   // the warp index through a shuffle: the compiler then knows it is warp-uniform, so the item loop (table reads, op
   // and coefficient decoding, branches) runs on the uniform datapath
   const int lane = threadIdx.x & 31, warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
+  const int ev_w = warp & (W - 1), role = warp / W;   // dot stages: this warp's event, and which half of the flows
   // a5: subset momenta / denominators and external wavefunctions, work = (subset or leg, event)
   {
     const int t = threadIdx.x, ev = t % W;
@@ -103,10 +109,12 @@ __device__ __forceinline__ double cta_me2(double* smem, double mass, double scal
   __syncthreads();
   double* base = smem + 4 * P::N_EXT;  // event e's scratch = base + e * STRIDE
   static_assert(P::N_HEL_EVAL <= 32, "one helicity combination per lane");
-  double jr[P::N_FLOW], ji[P::N_FLOW];
-  const double* my = base + warp * STRIDE;
+  constexpr int NFW = JPark<P>::NFW;
+  double jr[NFW], ji[NFW];
+  const double* my = base + ev_w * STRIDE;
   double* sm_e = base + (lane % W) * STRIDE;   // items: lane = local variant j x event
   const int j = lane / W;
+  const bool dot_warp = SPLIT || P::N_WARPS == W || warp < W;   // helper warps (if any) only run items
   int it = 0;
   // ONE copy of the item interpreter and one of each round's dot products in the instruction stream.  Warp w runs
   // items w, w + N_WARPS, ... of a stage: the generator balanced them by cost (a shared work counter was measured
@@ -115,27 +123,68 @@ __device__ __forceinline__ double cta_me2(double* smem, double mass, double scal
   for (int p = 0; p < P::N_STAGES; ++p) {
     const int end = P::stage_end(p);
 #pragma unroll 1
-    for (int i = it + warp; i < end; i += P::N_WARPS) me_run_item(c_items[i], c_members, j, sm_e, mass);
+    for (int i = it + warp; i < end; i += P::N_WARPS) me_run_item<!SPLIT>(c_items[i], c_members, j, sm_e, mass);
     it = end;
     __syncthreads();
     const int r = P::stage_dots(p);
     if (r >= 0) {
       // J is defined here on every path (zero in the first round, un-parked afterwards): dead during the items
-      if (P::N_WARPS == W || warp < W) {   // helper warps (>= W), if any, only run items
+      if (dot_warp) {
         if (r == 0) {
 #pragma unroll
-          for (int f = 0; f < P::N_FLOW; ++f) { jr[f] = 0.0; ji[f] = 0.0; }
+          for (int f = 0; f < NFW; ++f) { jr[f] = 0.0; ji[f] = 0.0; }
         } else if (JPark<P>::ON) {
-          JPark<P>::unpark(tmem, jr, ji);
+          JPark<P>::template load<NFW>(tmem, warp, 0, jr, ji);
         }
-        if (lane < P::N_HEL_EVAL) P::dots(r, my, lane, jr, ji);
-        if (JPark<P>::ON && r + 1 < P::N_ROUNDS) JPark<P>::park(tmem, jr, ji);
+        if (lane < P::N_HEL_EVAL) {
+          if (!SPLIT) P::dots(r, my, lane, jr, ji);
+          else if (role == 0) P::dots_a(r, my, lane, jr, ji);
+          else P::dots_b(r, my, lane, jr, ji);
+        }
+        if (JPark<P>::ON && (SPLIT || r + 1 < P::N_ROUNDS)) JPark<P>::park(tmem, warp, jr, ji);
       }
       if (r + 1 < P::N_ROUNDS) __syncthreads();   // the next round's items overwrite the round region
     }
   }
-  if (P::N_WARPS > W && warp >= W) return 0.0;
-  double v = (lane < P::N_HEL_EVAL) ? P::colour(jr, ji) : 0.0;
+  double v = 0.0;
+  if (!SPLIT) {
+    if (P::N_WARPS > W && warp >= W) return 0.0;
+    if (lane < P::N_HEL_EVAL) v = P::colour(jr, ji);
+  } else {
+    // a9 with two warps per event: both halves are parked; role A contracts (A, A) and A x (first chunk of B), role B
+    // (B, B) and (rest of B) x A read in two chunks; the two partial sums meet in shared memory
+    __shared__ double v_b[W][32];
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    if (role == 0) {
+      v = P::colour_own_a(jr, ji);
+      if constexpr (P::CHUNK_B > 0) {
+        double pr[P::CHUNK_B], pi[P::CHUNK_B];
+        JPark<P>::template load<P::CHUNK_B>(tmem, warp + W, 0, pr, pi);
+        v += P::colour_cross_a(jr, ji, pr, pi);
+      }
+    } else if constexpr (P::N_FLOW_B > 0) {
+      v = P::colour_own_b(jr, ji);
+      if constexpr (P::N_FLOW_B > P::CHUNK_B) {
+        {
+          double pr[P::CHUNK_A], pi[P::CHUNK_A];
+          JPark<P>::template load<P::CHUNK_A>(tmem, warp - W, 0, pr, pi);
+          v += P::colour_cross_b0(jr, ji, pr, pi);
+        }
+        if constexpr (P::N_FLOW_A > P::CHUNK_A) {
+          double pr[P::N_FLOW_A - P::CHUNK_A], pi[P::N_FLOW_A - P::CHUNK_A];
+          JPark<P>::template load<P::N_FLOW_A - P::CHUNK_A>(tmem, warp - W, P::CHUNK_A, pr, pi);
+          v += P::colour_cross_b1(jr, ji, pr, pi);
+        }
+      }
+    }
+    if (lane >= P::N_HEL_EVAL) v = 0.0;
+    if (role == 1) v_b[ev_w][lane] = v;
+    __syncthreads();
+    if (role == 1) return 0.0;
+    v += v_b[ev_w][lane];
+  }
   if (hel_out && lane < P::N_HEL_EVAL) {  // full index: leg 0 at +1 is bit 0; the parity partner has every helicity flipped
     const int hf = (lane << 1) | 1;
     hel_out[hf] = v * scale;
@@ -158,10 +207,10 @@ __global__ void __launch_bounds__(32 * P::N_WARPS, 1) me_eval_kernel(const doubl
   const long long n_batches = (n_ev + W - 1) / W;
   for (long long b = blockIdx.x; b < n_batches; b += gridDim.x) {
     // events past the end repeat the last one (computed, not stored)
-    const long long ev = min(b * W + warp, n_ev - 1);
+    const long long ev = min(b * W + (warp & (W - 1)), n_ev - 1);
     if ((P::N_WARPS == W || warp < W) && lane < 4 * P::N_EXT) smem[warp * STRIDE + lane] = momenta[ev * (4 * P::N_EXT) + lane];
     __syncthreads();
-    const double r = cta_me2<P>(smem, mass, scale, (me2_hel && b * W + warp < n_ev) ? me2_hel + ev * P::N_HEL : nullptr, tmem);
+    const double r = cta_me2<P>(smem, mass, scale, (me2_hel && b * W + (warp & (W - 1)) < n_ev) ? me2_hel + ev * P::N_HEL : nullptr, tmem);
     if ((P::N_WARPS == W || warp < W) && lane == 0 && me2 && b * W + warp < n_ev) me2[ev] = r;
     __syncthreads();
   }

@@ -155,7 +155,9 @@ ME_HD void acc_term(wf4 (&acc)[ME_NSLOT], const wf4& x, unsigned code, bool wide
   }
 }
 
-// a6: one item for local variant j (0 .. VPI-1) of one event (scratch at sm)
+// a6: one item for local variant j (0 .. VPI-1) of one event (scratch at sm).  PREFETCH: fetch the operands of member
+// i + 1 before member i is evaluated (32 more registers; for CTAs with two warps per scheduler).
+template <bool PREFETCH>
 ME_HD void me_run_item(const MeItem H, const MeMember* __restrict__ members, int j, double* __restrict__ sm, double mass) {
   const int n_mem = H.w0 & 0xff;
   const int nv = (H.w0 >> 16) & 0xff, v = static_cast<int>(H.w0 >> 24) + j;
@@ -167,7 +169,6 @@ ME_HD void me_run_item(const MeItem H, const MeMember* __restrict__ members, int
   for (int s = 0; s < ME_NSLOT; ++s)
     for (int c = 0; c < 4; ++c) acc[s].c[c] = mk(0.0, 0.0);
   const MeMember* m = members + (H.w1 & 0xffff);
-  // the operands of member i + 1 are fetched before member i is evaluated
   unsigned w0 = m->w[0], w2 = m->w[2], w4 = m->w[4];
   wf4 A, B;
   {
@@ -181,7 +182,7 @@ ME_HD void me_run_item(const MeItem H, const MeMember* __restrict__ members, int
   for (int i = 0; i < n_mem; ++i) {
     const unsigned c0 = w0, c2 = w2, c4 = w4;
     const wf4 a = A, b = B;
-    if (i + 1 < n_mem) {
+    if (PREFETCH ? (i + 1 < n_mem) : false) {
       ++m;
       const unsigned w1 = m->w[1], w3 = m->w[3];
       w0 = m->w[0]; w2 = m->w[2]; w4 = m->w[4];
@@ -204,6 +205,13 @@ ME_HD void me_run_item(const MeItem H, const MeMember* __restrict__ members, int
       acc_term(acc, t1, c4 & 0x1ffu, wide);
       acc_term(acc, t2, (c4 >> 9) & 0x1ffu, wide);
       acc_term(acc, t3, (c4 >> 18) & 0x1ffu, wide);
+    }
+    if (!PREFETCH && i + 1 < n_mem) {
+      ++m;
+      const unsigned w1 = m->w[1], w3 = m->w[3];
+      w0 = m->w[0]; w2 = m->w[2]; w4 = m->w[4];
+      A = ld_wf(sm + (w1 & 0xffff) + 2 * ((w3 >> sh) & 15u));
+      B = ld_wf(sm + (w1 >> 16) + 2 * ((w3 >> (16 + sh)) & 15u));
     }
   }
   // the common propagator, once per colour-ordered current

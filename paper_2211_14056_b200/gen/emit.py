@@ -249,6 +249,49 @@ class Layout:
         return {"V": KIND_VEC, "O": KIND_ROW, "I": KIND_COL}[o.type[0]]
 
 
+def split_flows(P, nf):
+    """Two balanced halves of the colour flows such that few U.C contractions feed flows of both halves (those are
+    contracted by both warps of an event).  Pairwise exchange to a local optimum from seeded random starts."""
+    import random
+    if nf < 2:
+        return [0] * nf
+    groups = {}
+    for (f, u, c, z, k) in P.dots:
+        groups.setdefault((u, c), set()).add(f)
+    gl = [tuple(sorted(v)) for v in groups.values()]
+
+    def cost(h):
+        dup, load = 0, [0, 0]
+        for fl in gl:
+            sides = {h[f] for f in fl}
+            dup += len(sides) > 1
+            for x in sides:
+                load[x] += 1
+        return 16 * dup + abs(load[0] - load[1])
+    rng = random.Random(20221114)
+    best = None
+    for trial in range(24 if nf > 6 else 4):
+        h = [0] * ((nf + 1) // 2) + [1] * (nf // 2)
+        if trial:
+            rng.shuffle(h)
+        c = cost(h)
+        improved = True
+        while improved:
+            improved = False
+            for a in range(nf):
+                for b in range(nf):
+                    if h[a] == 0 and h[b] == 1:
+                        h[a], h[b] = 1, 0
+                        c2 = cost(h)
+                        if c2 < c:
+                            c, improved = c2, True
+                        else:
+                            h[a], h[b] = 0, 1
+        if best is None or c < best[0]:
+            best = (c, list(h))
+    return best[1]
+
+
 def pick_rounds(P):
     if N_ROUNDS:
         return Layout(P, N_ROUNDS)
@@ -427,80 +470,126 @@ def emit_process(name, n_rounds=None):
     by_split = {}
     for d in P.dots:
         by_split.setdefault(P.objs[d[1]].legs, []).append(d)
-    amp_flops = 0
+    def emit_dots(fname, keep, local):
+        """dots of the flows in `keep` (global flow -> index into jr/ji given by `local`); returns the flop count"""
+        flops = 0
+        w("  static ME_HD void %s(int r, const double* __restrict__ sm, int h, double* __restrict__ jr, double* __restrict__ ji) {" % fname)
+        for l in range(1, n):
+            w("    const int b%d = (h >> %d) & 1; (void)b%d;" % (l, l - 1, l))
+        w("    switch (r) {")
+        for r, split_list in enumerate(L.rounds):
+            w("      case %d: {" % r)
+            for legs in split_list:
+                dots = [d for d in by_split[legs] if d[0] in keep]
+                if not dots:
+                    continue
+                w("        {  // split %s | rest: %d dot products" % ("".join(str(l) for l in legs), len(dots)))
+                if not DOTS_C_PER_U:
+                    for c in sorted({d[2] for d in dots}):
+                        w("          const wf4 c%d = %s;" % (c, ldw(c)))
+                for u in sorted({d[1] for d in dots}):
+                    w("          { const wf4 u = %s;" % ldw(u))
+                    by_c = {}
+                    for (f, uu, c, z, kind) in dots:
+                        if uu == u:     # the phases i^a of the stored operands go into the dot product's phase
+                            by_c.setdefault((c, kind), []).append((local[f], (zcode[z] + out_phase.get(u, 0) + out_phase.get(c, 0)) % 4))
+                    for (c, kind), fl in sorted(by_c.items()):
+                        mink = "true" if kind == "V" else "false"
+                        if DOTS_C_PER_U:     # one C operand live at a time
+                            w("            { const wf4 c%d = %s;" % (c, ldw(c)))
+                        if len(fl) == 1:
+                            w("            dot_acc<%d, %s>(jr[%d], ji[%d], u, c%d);" % (fl[0][1], mink, fl[0][0], fl[0][0], c))
+                            flops += FLOPS_DOT
+                        else:   # one contraction feeds several colour flows: computed once, added with each flow's phase
+                            w("            { const cplx t = dot_val<%s>(u, c%d);" % (mink, c))
+                            for f, zc in fl:
+                                w("              jadd<%d>(jr[%d], ji[%d], t);" % (zc, f, f))
+                            w("            }")
+                            flops += FLOPS_DOT - 4 + 2 * len(fl)
+                        if DOTS_C_PER_U:
+                            w("            }")
+                    w("          }")
+                w("        }")
+            w("      } break;")
+        w("      default: break;")
+        w("    }")
+        w("  }")
+        return flops
+
     w("  // a7-a8: the dot products of round r for helicity combination h (leg 0 has helicity +1; bit l-1 of h is the")
     w("  // helicity of leg l, 0 <-> -1, 1 <-> +1), accumulated into the colour-flow vector J = (jr, ji).")
-    w("  static ME_HD void dots(int r, const double* __restrict__ sm, int h, double* __restrict__ jr, double* __restrict__ ji) {")
-    for l in range(1, n):
-        w("    const int b%d = (h >> %d) & 1; (void)b%d;" % (l, l - 1, l))
-    w("    switch (r) {")
-    for r, split_list in enumerate(L.rounds):
-        w("      case %d: {" % r)
-        for legs in split_list:
-            dots = by_split[legs]
-            w("        {  // split %s | rest: %d dot products" % ("".join(str(l) for l in legs), len(dots)))
-            if not DOTS_C_PER_U:
-                for c in sorted({d[2] for d in dots}):
-                    w("          const wf4 c%d = %s;" % (c, ldw(c)))
-            for u in sorted({d[1] for d in dots}):
-                w("          { const wf4 u = %s;" % ldw(u))
-                by_c = {}
-                for (f, uu, c, z, kind) in dots:
-                    if uu == u:     # the phases i^a of the stored operands go into the dot product's phase
-                        by_c.setdefault((c, kind), []).append((f, (zcode[z] + out_phase.get(u, 0) + out_phase.get(c, 0)) % 4))
-                for (c, kind), fl in sorted(by_c.items()):
-                    mink = "true" if kind == "V" else "false"
-                    if DOTS_C_PER_U:     # one C operand live at a time (register budget of CTAs with helper warps)
-                        w("            { const wf4 c%d = %s;" % (c, ldw(c)))
-                    if len(fl) == 1:
-                        w("            dot_acc<%d, %s>(jr[%d], ji[%d], u, c%d);" % (fl[0][1], mink, fl[0][0], fl[0][0], c))
-                        amp_flops += FLOPS_DOT
-                    else:   # one contraction feeds several colour flows: computed once, added with each flow's phase
-                        w("            { const cplx t = dot_val<%s>(u, c%d);" % (mink, c))
-                        for f, zc in fl:
-                            w("              jadd<%d>(jr[%d], ji[%d], t);" % (zc, f, f))
-                        w("            }")
-                        amp_flops += FLOPS_DOT - 4 + 2 * len(fl)
-                    if DOTS_C_PER_U:
-                        w("            }")
-                w("          }")
-            w("        }")
-        w("      } break;")
-    w("      default: break;")
-    w("    }")
-    w("  }")
+    amp_flops = emit_dots("dots", set(range(nf)), {f: f for f in range(nf)})
 
     # ---- colour contraction grouped by distinct CF numerator (SURVEY §8(c) E: 9 distinct values for 4 gluons) ----
-    w("  // a9: sum_{f,f'} J_f^* CFnum_{ff'} J_f'  (CF real symmetric, integer numerators over CF_DEN)")
-    w("  static ME_HD double colour(const double* __restrict__ jr, const double* __restrict__ ji) {")
     cf = P.cf_num
-    vals = sorted({int(cf[f, g]) for f in range(nf) for g in range(f, nf)}, key=lambda v: -abs(v))
-    NPART = 2 if nf > 2 else 1
-    nm_of = lambda v: "s%s" % (("m%d" % -v) if v < 0 else str(v))
-    for v in vals:
-        for p in range(NPART):
-            w("    double %s_%d = 0.0;" % (nm_of(v), p))
-    cnt = {v: 0 for v in vals}
-    col_flops = 0
-    for f in range(nf):
-        for g in range(f, nf):
-            v = int(cf[f, g])
-            nm = "%s_%d" % (nm_of(v), cnt[v] % NPART)
-            cnt[v] += 1
-            w("    %s = fma(jr[%d], jr[%d], fma(ji[%d], ji[%d], %s));" % (nm, f, g, f, g, nm))
-            col_flops += 4
-    diag_vals = {int(cf[f, f]) for f in range(nf)}
-    expr = []
-    for v in vals:
-        tot = " + ".join("%s_%d" % (nm_of(v), p) for p in range(NPART))
-        # off-diagonal pairs count twice (CF symmetric); a value on the diagonal must not also be off-diagonal
-        on_diag = v in diag_vals
-        off_diag = any(int(cf[f, g]) == v for f in range(nf) for g in range(f + 1, nf))
-        assert not (on_diag and off_diag), "colour value on and off the diagonal: split the accumulators"
-        expr.append("%d.0 * (%s)" % (v if on_diag else 2 * v, tot))
-        col_flops += 2
-    w("    return " + " + ".join(expr) + ";")
-    w("  }")
+
+    def emit_colour(signature, pairs):
+        """sum over the listed pairs (name_f, name_g, CF numerator, weight 1 (diagonal) | 2) of w CF (re re + im im);
+        name = (array prefix, index).  Returns the flop count."""
+        w("  static ME_HD double %s {" % signature)
+        if not pairs:
+            w("    return 0.0;")
+            w("  }")
+            return 0
+        keys = sorted({(v * wt) for (_, _, v, wt) in pairs}, key=lambda v: -abs(v))
+        NPART = 2 if len(pairs) > 8 else 1
+        nm_of = lambda v: "s%s" % (("m%d" % -v) if v < 0 else str(v))
+        for v in keys:
+            for p in range(NPART):
+                w("    double %s_%d = 0.0;" % (nm_of(v), p))
+        cnt = {v: 0 for v in keys}
+        flops = 0
+        for (fa, ga, v, wt) in pairs:
+            nm = "%s_%d" % (nm_of(v * wt), cnt[v * wt] % NPART)
+            cnt[v * wt] += 1
+            re = lambda a: ("or_[%d]" if a[0] == "o" else "jr[%d]") % a[1]
+            im = lambda a: ("oi[%d]" if a[0] == "o" else "ji[%d]") % a[1]
+            w("    %s = fma(%s, %s, fma(%s, %s, %s));" % (nm, re(fa), re(ga), im(fa), im(ga), nm))
+            flops += 4
+        expr = []
+        for v in keys:
+            expr.append("%d.0 * (%s)" % (v, " + ".join("%s_%d" % (nm_of(v), p) for p in range(NPART))))
+            flops += 2
+        w("    return " + " + ".join(expr) + ";")
+        w("  }")
+        return flops
+
+    w("  // a9: sum_{f,f'} J_f^* CFnum_{ff'} J_f'  (CF real symmetric, integer numerators over CF_DEN)")
+    all_pairs = [(("j", f), ("j", g), int(cf[f, g]), 1 if f == g else 2) for f in range(nf) for g in range(f, nf)]
+    col_flops = emit_colour("colour(const double* __restrict__ jr, const double* __restrict__ ji)", all_pairs)
+
+    # ---- the same for TWO warps per event: each owns half of the colour flows ------------------------------------
+    # (me_kernel.cuh, P::SPLIT_J).  Flows are split so that few U.C contractions feed both halves; warp role A holds
+    # flows FLOWS_A, role B flows FLOWS_B.  J^dagger CF J = pairs inside A + pairs inside B + cross pairs; role A takes
+    # the cross pairs with the first half of B, role B those of its second half with A (read in two chunks).
+    half = split_flows(P, nf)
+    fl_a = [f for f in range(nf) if half[f] == 0]
+    fl_b = [f for f in range(nf) if half[f] == 1]
+    na, nb = len(fl_a), len(fl_b)
+    ha, hb = (na + 1) // 2, (nb + 1) // 2
+    loc = {f: k for k, f in enumerate(fl_a)}
+    loc.update({f: k for k, f in enumerate(fl_b)})
+    w("  static constexpr int N_FLOW_A = %d, N_FLOW_B = %d, N_FLOW_HALF = %d, CHUNK_A = %d, CHUNK_B = %d;" % (na, nb, max(na, nb, 1), ha, hb))
+    w("  // colour flows of warp role A: %s; of role B: %s" % (fl_a, fl_b))
+    flops_a = emit_dots("dots_a", set(fl_a), loc)
+    flops_b = emit_dots("dots_b", set(fl_b), loc)
+    wt = lambda f, g: 1 if f == g else 2
+    own_a = [(("j", loc[f]), ("j", loc[g]), int(cf[f, g]), wt(f, g)) for i, f in enumerate(fl_a) for g in fl_a[i:]]
+    own_b = [(("j", loc[f]), ("j", loc[g]), int(cf[f, g]), wt(f, g)) for i, f in enumerate(fl_b) for g in fl_b[i:]]
+    # o = the other role's chunk, indexed from the chunk's first flow
+    cross_a = [(("j", loc[f]), ("o", loc[g]), int(cf[f, g]), 2) for f in fl_a for g in fl_b[:hb]]
+    cross_b0 = [(("j", loc[g]), ("o", loc[f]), int(cf[f, g]), 2) for g in fl_b[hb:] for f in fl_a[:ha]]
+    cross_b1 = [(("j", loc[g]), ("o", loc[f] - ha), int(cf[f, g]), 2) for g in fl_b[hb:] for f in fl_a[ha:]]
+    two = "const double* __restrict__ jr, const double* __restrict__ ji"
+    four = two + ", const double* __restrict__ or_, const double* __restrict__ oi"
+    fa_ = emit_colour("colour_own_a(%s)" % two, own_a)
+    fb_ = emit_colour("colour_own_b(%s)" % two, own_b)
+    fca = emit_colour("colour_cross_a(%s)" % four, cross_a)
+    fcb0 = emit_colour("colour_cross_b0(%s)" % four, cross_b0)
+    fcb1 = emit_colour("colour_cross_b1(%s)" % four, cross_b1)
+    w("  static constexpr bool SPLIT_J = %s;" % ("true" if N_WARPS == 2 * W_EVENTS else "false"))
+    if N_WARPS == 2 * W_EVENTS:
+        amp_flops, col_flops = flops_a + flops_b, fa_ + fb_ + fca + fcb0 + fcb1
     ext_flops = FLOPS_EXT * 2 * n
     nh = 1 << (n - 1)
     per_event = ext_flops + cur_flops + nh * (amp_flops + col_flops)

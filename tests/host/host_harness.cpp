@@ -31,10 +31,13 @@ DEF_TABLES(gg_ttxgg, GG_TTXGG)
 // items [begin, end) of one stage for ONE event: the device runs them with lanes = (local variant j, event)
 template <class P> void items(double* sm, int begin, int end, double mass) {
   for (int it = begin; it < end; ++it)
-    for (int j = 0; j < 4; ++j) me_run_item(Tables<P>::items()[it], Tables<P>::members(), j, sm, mass);
+    for (int j = 0; j < 4; ++j) {
+      if (it & 1) me_run_item<true>(Tables<P>::items()[it], Tables<P>::members(), j, sm, mass);   // both forms of the member loop
+      else me_run_item<false>(Tables<P>::items()[it], Tables<P>::members(), j, sm, mass);
+    }
 }
 
-template <class P> void eval(const double* mom, double* me2, long long n, double mass, double coupling, double* per_hel) {
+template <class P> void eval(const double* mom, double* me2, long long n, double mass, double coupling, double* per_hel, bool split) {
   std::vector<double> sm(P::SMEM_DOUBLES);
   double g2 = 1;
   for (int i = 0; i < P::COUPLING_POWER; ++i) g2 *= coupling;
@@ -44,17 +47,29 @@ template <class P> void eval(const double* mom, double* me2, long long n, double
       me_phase0(lane, 32, sm.data(), mom + e * 4 * P::N_EXT, P::N_EXT, P::N_SUB, Tables<P>::masks(), Tables<P>::kind(),
                 Tables<P>::massive(), Tables<P>::ext_off(), mass);
     int it = 0;
+    // both forms of the dot / colour stages: one warp per event (J whole) and two warps per event (each half of the flows)
     std::vector<double> jr(P::N_HEL_EVAL * P::N_FLOW, 0.0), ji(P::N_HEL_EVAL * P::N_FLOW, 0.0);
+    constexpr int NH = P::N_FLOW_HALF;
+    std::vector<double> ar(P::N_HEL_EVAL * NH, 0.0), ai(P::N_HEL_EVAL * NH, 0.0), br(P::N_HEL_EVAL * NH, 0.0), bi(P::N_HEL_EVAL * NH, 0.0);
     for (int p = 0; p < P::N_STAGES; ++p) {
       items<P>(sm.data(), it, P::stage_end(p), mass);
       it = P::stage_end(p);
       const int r = P::stage_dots(p);
       if (r >= 0)
-        for (int h = 0; h < P::N_HEL_EVAL; ++h) P::dots(r, sm.data(), h, &jr[h * P::N_FLOW], &ji[h * P::N_FLOW]);
+        for (int h = 0; h < P::N_HEL_EVAL; ++h) {
+          P::dots(r, sm.data(), h, &jr[h * P::N_FLOW], &ji[h * P::N_FLOW]);
+          P::dots_a(r, sm.data(), h, &ar[h * NH], &ai[h * NH]);
+          P::dots_b(r, sm.data(), h, &br[h * NH], &bi[h * NH]);
+        }
     }
     double s = 0;
     for (int h = 0; h < P::N_HEL_EVAL; ++h) {
-      const double v = P::colour(&jr[h * P::N_FLOW], &ji[h * P::N_FLOW]);
+      double v = P::colour(&jr[h * P::N_FLOW], &ji[h * P::N_FLOW]);
+      // role A: pairs inside A + A x (first chunk of B); role B: pairs inside B + (second part of B) x A in two chunks
+      const double* Ar = &ar[h * NH]; const double* Ai = &ai[h * NH]; const double* Br = &br[h * NH]; const double* Bi = &bi[h * NH];
+      const double va = P::colour_own_a(Ar, Ai) + P::colour_cross_a(Ar, Ai, Br, Bi);
+      const double vb = P::colour_own_b(Br, Bi) + P::colour_cross_b0(Br, Bi, Ar, Ai) + P::colour_cross_b1(Br, Bi, Ar + P::CHUNK_A, Ai + P::CHUNK_A);
+      if (split) v = va + vb;
       if (per_hel) per_hel[e * P::N_HEL_EVAL + h] = v * scale;
       s += v;
     }
@@ -62,12 +77,13 @@ template <class P> void eval(const double* mom, double* me2, long long n, double
   }
 }
 
+// split != 0: the two-warps-per-event form of the dot and colour stages (each warp half of the colour flows)
 extern "C" int host_me_eval(const char* proc, const double* mom, double* me2, long long n, double mass, double coupling,
-                            double* per_hel) {
-  if (!strcmp(proc, "epem_mupmum")) eval<epem_mupmum>(mom, me2, n, mass, coupling, per_hel);
-  else if (!strcmp(proc, "gg_ttx")) eval<gg_ttx>(mom, me2, n, mass, coupling, per_hel);
-  else if (!strcmp(proc, "gg_ttxg")) eval<gg_ttxg>(mom, me2, n, mass, coupling, per_hel);
-  else if (!strcmp(proc, "gg_ttxgg")) eval<gg_ttxgg>(mom, me2, n, mass, coupling, per_hel);
+                            double* per_hel, int split) {
+  if (!strcmp(proc, "epem_mupmum")) eval<epem_mupmum>(mom, me2, n, mass, coupling, per_hel, split != 0);
+  else if (!strcmp(proc, "gg_ttx")) eval<gg_ttx>(mom, me2, n, mass, coupling, per_hel, split != 0);
+  else if (!strcmp(proc, "gg_ttxg")) eval<gg_ttxg>(mom, me2, n, mass, coupling, per_hel, split != 0);
+  else if (!strcmp(proc, "gg_ttxgg")) eval<gg_ttxgg>(mom, me2, n, mass, coupling, per_hel, split != 0);
   else return -1;
   return 0;
 }

@@ -22,7 +22,7 @@ def host():
     src = os.path.join(HERE, "host", "host_harness.cpp")
     subprocess.check_call(["g++", "-std=c++17", "-O1", "-shared", "-fPIC", "-o", so, src])
     lib = C.CDLL(so)
-    lib.host_me_eval.argtypes = [C.c_char_p, C.c_void_p, C.c_void_p, C.c_longlong, C.c_double, C.c_double, C.c_void_p]
+    lib.host_me_eval.argtypes = [C.c_char_p, C.c_void_p, C.c_void_p, C.c_longlong, C.c_double, C.c_double, C.c_void_p, C.c_int]
     return lib
 
 
@@ -52,13 +52,15 @@ def test_generator_colour_matrix_golden():
         assert list(P.cf_num[0]) == rows[n][1]
 
 
+@pytest.mark.parametrize("split", [0, 1])
 @pytest.mark.parametrize("cfg,n", [("config0", 64), ("config1", 64), ("config2", 32), ("config3", 12)])
-def test_generated_program_matches_oracle(host, cfg, n):
+def test_generated_program_matches_oracle(host, cfg, n, split):
+    """split = 1: the form with two warps per event, each holding half of the colour flows (me_kernel.cuh, SPLIT_J)."""
     w = BY_NAME[cfg]
     mom = _momenta(cfg, n)
     out = np.empty(n)
     qed = w.process == "epem_mupmum"
     g = np.sqrt(4 * np.pi * (PARAMS["alpha_em"] if qed else PARAMS["alpha_s"]))
-    assert host.host_me_eval(w.process.encode(), mom.ctypes.data, out.ctypes.data, n, 0.0 if qed else PARAMS["m_top"], g, None) == 0
+    assert host.host_me_eval(w.process.encode(), mom.ctypes.data, out.ctypes.data, n, 0.0 if qed else PARAMS["m_top"], g, None, split) == 0
     expect = ref.MatrixElementRef(w.process).eval(mom)
     assert np.max(np.abs(out / expect - 1)) < 1e-11
