@@ -54,7 +54,20 @@ PROCESSES = {
                   Leg(LEG_FB_OUT, "t", True), Leg(LEG_V_OUT, "g", False), Leg(LEG_V_OUT, "g", False)],
                  "gs", 4 * 64 * 2),
 }
-VECTOR_OF = {"t": "g", "e": "a", "mu": "a"}
+# Processes whose diagrams are ENUMERATED only (counts pinned in tests/test_generated_host.py against PAPER.md:57-58 and
+# SURVEY.md §8(f)); no kernels are generated for them: the quark-initiated channels need a colour basis with two open
+# quark lines, g g -> t tbar g g g needs J in tensor memory.
+COUNT_ONLY = {
+    "qqx_ttx": [Leg(LEG_F_IN, "q", False), Leg(LEG_FB_IN, "q", False), Leg(LEG_F_OUT, "t", True), Leg(LEG_FB_OUT, "t", True)],
+    "qg_ttxq": [Leg(LEG_F_IN, "q", False), Leg(LEG_V_IN, "g", False), Leg(LEG_F_OUT, "t", True), Leg(LEG_FB_OUT, "t", True),
+                Leg(LEG_F_OUT, "q", False)],
+}
+_G_OUT = Leg(LEG_V_OUT, "g", False)
+COUNT_ONLY["qqx_ttxg"] = COUNT_ONLY["qqx_ttx"] + [_G_OUT]
+COUNT_ONLY["qqx_ttxgg"] = COUNT_ONLY["qqx_ttx"] + [_G_OUT, _G_OUT]
+COUNT_ONLY["qg_ttxqg"] = COUNT_ONLY["qg_ttxq"] + [_G_OUT]
+COUNT_ONLY["gg_ttxggg"] = PROCESSES["gg_ttxgg"][0] + [_G_OUT]
+VECTOR_OF = {"t": "g", "q": "g", "e": "a", "mu": "a"}
 CUT_ALL = True   # every diagram is the contraction of an open current U with a propagated current C (see _pick_cut)
 
 # ---- SU(3) ---------------------------------------------------------------------------------------------------
@@ -132,9 +145,10 @@ def _set_partitions(items, k):
 class Program:
     """The evaluated-closed-at-centroid diagram list of one process."""
 
-    def __init__(self, name):
+    def __init__(self, name, count_only=False):
+        """count_only: enumerate the diagrams of a COUNT_ONLY process (no colour flows, no factorisation)."""
         self.name = name
-        self.legs, self.coupling, self.avg = PROCESSES[name]
+        self.legs, self.coupling, self.avg = (COUNT_ONLY[name], "gs", 1) if count_only else PROCESSES[name]
         self.n = len(self.legs)
         self.objs = []
         self._memo = {}
@@ -155,6 +169,8 @@ class Program:
                 t = ("I", leg.flavour)
             self._ext[i] = self._new((i,), t, "EXT", (), 1)
         self._close()
+        if count_only:
+            return
         self._colour()
         self.factorise()
 

@@ -39,6 +39,24 @@ def test_generator_counts(name, nd, n4, nt, nf):
     assert (s["n_diagrams"], s["n_diagrams_4g"], s["n_terms"], s["n_flows"]) == (nd, n4, nt, nf)
 
 
+def test_diagram_counts_of_the_hadronic_processes():
+    """PAPER.md:57-58 (Table 1) prints 36 diagrams for p p -> t tbar g and 267 for p p -> t tbar g g.  The generator's own
+    enumeration of every partonic channel reproduces both totals: 36 = 16 (gg) + 4 x 5 (q qbar, qbar q, q g, g q) and
+    267 = 123 + 4 x 36.  Only the gg channels have kernels; the others are enumerated for this pin.
+    g g -> t tbar g g g: 1 240 diagrams, 295 with a four-gluon vertex — 10 of those with two (three
+    external gluons on one, two on the other), hence 945 + 3 x 285 + 9 x 10 = 1 890 colour-pure terms (SURVEY's 1 830
+    counts one vertex each)."""
+    n = lambda name: diagrams.Program(name, count_only=True)
+    counts = {k: n(k).n_diagrams for k in ("qqx_ttx", "qqx_ttxg", "qqx_ttxgg", "qg_ttxq", "qg_ttxqg")}
+    assert counts == {"qqx_ttx": 1, "qqx_ttxg": 5, "qqx_ttxgg": 36, "qg_ttxq": 5, "qg_ttxqg": 36}
+    gg = {k: diagrams.Program(k).summary()["n_diagrams"] for k in ("gg_ttxg", "gg_ttxgg")}
+    assert gg["gg_ttxg"] + 2 * counts["qqx_ttxg"] + 2 * counts["qg_ttxq"] == 36
+    assert gg["gg_ttxgg"] + 2 * counts["qqx_ttxgg"] + 2 * counts["qg_ttxqg"] == 267
+    big = n("gg_ttxggg")
+    assert (big.n_diagrams, big.n_diagrams_4g, len(big.terms)) == (1240, 295, 1890)
+    assert len(big.terms) == (1240 - 295) + 3 * 285 + 9 * 10
+
+
 def test_generator_colour_matrix_golden():
     rows = {}
     for line in open(os.path.join(HERE, "golden", "colour_matrix_rows.txt")):

@@ -32,8 +32,13 @@ def test_default_workload_line():
     assert 0.05 < r["frac"] < 1.0 and r["peak_measured_dfma_chain"] > 20
     c = d["cpu_baseline"]
     assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and "sample" in c
+    assert abs(c["events_per_s_per_core"] * c["cores"] / c["value"] - 1) < 1e-12
     e = d["e2e"]
     assert e["value"] > 0 and e["h2d_bytes_per_step"] > 0 and e["d2h_bytes_per_step"] > 0
+    assert e["events_per_step"] == 262144          # the same events per step as the device-resident number
+    v = d["vegas"]                                  # config 4 beside the headline: 5 iterations from a uniform grid
+    assert len(v["events_per_s_per_iteration"]) == 5 and min(v["events_per_s_per_iteration"]) > 1e6
+    assert v["integral_pb_combined"] > 0 and v["sigma_pb_combined"] > 0 and 0 < v["cut_pass_fraction_last"] <= 1
     assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
 
 
