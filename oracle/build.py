@@ -10,7 +10,7 @@ import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SOURCES = ["oracle_api.cpp", "me_tier0.cpp", "me_tier1.cpp", "me_qed.cpp", "phase_space_ref.cpp", "vegas_ref.cpp"]
+SOURCES = ["oracle_api.cpp", "me_tier0.cpp", "me_tier1.cpp", "me_tier1g.cpp", "me_qed.cpp", "phase_space_ref.cpp", "vegas_ref.cpp"]
 HEADERS = ["algebra.hpp", "wavefunctions.hpp", "process.hpp", "me_ref.hpp", "oracle_ref.h"]
 LIB = os.path.join(HERE, "liboracle_ref.so")
 

@@ -21,7 +21,8 @@ struct Ext {
   Sp sp[NMAX][2];   // fermion legs: u / v-bar / u-bar / v according to LegKind
 };
 
-struct Tier1;  // defined in me_tier1.cpp
+struct Tier1;   // defined in me_tier1.cpp  (one quark line, colour-flow basis)
+struct Tier1G;  // defined in me_tier1g.cpp (any number of lines, diagram basis)
 
 }  // namespace orc
 
@@ -31,7 +32,8 @@ struct me_handle_ref {
   int spin_basis = orc::BASIS_FIXED_AXIS;
   int pol_basis = orc::POL_LINEAR;
   int ward_leg = -1;  // test hook: replace this gluon's polarisation vector by its momentum
-  std::shared_ptr<orc::Tier1> t1;
+  std::shared_ptr<orc::Tier1> t1;    // processes with one quark line
+  std::shared_ptr<orc::Tier1G> t1g;  // processes with two quark lines; built on demand for the others (cross-check)
 };
 
 namespace orc {
@@ -69,6 +71,13 @@ int tier1_n_4g_diagrams(const Tier1& t);
 int tier1_n_flows(const Tier1& t);
 const double* tier1_cf(const Tier1& t);          // [n_flow][n_flow], row-major
 const int* tier1_flow_perms(const Tier1& t);     // [n_flow][n_gluon] leg indices, lexicographic
+// tier 1, diagram basis (me_tier1g.cpp)
+std::shared_ptr<Tier1G> tier1g_build(const Process& P);
+double tier1g_me2(const me_handle_ref& h, const Tier1G& T, const double* mom);
+cd tier1g_amplitude(const me_handle_ref& h, const Tier1G& T, const Ext& E, const int* hel, const int* col);
+int tier1g_n_diagrams(const Tier1G& t);
+int tier1g_n_terms(const Tier1G& t);
+int tier1g_n_4g_diagrams(const Tier1G& t);
 // QED literal (me_qed.cpp)
 double qed_me2(const me_handle_ref& h, const double* mom);
 

@@ -30,7 +30,15 @@ namespace orc {
 
 namespace {
 
-enum CurType { T_GLUON = 0, T_ROW = 1, T_COL = 2 };
+// Type of a current over a leg subset S: a gluon if every fermion line has both or neither of its ends in S, the row
+// (psi-bar side) or column (psi side) spinor of line f if exactly one end of exactly one line is in S, nothing (no such
+// current exists: two different flavours cannot meet at a vertex) otherwise.  Line 0 = top, line 1 = the light quark.
+enum CurType { T_NONE = -1, T_GLUON = 0 };
+inline int t_row(int line) { return 1 + 2 * line; }
+inline int t_col(int line) { return 2 + 2 * line; }
+inline bool is_row(int t) { return t > 0 && (t & 1); }
+inline bool is_col(int t) { return t > 0 && !(t & 1); }
+inline int line_of(int t) { return (t - 1) / 2; }
 
 // A colour-dressed off-shell current.
 //   gluon : c[a][mu], a = 0..7 adjoint colour, mu upper Lorentz index
@@ -50,16 +58,22 @@ struct Ctx {
   const me_handle_ref* h;
   const Ext* E;
   int n;
-  double gs, mq;
-  int ileg_q = -1, ileg_qb = -1;
+  double gs;
+  int row_leg[2] = {-1, -1}, col_leg[2] = {-1, -1};  // the psi-bar end and the psi end of each fermion line
+  double mline[2] = {0, 0};                          // mass of each line
   std::vector<Cur> J;   // propagated currents, index = subset mask over legs (bit i = leg i)
   std::vector<P4> K;    // K_S
   int type_of(unsigned S) const {
-    bool q = ileg_q >= 0 && (S >> ileg_q & 1u), qb = ileg_qb >= 0 && (S >> ileg_qb & 1u);
-    if (q == qb) return T_GLUON;
-    return q ? T_ROW : T_COL;
+    int t = T_GLUON;
+    for (int f = 0; f < 2; ++f) {
+      if (row_leg[f] < 0) continue;
+      const bool r = S >> row_leg[f] & 1u, c = S >> col_leg[f] & 1u;
+      if (r == c) continue;
+      if (t != T_GLUON) return T_NONE;
+      t = r ? t_row(f) : t_col(f);
+    }
+    return t;
   }
-  bool has_pair(unsigned S) const { return ileg_q >= 0 && (S >> ileg_q & 1u) && (S >> ileg_qb & 1u); }
 };
 
 // ggg vertex with legs (A, B, off-shell third leg), all momenta incoming, k3 = -(kA+kB):
@@ -177,6 +191,7 @@ void add_row_col(const Ctx& X, const Cur& R, const Cur& C, Cur& out) {
 void build_B(Ctx& X, unsigned S, Cur& B) {
   const int tS = X.type_of(S);
   B.type = tS; B.set = true; B.zero();
+  if (tS == T_NONE) return;
   const unsigned low = S & (~S + 1u);
   // 2-way splits {A, Bm}; A holds the lowest leg of S so each unordered split appears once
   for (unsigned A = (S - 1) & S; A; A = (A - 1) & S) {
@@ -184,16 +199,17 @@ void build_B(Ctx& X, unsigned S, Cur& B) {
     const unsigned Bm = S & ~A;
     const int tA = X.type_of(A), tB = X.type_of(Bm);
     const Cur &JA = X.J[A], &JB = X.J[Bm];
-    if (tS == T_GLUON) {
+    if (tA == T_NONE || tB == T_NONE) continue;
+    if (tS == T_GLUON) {   // g g -> g, or the two ends of ONE line -> g
       if (tA == T_GLUON && tB == T_GLUON) add_ggg(X, JA, X.K[A], JB, X.K[Bm], B);
-      else if (tA == T_ROW && tB == T_COL) add_row_col(X, JA, JB, B);
-      else if (tA == T_COL && tB == T_ROW) add_row_col(X, JB, JA, B);
-    } else if (tS == T_ROW) {
-      if (tA == T_ROW && tB == T_GLUON && !X.has_pair(Bm)) add_row_g(X, JA, JB, B);
-      else if (tB == T_ROW && tA == T_GLUON && !X.has_pair(A)) add_row_g(X, JB, JA, B);
+      else if (is_row(tA) && is_col(tB) && line_of(tA) == line_of(tB)) add_row_col(X, JA, JB, B);
+      else if (is_col(tA) && is_row(tB) && line_of(tA) == line_of(tB)) add_row_col(X, JB, JA, B);
+    } else if (is_row(tS)) {   // the line's row absorbs a gluon
+      if (tA == tS && tB == T_GLUON) add_row_g(X, JA, JB, B);
+      else if (tB == tS && tA == T_GLUON) add_row_g(X, JB, JA, B);
     } else {
-      if (tA == T_COL && tB == T_GLUON && !X.has_pair(Bm)) add_g_col(X, JB, JA, B);
-      else if (tB == T_COL && tA == T_GLUON && !X.has_pair(A)) add_g_col(X, JA, JB, B);
+      if (tA == tS && tB == T_GLUON) add_g_col(X, JB, JA, B);
+      else if (tB == tS && tA == T_GLUON) add_g_col(X, JA, JB, B);
     }
   }
   // 3-way splits {A, Bm, C}, all gluon-type (4-gluon vertex)
@@ -216,17 +232,20 @@ void build_B(Ctx& X, unsigned S, Cur& B) {
 void propagate(const Ctx& X, unsigned S, const Cur& B, Cur& J) {
   J = B;
   const P4& K = X.K[S];
+  if (B.type == T_NONE) return;
   if (B.type == T_GLUON) {
     const cd pr = cd(0, -1) / mdot(K, K);  // -i / q^2
     for (int a = 0; a < 8; ++a) for (int m = 0; m < 4; ++m) J.c[a][m] = pr * B.c[a][m];
-  } else if (B.type == T_ROW) {
+  } else if (is_row(B.type)) {
     // fermion arrow runs INTO this blob: momentum along the arrow is q = -K_S; row * S(q)
+    const double mq = X.mline[line_of(B.type)];
     const P4 q = (-1.0) * K;
-    const M4 Sq = (cd(0, 1) / (mdot(q, q) - X.mq * X.mq)) * (slash(q) + cd(X.mq) * mident());
+    const M4 Sq = (cd(0, 1) / (mdot(q, q) - mq * mq)) * (slash(q) + cd(mq) * mident());
     for (int j = 0; j < 3; ++j) { Sp r = mul(spn(B, j), Sq); for (int al = 0; al < 4; ++al) J.c[j][al] = r[al]; }
   } else {
     // fermion arrow runs OUT of this blob: q = +K_S; S(q) * column
-    const M4 Sq = (cd(0, 1) / (mdot(K, K) - X.mq * X.mq)) * (slash(K) + cd(X.mq) * mident());
+    const double mq = X.mline[line_of(B.type)];
+    const M4 Sq = (cd(0, 1) / (mdot(K, K) - mq * mq)) * (slash(K) + cd(mq) * mident());
     for (int i = 0; i < 3; ++i) { Sp r = mul(Sq, spn(B, i)); for (int al = 0; al < 4; ++al) J.c[i][al] = r[al]; }
   }
 }
@@ -234,13 +253,15 @@ void propagate(const Ctx& X, unsigned S, const Cur& B, Cur& J) {
 }  // namespace
 
 // i*M for one assignment hel[leg] in {0,1}, col[leg] (gluon 0..7, quark 0..2).  Root = leg 0.
+// Two fermion lines of different flavour (t and q): every diagram has the same two open lines, so
+// there is no relative sign between diagrams from fermion statistics (no exchange diagram exists).
 cd tier0_amplitude(const me_handle_ref& h, const Ext& E, const int* hel, const int* col) {
   const Process& P = h.P;
   Ctx X;
-  X.h = &h; X.E = &E; X.n = P.n_ext; X.gs = P.gs; X.mq = 0;
+  X.h = &h; X.E = &E; X.n = P.n_ext; X.gs = P.gs;
   for (int i = 0; i < P.n_ext; ++i) {
-    if (P.kind[i] == Q_OUT) { X.ileg_q = i; X.mq = P.mass[i]; }
-    if (P.kind[i] == QB_OUT) X.ileg_qb = i;
+    if (is_row_kind(P.kind[i])) { X.row_leg[P.line[i]] = i; X.mline[P.line[i]] = P.mass[i]; }
+    if (is_col_kind(P.kind[i])) X.col_leg[P.line[i]] = i;
   }
   const unsigned full = (1u << P.n_ext) - 1u, rest = full & ~1u;
   X.J.assign(full + 1, Cur());
@@ -252,9 +273,9 @@ cd tier0_amplitude(const me_handle_ref& h, const Ext& E, const int* hel, const i
   for (int i = 1; i < P.n_ext; ++i) {
     Cur& J = X.J[1u << i];
     J.set = true; J.zero();
-    if (P.kind[i] == G_IN || P.kind[i] == G_OUT) { J.type = T_GLUON; for (int m = 0; m < 4; ++m) J.c[col[i]][m] = E.eps[i][hel[i]][m]; }
-    else if (P.kind[i] == Q_OUT) { J.type = T_ROW; for (int m = 0; m < 4; ++m) J.c[col[i]][m] = E.sp[i][hel[i]][m]; }
-    else { J.type = T_COL; for (int m = 0; m < 4; ++m) J.c[col[i]][m] = E.sp[i][hel[i]][m]; }
+    if (is_gluon_kind(P.kind[i])) { J.type = T_GLUON; for (int m = 0; m < 4; ++m) J.c[col[i]][m] = E.eps[i][hel[i]][m]; }
+    else if (is_row_kind(P.kind[i])) { J.type = t_row(P.line[i]); for (int m = 0; m < 4; ++m) J.c[col[i]][m] = E.sp[i][hel[i]][m]; }
+    else { J.type = t_col(P.line[i]); for (int m = 0; m < 4; ++m) J.c[col[i]][m] = E.sp[i][hel[i]][m]; }
   }
   // subsets of the non-root legs in order of size
   for (int sz = 2; sz <= P.n_ext - 1; ++sz)
@@ -263,9 +284,11 @@ cd tier0_amplitude(const me_handle_ref& h, const Ext& E, const int* hel, const i
       Cur B;
       build_B(X, S, B);
       if (S == rest) {
-        // close on the root gluon: sum_a eps^a_mu B^{a mu}
-        const V4 e = E.eps[0][hel[0]];
-        return mdot(e, gl(B, col[0]));
+        // close on the root leg with its wavefunction and its colour: a gluon (eps_mu B^{a mu}), the psi end of a
+        // line (B is that line's row: B[j] u) or its psi-bar end (B is the column: vbar B[i])
+        if (is_gluon_kind(P.kind[0])) return B.type == T_GLUON ? mdot(E.eps[0][hel[0]], gl(B, col[0])) : cd(0);
+        if (is_col_kind(P.kind[0])) return B.type == t_row(P.line[0]) ? dot(spn(B, col[0]), E.sp[0][hel[0]]) : cd(0);
+        return B.type == t_col(P.line[0]) ? dot(E.sp[0][hel[0]], spn(B, col[0])) : cd(0);
       }
       propagate(X, S, B, X.J[S]);
     }

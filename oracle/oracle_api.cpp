@@ -38,7 +38,10 @@ int me_init_ref(const char* process, const me_params_ref* p, me_handle_ref** out
   auto* h = new me_handle_ref();
   h->par = *p;
   if (!make_process(process, *p, h->P)) { delete h; return -2; }
-  if (!h->P.qed) h->t1 = tier1_build(h->P);
+  if (!h->P.qed) {
+    if (h->P.n_lines() > 1) h->t1g = tier1g_build(h->P);   // two quark lines: the diagram basis (me_tier1g.cpp)
+    else h->t1 = tier1_build(h->P);
+  }
   *out = h;
   return 0;
 }
@@ -52,7 +55,28 @@ int me_eval_ref(me_handle_ref* h, const double* momenta, double* me2, long long 
   const int nt = oracle_get_threads_ref();
 #pragma omp parallel for schedule(static) num_threads(nt)
   for (long long e = 0; e < n_ev; ++e)
-    me2[e] = h->P.qed ? qed_me2(*h, momenta + e * stride) : tier1_me2(*h, momenta + e * stride);
+    me2[e] = h->P.qed ? qed_me2(*h, momenta + e * stride)
+                      : (h->t1 ? tier1_me2(*h, momenta + e * stride) : tier1g_me2(*h, *h->t1g, momenta + e * stride));
+  return 0;
+}
+
+// tier 1 in the diagram basis for ANY QCD process (the default of the two-line processes; for the one-line ones a
+// second, independent organisation of the same diagrams that the tests compare with the flow basis)
+int me_eval_diag_ref(me_handle_ref* h, const double* momenta, double* me2, long long n_ev) {
+  if (!h || !momenta || !me2 || n_ev < 0 || h->P.qed) return -1;
+  if (!h->t1g) h->t1g = tier1g_build(h->P);
+  const int stride = 4 * h->P.n_ext;
+  const int nt = oracle_get_threads_ref();
+#pragma omp parallel for schedule(static) num_threads(nt)
+  for (long long e = 0; e < n_ev; ++e) me2[e] = tier1g_me2(*h, *h->t1g, momenta + e * stride);
+  return 0;
+}
+int me_amplitude_diag_ref(me_handle_ref* h, const double* mom, const int* hel, const int* col, double* re_im) {
+  if (!h || h->P.qed) return -1;
+  if (!h->t1g) h->t1g = tier1g_build(h->P);
+  Ext E; build_ext(*h, mom, E);
+  const cd a = tier1g_amplitude(*h, *h->t1g, E, hel, col);
+  re_im[0] = a.real(); re_im[1] = a.imag();
   return 0;
 }
 
@@ -77,23 +101,27 @@ int me_set_ward_leg_ref(me_handle_ref* h, int leg) { if (!h) return -1; h->ward_
 int me_info_ref(const me_handle_ref* h, int what) {
   if (!h) return -1;
   if (h->P.qed) return what == 0 || what == 1 || what == 3 ? 1 : 0;
+  if (what >= 5 && what <= 7 && !h->t1g) return -1;
   switch (what) {
-    case 0: return tier1_n_diagrams(*h->t1);
-    case 1: return tier1_n_terms(*h->t1);
-    case 2: return tier1_n_4g_diagrams(*h->t1);
-    case 3: return tier1_n_flows(*h->t1);
+    case 0: return h->t1 ? tier1_n_diagrams(*h->t1) : tier1g_n_diagrams(*h->t1g);
+    case 1: return h->t1 ? tier1_n_terms(*h->t1) : tier1g_n_terms(*h->t1g);
+    case 2: return h->t1 ? tier1_n_4g_diagrams(*h->t1) : tier1g_n_4g_diagrams(*h->t1g);
+    case 3: return h->t1 ? tier1_n_flows(*h->t1) : 0;   // the diagram basis has no flows
     case 4: return h->P.n_gluon();
+    case 5: return tier1g_n_diagrams(*h->t1g);           // the diagram-basis counts, where it has been built
+    case 6: return tier1g_n_terms(*h->t1g);
+    case 7: return tier1g_n_4g_diagrams(*h->t1g);
   }
   return -1;
 }
 int me_colour_matrix_ref(const me_handle_ref* h, double* cf) {
-  if (!h || !cf || h->P.qed) return -1;
+  if (!h || !cf || h->P.qed || !h->t1) return -1;
   const int nf = tier1_n_flows(*h->t1);
   for (int i = 0; i < nf * nf; ++i) cf[i] = tier1_cf(*h->t1)[i];
   return 0;
 }
 int me_flow_perms_ref(const me_handle_ref* h, int* perms) {
-  if (!h || !perms || h->P.qed) return -1;
+  if (!h || !perms || h->P.qed || !h->t1) return -1;
   const int n = tier1_n_flows(*h->t1) * h->P.n_gluon();
   for (int i = 0; i < n; ++i) perms[i] = tier1_flow_perms(*h->t1)[i];
   return 0;
@@ -106,7 +134,7 @@ int me_amplitude_def_ref(me_handle_ref* h, const double* mom, const int* hel, co
   return 0;
 }
 int me_flows_ref(me_handle_ref* h, const double* mom, const int* hel, double* J) {
-  if (!h || h->P.qed) return -1;
+  if (!h || h->P.qed || !h->t1) return -1;
   Ext E; build_ext(*h, mom, E);
   std::vector<cd> j(tier1_n_flows(*h->t1));
   tier1_flows(*h, E, hel, j.data());

@@ -6,7 +6,9 @@
  * and the two share no source.
  *
  * What each function computes, and from where:
- *   me_eval_ref        tier 1: diagram-by-diagram |M|^2 (SURVEY.md §8(c) tier 1; north_star)
+ *   me_eval_ref        tier 1: diagram-by-diagram |M|^2 (SURVEY.md §8(c) tier 1; north_star): colour-flow basis for the
+ *                      one-quark-line processes (me_tier1.cpp), diagram basis for the quark-initiated channels of
+ *                      SURVEY.md §8(f) N1 / PAPER.md:57-58 (me_tier1g.cpp)
  *   me_eval_def_ref    tier 0: the definition — colour-dressed recursion + brute-force sums
  *   philox/rambo/cuts
  *   vegas_*            SURVEY.md §8(c) G6, G7 (Lepage's Vegas)
@@ -62,10 +64,13 @@ int me_n_external_ref(const me_handle_ref* h);
 int me_n_final_ref(const me_handle_ref* h);
 int me_eval_ref(me_handle_ref* h, const double* momenta, double* me2, long long n_ev);     /* tier 1 */
 int me_eval_def_ref(me_handle_ref* h, const double* momenta, double* me2, long long n_ev); /* tier 0 */
+/* tier 1 in the diagram basis (me_tier1g.cpp): me_eval_ref of the two-quark-line processes; a cross-check for the others */
+int me_eval_diag_ref(me_handle_ref* h, const double* momenta, double* me2, long long n_ev);
+int me_amplitude_diag_ref(me_handle_ref* h, const double* mom, const int* hel, const int* col, double* re_im);
 /* test hooks */
 int me_set_basis_ref(me_handle_ref* h, int spin_basis, int pol_basis);
 int me_set_ward_leg_ref(me_handle_ref* h, int leg); /* -1 = off */
-int me_info_ref(const me_handle_ref* h, int what);  /* 0 n_diag, 1 n_terms, 2 n_diag with 4g, 3 n_flow, 4 n_gluon */
+int me_info_ref(const me_handle_ref* h, int what);  /* 0 n_diag, 1 n_terms, 2 n_diag with 4g, 3 n_flow, 4 n_gluon; 5-7 = 0-2 of the diagram basis */
 int me_colour_matrix_ref(const me_handle_ref* h, double* cf /*[n_flow][n_flow]*/);
 int me_flow_perms_ref(const me_handle_ref* h, int* perms /*[n_flow][n_gluon]*/);
 int me_amplitude_def_ref(me_handle_ref* h, const double* mom, const int* hel, const int* col, double* re_im);

@@ -40,6 +40,8 @@ def lib():
             getattr(_lib, name).argtypes = [C.c_void_p]
         _lib.me_eval_ref.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_longlong]
         _lib.me_eval_def_ref.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_longlong]
+        _lib.me_eval_diag_ref.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_longlong]
+        _lib.me_amplitude_diag_ref.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         _lib.me_set_basis_ref.argtypes = [C.c_void_p, C.c_int, C.c_int]
         _lib.me_set_ward_leg_ref.argtypes = [C.c_void_p, C.c_int]
         _lib.me_info_ref.argtypes = [C.c_void_p, C.c_int]
@@ -127,6 +129,26 @@ class MatrixElementRef:
         rc = lib().me_eval_def_ref(self._h, _p(m), _p(out), n)
         assert rc == 0, rc
         return out
+
+    def eval_diag(self, momenta):
+        """tier 1 in the diagram basis (me_tier1g.cpp)"""
+        m, n = self._mom(momenta)
+        out = np.empty(n)
+        rc = lib().me_eval_diag_ref(self._h, _p(m), _p(out), n)
+        assert rc == 0, rc
+        return out
+
+    def amplitude_diag(self, mom, hel, col):
+        m = _f64(mom).reshape(self.n_external, 4)
+        hel = np.ascontiguousarray(hel, dtype=np.int32)
+        col = np.ascontiguousarray(col, dtype=np.int32)
+        out = np.empty(2)
+        assert lib().me_amplitude_diag_ref(self._h, _p(m), _p(hel), _p(col), _p(out)) == 0
+        return complex(out[0], out[1])
+
+    def info_diag(self):
+        return dict(n_diag=lib().me_info_ref(self._h, 5), n_terms=lib().me_info_ref(self._h, 6),
+                    n_diag_4g=lib().me_info_ref(self._h, 7))
 
     def set_basis(self, spin_basis, pol_basis):
         lib().me_set_basis_ref(self._h, spin_basis, pol_basis)

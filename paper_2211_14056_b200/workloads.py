@@ -6,6 +6,7 @@ sqrt(s), final-state masses, seed, event count, phase-space mode, cuts.
 """
 from collections import namedtuple
 
+# is_gluon: the final-state partons the jet cuts (p_T > ptj_min, Delta R > dr_min) apply to: the massless ones
 Workload = namedtuple("Workload", "name process sqrt_s masses is_gluon seed n_events ps_mode n_dim cuts")
 
 M_TOP = 173.0
@@ -25,6 +26,14 @@ WORKLOADS = [
     # the literal "10-dimensional" reading of configs[4] — hadronic, momentum fractions x1, x2 in front of
     # the 8 RAMBO-on-diet dimensions, a DECLARED toy gluon density (no PDF grids in the container), sqrt(S) = 13 TeV
     Workload("config4_hadronic", "gg_ttxgg", 13000.0, (M_TOP, M_TOP, 0.0, 0.0), (0, 0, 1, 1), 4, 1 << 24, 2, 10, True),
+    # the quark-initiated channels of the paper's hadronic processes p p -> t tbar g (36 = 16 + 4 x 5
+    # diagrams) and p p -> t tbar g g (267 = 123 + 4 x 36), PAPER.md:57-58 (Table 1), as partonic events at fixed sqrt(s)
+    # like configs 1-3; the final light quark of q g -> t tbar q (g) is a jet like the gluons (cuts apply to it)
+    Workload("qqx_ttx", "qqx_ttx", 1000.0, (M_TOP, M_TOP), (0, 0), 11, 1 << 20, 0, 8, False),
+    Workload("qqx_ttxg", "qqx_ttxg", 1000.0, (M_TOP, M_TOP, 0.0), (0, 0, 1), 12, 1 << 20, 0, 12, True),
+    Workload("qg_ttxq", "qg_ttxq", 1000.0, (M_TOP, M_TOP, 0.0), (0, 0, 1), 13, 1 << 20, 0, 12, True),
+    Workload("qqx_ttxgg", "qqx_ttxgg", 1000.0, (M_TOP, M_TOP, 0.0, 0.0), (0, 0, 1, 1), 14, 1 << 22, 0, 16, True),
+    Workload("qg_ttxqg", "qg_ttxqg", 1000.0, (M_TOP, M_TOP, 0.0, 0.0), (0, 0, 1, 1), 15, 1 << 22, 0, 16, True),
 ]
 BY_NAME = {w.name: w for w in WORKLOADS}
 VEGAS_BINS = 50
