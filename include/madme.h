@@ -66,7 +66,10 @@ typedef struct {
 } vegas_result;
 
 /* me_init — select the generated kernel of `process` and fix its parameters.
- * process: "epem_mupmum" (e+ e- -> mu- mu+), "gg_ttx", "gg_ttxg", "gg_ttxgg" (BASELINE.json:configs[0-3]).
+ * process: "epem_mupmum" (e+ e- -> mu- mu+), "gg_ttx", "gg_ttxg", "gg_ttxgg" (BASELINE.json:configs[0-3]), and the
+ * quark-initiated channels of the paper's hadronic processes (Table 1), legs in the
+ * order of the name: "qqx_ttx", "qqx_ttxg", "qqx_ttxgg" (q qbar -> t tbar + 0, 1, 2 gluons) and "qg_ttxq", "qg_ttxqg"
+ * (q g -> t tbar q + 0, 1 gluons); q is one massless flavour.
  * Allocates the handle and the fixed-size device scratch of the Vegas path (reduction partials, the survivor staging
  * of the fused integrand: about 25 MB, independent of the event count). */
 int me_init(const char* process, const me_params* params, me_handle** out);
@@ -107,8 +110,9 @@ int philox_uniform(uint64_t seed, uint64_t iteration, long long first_event, int
 int rambo_generate(const double* rand, double sqrt_s, const double* masses, int n_final, int ps_mode,
                    double* momenta, double* weights, long long n_ev, void* stream);
 
-/* apply_cuts — step a4: pass[ev] = 1 iff every final gluon has pT > ptj_min and DeltaR > dr_min to every
- * other final parton (true rapidity; strict).  is_gluon: HOST [n_final]; pass: dev int32 [n_ev]. */
+/* apply_cuts — step a4: pass[ev] = 1 iff every final jet (gluon; also the massless final quark of q g -> t tbar q (g))
+ * has pT > ptj_min and DeltaR > dr_min to every other final parton (true rapidity; strict).
+ * is_gluon: HOST [n_final], 1 for the jets; pass: dev int32 [n_ev]. */
 int apply_cuts(const double* momenta, int n_final, const int* is_gluon, double ptj_min, double dr_min,
                int* pass, long long n_ev, void* stream);
 

@@ -21,6 +21,13 @@ using namespace orc;
 
 static int g_threads = 0;  // 0 = OpenMP default
 
+// tier 1 of a QCD process: the flow basis (one quark line) or the diagram basis (two lines)
+static double me2_tier1(const me_handle_ref& h, const double* mom) {
+  return h.t1 ? tier1_me2(h, mom) : tier1g_me2(h, *h.t1g, mom);
+}
+// the final-state partons the jet cuts apply to: gluons, and the massless final quark of q g -> t tbar q (g)
+static bool is_jet(const Process& P, int leg) { return P.kind[leg] == G_OUT || (P.kind[leg] == Q_OUT && P.mass[leg] == 0.0); }
+
 extern "C" {
 
 void oracle_set_threads_ref(int n) { g_threads = n; }
@@ -55,8 +62,7 @@ int me_eval_ref(me_handle_ref* h, const double* momenta, double* me2, long long 
   const int nt = oracle_get_threads_ref();
 #pragma omp parallel for schedule(static) num_threads(nt)
   for (long long e = 0; e < n_ev; ++e)
-    me2[e] = h->P.qed ? qed_me2(*h, momenta + e * stride)
-                      : (h->t1 ? tier1_me2(*h, momenta + e * stride) : tier1g_me2(*h, *h->t1g, momenta + e * stride));
+    me2[e] = h->P.qed ? qed_me2(*h, momenta + e * stride) : me2_tier1(*h, momenta + e * stride);
   return 0;
 }
 
@@ -217,7 +223,7 @@ int vegas_integrand_ref(me_handle_ref* h, const vegas_grid_ref* g, double sqrt_s
   if (g->ps_mode < 0 || g->ps_mode > 2) return -4;
   if (D != (g->ps_mode == 0 ? 4 * nf : g->ps_mode == 1 ? 3 * nf - 4 : 3 * nf - 2)) return -4;
   std::vector<double> masses(nf); std::vector<int> isg(nf);
-  for (int i = 0; i < nf; ++i) { masses[i] = h->P.mass[2 + i]; isg[i] = h->P.kind[2 + i] == G_OUT; }
+  for (int i = 0; i < nf; ++i) { masses[i] = h->P.mass[2 + i]; isg[i] = is_jet(h->P, 2 + i); }
   std::vector<double> f(n_ev); std::vector<int> idx(size_t(n_ev) * D);
   const double conv = 0.3893793721e9, flux = 1.0 / (2.0 * sqrt_s * sqrt_s);
   const int nt = oracle_get_threads_ref();
@@ -234,12 +240,12 @@ int vegas_integrand_ref(me_handle_ref* h, const vegas_grid_ref* g, double sqrt_s
       if (rs_hat > msum) {
         const double wps = rambo_event(x + 2, rs_hat, masses.data(), nf, 1, mom);
         if (passes_cuts(mom, nf, isg.data(), h->par.ptj_min, h->par.dr_min))
-          val = jac * toy_gluon_density(x[0]) * toy_gluon_density(x[1]) * wps * tier1_me2(*h, mom) / (2.0 * rs_hat * rs_hat) * conv;
+          val = jac * toy_gluon_density(x[0]) * toy_gluon_density(x[1]) * wps * me2_tier1(*h, mom) / (2.0 * rs_hat * rs_hat) * conv;
       }
     } else {
       const double wps = rambo_event(x, sqrt_s, masses.data(), nf, g->ps_mode, mom);
       if (passes_cuts(mom, nf, isg.data(), h->par.ptj_min, h->par.dr_min))
-        val = jac * wps * tier1_me2(*h, mom) * flux * conv;
+        val = jac * wps * me2_tier1(*h, mom) * flux * conv;
     }
     f[e] = val;
   }

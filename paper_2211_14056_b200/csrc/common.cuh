@@ -24,12 +24,14 @@ inline int cuda_fail(cudaError_t e, const char* where) { return fail(ME_ECUDA, "
     if (e__ != cudaSuccess) return madme::cuda_fail(e__, #call);  \
   } while (0)
 
-enum Proc { P_EPEM = 0, P_GGTT = 1, P_GGTTG = 2, P_GGTTGG = 3 };
+struct ProcOps;
 
 }  // namespace madme
 
 struct me_handle {
-  madme::Proc proc;
+  const madme::ProcOps* ev = nullptr;  // the process's me_eval entry points (proc_eval.cu)
+  const madme::ProcOps* vg = nullptr;  // its fused Vegas integrand (proc_vegas.cu); QCD processes only
+  bool qed = false;
   me_params par;
   int n_ext, n_hel, n_flow, n_diag, n_terms, n_diag4g, n_cur;
   double mass, scale, flops;
@@ -61,9 +63,9 @@ struct ProcOps {
   int (*integrand)(me_handle* h, const VegasArgs& a, double* f, unsigned long long* idx, int words, cudaStream_t s);
 };
 #define MADME_DECLARE_OPS(P) const ProcOps* ops_##P##_eval(); const ProcOps* ops_##P##_vegas();
-MADME_DECLARE_OPS(epem_mupmum)
-MADME_DECLARE_OPS(gg_ttx)
-MADME_DECLARE_OPS(gg_ttxg)
-MADME_DECLARE_OPS(gg_ttxgg)
+// every process of gen/diagrams.py::PROCESSES (build.py compiles proc_eval.cu / proc_vegas.cu once for each)
+#define MADME_FOR_EACH_PROCESS(X) \
+  X(epem_mupmum) X(gg_ttx) X(gg_ttxg) X(gg_ttxgg) X(qqx_ttx) X(qqx_ttxg) X(qg_ttxq) X(qqx_ttxgg) X(qg_ttxqg)
+MADME_FOR_EACH_PROCESS(MADME_DECLARE_OPS)
 
 }  // namespace madme

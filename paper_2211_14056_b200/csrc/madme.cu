@@ -224,7 +224,7 @@ __global__ void vegas_generate_kernel(VegasArgs a, const long long* __restrict__
 }
 
 int check_grid(const me_handle* h, const vegas_grid* g, double sqrt_s, const char* who) {
-  if (h->proc == P_EPEM) return fail(ME_EINVAL, "%s: QCD processes only%s", who);
+  if (h->qed) return fail(ME_EINVAL, "%s: QCD processes only%s", who);
   const int nf = h->n_ext - 2, D = g->n_dim, nb = g->n_bins;
   if (g->ps_mode < 0 || g->ps_mode > 2 || D != (g->ps_mode == 0 ? 4 * nf : g->ps_mode == 1 ? 3 * nf - 4 : 3 * nf - 2))
     return fail(ME_EDIM, "%s: n_dim must be 4 n_final (ps_mode 0), 3 n_final - 4 (1) or 3 n_final - 2 (2)%s", who);
@@ -251,43 +251,33 @@ const char* me_last_error(void) { return g_err; }
 int me_init(const char* process, const me_params* params, me_handle** out) {
   if (!process || !params || !out) return fail(ME_EINVAL, "me_init: null argument%s%s");
   *out = nullptr;
-  Proc pr;
-  if (!strcmp(process, "epem_mupmum")) pr = P_EPEM;
-  else if (!strcmp(process, "gg_ttx")) pr = P_GGTT;
-  else if (!strcmp(process, "gg_ttxg")) pr = P_GGTTG;
-  else if (!strcmp(process, "gg_ttxgg")) pr = P_GGTTGG;
-  else return fail(ME_EPROCESS, "me_init: unknown process '%s'%s", process);
+  struct Entry { const char* name; const ProcOps* (*ev)(); const ProcOps* (*vg)(); };
+#define MADME_ENTRY(P) {#P, ops_##P##_eval, ops_##P##_vegas},
+  static const Entry table[] = {MADME_FOR_EACH_PROCESS(MADME_ENTRY)};
+#undef MADME_ENTRY
+  const Entry* pe = nullptr;
+  for (const Entry& e : table)
+    if (!strcmp(process, e.name)) pe = &e;
+  if (!pe) return fail(ME_EPROCESS, "me_init: unknown process '%s'%s", process);
   if (params->w_top != 0.0) return fail(ME_EINVAL, "me_init: w_top must be 0 (no width in propagators)%s%s");
   if (!have_device()) return fail(ME_ENODEV, "me_init: no CUDA device (this library has no CPU path)%s%s");
   me_handle* h = new me_handle();
   if (cudaGetDevice(&h->device) != cudaSuccess) { delete h; return fail(ME_ECUDA, "me_init: cudaGetDevice failed%s%s"); }
-  h->proc = pr;
+  h->ev = pe->ev();
   h->par = *params;
-  h->mass = (pr == P_EPEM) ? 0.0 : params->m_top;
-  for (int i = 0; i < PS_MAX_FINAL; ++i) h->masses[i] = 0.0;
-  h->gluon_mask = 0;
-  if (pr != P_EPEM) { h->masses[0] = h->masses[1] = params->m_top; }
-  if (pr == P_GGTTG) h->gluon_mask = 0x4;
-  if (pr == P_GGTTGG) h->gluon_mask = 0xC;
-  int rc;
-  switch (pr) {
-    case P_EPEM: rc = ops_epem_mupmum_eval()->fill(h); break;
-    case P_GGTT: rc = ops_gg_ttx_eval()->fill(h); break;
-    case P_GGTTG: rc = ops_gg_ttxg_eval()->fill(h); break;
-    default: rc = ops_gg_ttxgg_eval()->fill(h); break;
-  }
-  if (rc == ME_OK && pr != P_EPEM) {
-    switch (pr) {
-      case P_GGTT: rc = ops_gg_ttx_vegas()->prepare(h); break;
-      case P_GGTTG: rc = ops_gg_ttxg_vegas()->prepare(h); break;
-      default: rc = ops_gg_ttxgg_vegas()->prepare(h); break;
-    }
+  // fill: the constants of the generated program (legs, masses of the final state, which final partons are jets,
+  // coupling and averaging factors) and the launch geometry
+  int rc = h->ev->fill(h);
+  const bool qed = h->qed;
+  if (rc == ME_OK && !qed) {
+    h->vg = pe->vg();
+    rc = h->vg->prepare(h);
   }
   if (rc == ME_OK) {
     // the fixed-size scratch of the Vegas path: sums, reduction partials, survivor staging, unweighting counters
     cudaError_t e = cudaMalloc(&h->sums_d, sizeof(double) * (VEGAS_MAX_OUT + 8));
     if (e == cudaSuccess) e = cudaMallocHost(&h->sums_h, sizeof(double) * 4);
-    if (e == cudaSuccess && pr != P_EPEM) {
+    if (e == cudaSuccess && !qed) {
       h->partial_len = static_cast<long long>(VEGAS_MAX_CHUNKS) * VEGAS_MAX_OUT;
       e = cudaMalloc(&h->partial, sizeof(double) * h->partial_len);
       if (e == cudaSuccess) e = cudaMalloc(&h->vegas_stage, sizeof(double) * h->vegas_stage_len);
@@ -360,12 +350,7 @@ static int eval_common(me_handle* h, const double* momenta, double* me2, double*
   if (!have_device()) return fail(ME_ENODEV, "me_eval: no CUDA device%s%s");
   ON_DEVICE_OF(h);
   cudaStream_t s = static_cast<cudaStream_t>(stream);
-  switch (h->proc) {
-    case P_EPEM: return ops_epem_mupmum_eval()->eval(h, momenta, me2, hel, n_ev, s);
-    case P_GGTT: return ops_gg_ttx_eval()->eval(h, momenta, me2, hel, n_ev, s);
-    case P_GGTTG: return ops_gg_ttxg_eval()->eval(h, momenta, me2, hel, n_ev, s);
-    default: return ops_gg_ttxgg_eval()->eval(h, momenta, me2, hel, n_ev, s);
-  }
+  return h->ev->eval(h, momenta, me2, hel, n_ev, s);
 }
 int me_eval(me_handle* h, const double* momenta, double* me2, long long n_ev, void* stream) {
   if (!me2 && n_ev > 0) return fail(ME_EINVAL, "me_eval: me2 is null%s%s");
@@ -473,11 +458,7 @@ int vegas_integrand(me_handle* h, const vegas_grid* g, double sqrt_s, long long 
   VegasArgs a;
   fill_args(h, g, sqrt_s, first_event, n_ev, a);
   double* f = f_out ? f_out : h->f_scratch;
-  switch (h->proc) {
-    case P_GGTT: rc = ops_gg_ttx_vegas()->integrand(h, a, f, h->idx_scratch, words, s); break;
-    case P_GGTTG: rc = ops_gg_ttxg_vegas()->integrand(h, a, f, h->idx_scratch, words, s); break;
-    default: rc = ops_gg_ttxgg_vegas()->integrand(h, a, f, h->idx_scratch, words, s); break;
-  }
+  rc = h->vg->integrand(h, a, f, h->idx_scratch, words, s);
   if (rc) return rc;
   vegas_reduce_chunks<<<n_chunks, 512, 0, s>>>(f, h->idx_scratch, words, D, nb, n_ev, chunk, h->partial);
   CU(cudaGetLastError());

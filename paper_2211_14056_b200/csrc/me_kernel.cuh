@@ -27,13 +27,9 @@
 
 namespace madme {
 
-#define MADME_UP_epem_mupmum EPEM_MUPMUM
-#define MADME_UP_gg_ttx GG_TTX
-#define MADME_UP_gg_ttxg GG_TTXG
-#define MADME_UP_gg_ttxgg GG_TTXGG
 #define MADME_CAT2_(a, b) a##b
 #define MADME_CAT2(a, b) MADME_CAT2_(a, b)
-#define MADME_TAB(suffix) MADME_CAT2(MADME_CAT2(MADME_UP_, MADME_PROC), suffix)
+#define MADME_TAB(suffix) MADME_CAT2(MADME_PROC, suffix)   // the table macros of generated/<process>.inc: <process>_ITEM_TABLE, ...
 
 // the process's tables: items and members in constant memory (every lane of a warp reads the same entry), the rest
 // in global memory (read once per event by phase 0)

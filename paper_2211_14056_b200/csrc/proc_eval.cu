@@ -36,6 +36,11 @@ int geom(me_handle* h) {
 int fill(me_handle* h) {
   h->n_ext = P::N_EXT; h->n_hel = P::N_HEL; h->n_flow = P::N_FLOW; h->n_diag = P::N_DIAGRAMS;
   h->n_terms = P::N_TERMS; h->n_diag4g = P::N_DIAGRAMS_4G; h->n_cur = P::N_CURRENTS; h->flops = P::FLOPS_PER_EVENT;
+  h->qed = P::QED;
+  h->mass = P::QED ? 0.0 : h->par.m_top;
+  // final-state particle i (leg i + 2): its mass, and whether the jet cuts apply to it (massless coloured partons)
+  for (int i = 0; i < PS_MAX_FINAL; ++i) h->masses[i] = ((P::FINAL_MASSIVE_MASK >> i) & 1) ? h->par.m_top : 0.0;
+  h->gluon_mask = P::JET_MASK;
   const double g2 = P::QED ? 4.0 * PS_PI * h->par.alpha_em : 4.0 * PS_PI * h->par.alpha_s;  // g^2
   double c = 1.0;
   for (int i = 0; i < P::COUPLING_POWER / 2; ++i) c *= g2;

@@ -5,8 +5,8 @@ MadGraph here, so the Feynman diagrams of a process are enumerated directly (SUR
 colour-flow coefficient table is derived numerically from explicit SU(3) tensors.
 It shares no source with oracle/ (which enumerates at run time in C++ with its own data structures).
 
-Model: one fermion line per flavour; vertices {f fbar V, ggg, gggg}; "V" is the gluon for the top line
-and the photon for the lepton lines.
+Model: one fermion line per flavour; vertices {f fbar V, ggg, gggg}; "V" is the gluon for the quark lines (t, and the
+massless q of the quark-initiated channels) and the photon for the lepton lines.
 
 A *diagram* is a tree whose leaves are the external legs.  Every diagram is evaluated "closed" at its
 centroid vertex: the vertex whose hanging subtrees all have <= n/2 leaves (ties — a propagator
@@ -34,6 +34,7 @@ Feynman rules, all momenta incoming:
 """
 import itertools
 from collections import namedtuple
+from fractions import Fraction
 
 import numpy as np
 
@@ -54,19 +55,21 @@ PROCESSES = {
                   Leg(LEG_FB_OUT, "t", True), Leg(LEG_V_OUT, "g", False), Leg(LEG_V_OUT, "g", False)],
                  "gs", 4 * 64 * 2),
 }
-# Processes whose diagrams are ENUMERATED only (counts pinned in tests/test_generated_host.py against PAPER.md:57-58 and
-# SURVEY.md §8(f)); no kernels are generated for them: the quark-initiated channels need a colour basis with two open
-# quark lines, g g -> t tbar g g g needs J in tensor memory.
-COUNT_ONLY = {
-    "qqx_ttx": [Leg(LEG_F_IN, "q", False), Leg(LEG_FB_IN, "q", False), Leg(LEG_F_OUT, "t", True), Leg(LEG_FB_OUT, "t", True)],
-    "qg_ttxq": [Leg(LEG_F_IN, "q", False), Leg(LEG_V_IN, "g", False), Leg(LEG_F_OUT, "t", True), Leg(LEG_FB_OUT, "t", True),
-                Leg(LEG_F_OUT, "q", False)],
-}
+# The quark-initiated channels of the paper's hadronic processes (Table 1: 36 = 16 + 4 x 5 and
+# 267 = 123 + 4 x 36 diagrams): a second quark line q (massless, a flavour different from t).
+# Averages: 1/4 spins x 1/9 (q qbar) or 1/24 (q g) colours x 1/n! for n identical final gluons.
 _G_OUT = Leg(LEG_V_OUT, "g", False)
-COUNT_ONLY["qqx_ttxg"] = COUNT_ONLY["qqx_ttx"] + [_G_OUT]
-COUNT_ONLY["qqx_ttxgg"] = COUNT_ONLY["qqx_ttx"] + [_G_OUT, _G_OUT]
-COUNT_ONLY["qg_ttxqg"] = COUNT_ONLY["qg_ttxq"] + [_G_OUT]
-COUNT_ONLY["gg_ttxggg"] = PROCESSES["gg_ttxgg"][0] + [_G_OUT]
+_QQX = [Leg(LEG_F_IN, "q", False), Leg(LEG_FB_IN, "q", False), Leg(LEG_F_OUT, "t", True), Leg(LEG_FB_OUT, "t", True)]
+_QG = [Leg(LEG_F_IN, "q", False), Leg(LEG_V_IN, "g", False), Leg(LEG_F_OUT, "t", True), Leg(LEG_FB_OUT, "t", True),
+       Leg(LEG_F_OUT, "q", False)]
+PROCESSES["qqx_ttx"] = (_QQX, "gs", 4 * 9)
+PROCESSES["qqx_ttxg"] = (_QQX + [_G_OUT], "gs", 4 * 9)
+PROCESSES["qg_ttxq"] = (_QG, "gs", 4 * 24)
+PROCESSES["qqx_ttxgg"] = (_QQX + [_G_OUT, _G_OUT], "gs", 4 * 9 * 2)
+PROCESSES["qg_ttxqg"] = (_QG + [_G_OUT], "gs", 4 * 24)
+# Processes whose diagrams are ENUMERATED only (counts pinned in tests/test_generated_host.py against SURVEY.md §8(f)
+# N2); no kernels are generated: g g -> t tbar g g g needs J in tensor memory.
+COUNT_ONLY = {"gg_ttxggg": PROCESSES["gg_ttxgg"][0] + [_G_OUT]}
 VECTOR_OF = {"t": "g", "q": "g", "e": "a", "mu": "a"}
 CUT_ALL = True   # every diagram is the contraction of an open current U with a propagated current C (see _pick_cut)
 
@@ -148,7 +151,7 @@ class Program:
     def __init__(self, name, count_only=False):
         """count_only: enumerate the diagrams of a COUNT_ONLY process (no colour flows, no factorisation)."""
         self.name = name
-        self.legs, self.coupling, self.avg = (COUNT_ONLY[name], "gs", 1) if count_only else PROCESSES[name]
+        self.legs, self.coupling, self.avg = (COUNT_ONLY[name], "gs", 1) if name in COUNT_ONLY else PROCESSES[name]
         self.n = len(self.legs)
         self.objs = []
         self._memo = {}
@@ -339,7 +342,7 @@ class Program:
     # -- colour ------------------------------------------------------------------------------------------------
     # colour tensor of an object: (array, labels); labels = external coloured legs it contains + 'out'
     def _coloured(self, leg):
-        return self.legs[leg].flavour in ("g", "t")
+        return self.legs[leg].flavour in ("g", "t", "q")
 
     def _col(self, o):
         if o._col is not None:
@@ -404,54 +407,78 @@ class Program:
             for t in self.terms:
                 t.flows = [(0, complex(np.round(t.phase)))]
             return
-        q = [i for i in col_legs if self.legs[i].kind == LEG_F_OUT][0]
-        qb = [i for i in col_legs if self.legs[i].kind == LEG_FB_OUT][0]
-        perms = list(itertools.permutations(glu))
+        # Colour basis.  Every quark line has a psi-bar end (row index: outgoing quark, incoming
+        # antiquark) and a psi end (column index).  A basis tensor = one string of T's per line,
+        # (T^{a..})_{row end of line k, column end of line pi(k)}, the gluons distributed over the strings in order.
+        # One line: the n! permutations.  Two lines: 2 pairings x (n+1)! ordered distributions; the gluon exchanged
+        # between the lines gives T^a_{ij} T^a_{kl} = (delta_il delta_kj - delta_ij delta_kl / 3) / 2, so the strings
+        # come with 1/2 (crossed pairing) and -1/6 (each line closed on itself): those magnitudes are found below and
+        # absorbed into the basis tensors, so that every diagram enters a flow with a pure phase, as with one line.
+        flavours = sorted({self.legs[i].flavour for i in col_legs if self.legs[i].flavour != "g"}, key=lambda f: f != "t")
+        rows = [[i for i in col_legs if self.legs[i].flavour == f and self.legs[i].kind in (LEG_F_OUT, LEG_FB_IN)][0] for f in flavours]
+        cols = [[i for i in col_legs if self.legs[i].flavour == f and self.legs[i].kind in (LEG_FB_OUT, LEG_F_IN)][0] for f in flavours]
+        nl = len(flavours)
+        assert nl in (1, 2)
+        perms, basis = [], []
+        gl_letter = {g: "abcdefgh"[k] for k, g in enumerate(glu)}
+        for pairing in itertools.permutations(range(nl)):
+            for s in itertools.permutations(glu):
+                for cutpts in itertools.combinations_with_replacement(range(len(s) + 1), nl - 1):
+                    bounds = (0,) + cutpts + (len(s),)
+                    strings = [s[bounds[k]:bounds[k + 1]] for k in range(nl)]
+                    ops, expr_in, lab = [], [], dict(gl_letter)
+                    idx = iter("ijklmnopqrstuvwxyz")
+                    for k in range(nl):
+                        cur = next(idx)
+                        lab[rows[k]] = cur
+                        for g in strings[k]:
+                            nxt = next(idx)
+                            expr_in.append(gl_letter[g] + cur + nxt)
+                            ops.append(_T)
+                            cur = nxt
+                        if strings[k]:
+                            lab[cols[pairing[k]]] = cur
+                        else:       # empty string: delta(row end, column end)
+                            nxt = next(idx)
+                            expr_in.append(cur + nxt)
+                            ops.append(np.eye(3, dtype=complex))
+                            lab[cols[pairing[k]]] = nxt
+                    out = "".join(lab[l] for l in col_legs)
+                    basis.append(np.einsum(",".join(expr_in) + "->" + out, *ops))
+                    perms.append((tuple(pairing), tuple(strings)) if nl > 1 else tuple(s))
         self.flow_perms = perms
-        # basis tensors B_sigma[legs in ascending order] = (T^{a_s1} ... T^{a_sn})_{i j}
-        basis = []
-        for s in perms:
-            # build einsum: chain of T's
-            letters = {g: "abcdefgh"[k] for k, g in enumerate(glu)}
-            idx = "ijklmnopq"
-            expr_in = []
-            for k, g in enumerate(s):
-                expr_in.append(letters[g] + idx[k] + idx[k + 1])
-            lab = {q: idx[0], qb: idx[len(s)]}
-            lab.update(letters)
-            out = "".join(lab[l] for l in col_legs)
-            basis.append(np.einsum(",".join(expr_in) + "->" + out, *[_T] * len(s)))
         nb = len(basis)
         Bm = np.array([b.ravel() for b in basis])
+        cfi0 = np.linalg.inv(Bm.conj() @ Bm.T)
+        arrs = []
+        for t in self.terms:
+            arr, labels = self._term_colour(t)
+            assert labels == col_legs, (labels, col_legs)
+            c = cfi0 @ (Bm.conj() @ arr.ravel())
+            assert np.allclose(Bm.T @ c, arr.ravel(), atol=1e-9), "colour factor outside the flow basis"
+            arrs.append(c)
+        # one magnitude per flow (1 with one line): scale the basis tensor by it
+        mag = np.ones(nb)
+        for f in range(nb):
+            m = sorted({Fraction(abs(c[f])).limit_denominator(1000) for c in arrs if abs(c[f]) > 1e-9})
+            assert len(m) <= 1, "a colour flow receives diagrams with different magnitudes: %s" % m
+            if m:
+                mag[f] = float(m[0])
+        self.flow_scale = mag
+        Bm = Bm * mag[:, None]
         cf = (Bm.conj() @ Bm.T)
         assert np.allclose(cf.imag, 0)
         cf = cf.real
-        den = {2: 3, 3: 9, 4: 54}.get(len(glu), None)
-        if den is None:
-            den = 2 * 3 ** len(glu)
+        den = next(d for d in range(1, 4000) if np.allclose(np.rint(cf * d), cf * d, atol=1e-9))
+        if nl == 1:
+            assert den == {2: 3, 3: 9, 4: 54}.get(len(glu), den)
         num = np.rint(cf * den)
-        assert np.allclose(num, cf * den, atol=1e-9), "colour matrix is not integer/den"
         self.cf_num = num.astype(np.int64)
         self.cf_den = den
         cfi = np.linalg.inv(cf)
         for t in self.terms:
-            ops = [self._col(self.objs[a]) for a in t.args]
-            if t.op == "FFV_AMP":
-                C = self._contract("mcn", _T.transpose(1, 0, 2), ops[0], "m", ops[1], "c", ops[2], "n")
-            elif t.op == "VVV_AMP":
-                C = self._contract("xyz", _F, ops[0], "x", ops[1], "y", ops[2], "z")
-            elif t.op == "DOT_V":   # gluon propagator: delta^{ab}
-                C = self._contract("xy", np.eye(8), ops[0], "x", ops[1], "y")
-            elif t.op == "DOT_F":   # quark propagator: delta_{ij}
-                C = self._contract("xy", np.eye(3), ops[0], "x", ops[1], "y")
-            else:
-                ff = {1: np.einsum("xye,zwe->xyzw", _F, _F), 2: np.einsum("xze,ywe->xyzw", _F, _F),
-                      3: np.einsum("xwe,yze->xyzw", _F, _F)}[t.which]
-                C = self._contract("xyzw", ff, ops[0], "x", ops[1], "y", ops[2], "z", ops[3], "w")
-            arr, labels = C
-            assert labels == col_legs, (labels, col_legs)
-            proj = Bm.conj() @ arr.ravel()
-            c = cfi @ proj
+            arr, _ = self._term_colour(t)
+            c = cfi @ (Bm.conj() @ arr.ravel())
             assert np.allclose(Bm.T @ c, arr.ravel(), atol=1e-9), "colour factor outside the flow basis"
             c = c * t.phase
             flows = []
@@ -462,6 +489,21 @@ class Program:
                 assert abs(z - c[f]) < 1e-9 and abs(z) == 1.0 and (z.real == 0 or z.imag == 0), c[f]
                 flows.append((f, z))
             t.flows = flows
+
+    def _term_colour(self, t):
+        """Colour tensor of a closing term over the external coloured legs (ascending)."""
+        ops = [self._col(self.objs[a]) for a in t.args]
+        if t.op == "FFV_AMP":
+            return self._contract("mcn", _T.transpose(1, 0, 2), ops[0], "m", ops[1], "c", ops[2], "n")
+        if t.op == "VVV_AMP":
+            return self._contract("xyz", _F, ops[0], "x", ops[1], "y", ops[2], "z")
+        if t.op == "DOT_V":   # gluon propagator: delta^{ab}
+            return self._contract("xy", np.eye(8), ops[0], "x", ops[1], "y")
+        if t.op == "DOT_F":   # quark propagator: delta_{ij}
+            return self._contract("xy", np.eye(3), ops[0], "x", ops[1], "y")
+        ff = {1: np.einsum("xye,zwe->xyzw", _F, _F), 2: np.einsum("xze,ywe->xyzw", _F, _F),
+              3: np.einsum("xwe,yze->xyzw", _F, _F)}[t.which]
+        return self._contract("xyzw", ff, ops[0], "x", ops[1], "y", ops[2], "z", ops[3], "w")
 
     # -- propagator-cut closings: colour-ordered combinations -------------------------------------------------
     def _combo(self, members):

@@ -320,8 +320,8 @@ def emit_process(name, n_rounds=None):
     n_tasks = n_units = 0
     sub_i = lambda legs: L.sub_index[legs]
 
-    def massive_of(o):
-        return 1 if (o.type[0] in "OI" and P.legs[[l for l in o.legs if P.legs[l].kind >= 2][0]].massive) else 0
+    def massive_of(o):   # the mass of a fermion current is that of its line (flavour)
+        return 1 if (o.type[0] in "OI" and any(leg.massive for leg in P.legs if leg.flavour == o.type[1])) else 0
 
     out_phase = {}        # stored object id -> a: true current = i^a x stored current
 
@@ -424,6 +424,10 @@ def emit_process(name, n_rounds=None):
     w("  static constexpr int CF_DEN = %d, AVG_DEN = %d, COUPLING_POWER = %d;  // me2 = g^(2*(n-2)) sum / (CF_DEN*AVG_DEN)"
       % (P.cf_den, P.avg, 2 * (n - 2)))
     w("  static constexpr bool QED = %s;" % ("true" if P.coupling == "ee" else "false"))
+    w("  // final-state particle i = leg i + 2: massive (m_top), a jet (massless coloured parton: the cuts apply to it)")
+    w("  static constexpr unsigned FINAL_MASSIVE_MASK = %d, JET_MASK = %d;"
+      % (sum(1 << (l - 2) for l in range(2, n) if P.legs[l].massive),
+         sum(1 << (l - 2) for l in range(2, n) if not P.legs[l].massive and P.legs[l].flavour in ("g", "q"))))
 
     def table_fn(fname, vals):
         w("  static ME_HD int %s(int i) {" % fname)
@@ -441,11 +445,11 @@ def emit_process(name, n_rounds=None):
     w("  // stage_dots(p) (if >= 0), barrier")
     table_fn("stage_end", stage_end)
     table_fn("stage_dots", stage_dots)
-    w("#define %s_ITEM_TABLE { \\" % name.upper())
+    w("#define %s_ITEM_TABLE { \\" % name)
     for r4 in items:
         w("  {%du,%du,%du,%du}, \\" % r4)
     w("  {0u,0u,0u,0u} }")
-    w("#define %s_MEMBER_TABLE { \\" % name.upper())
+    w("#define %s_MEMBER_TABLE { \\" % name)
     for r8 in members:
         w("  {{%du,%du,%du,%du,%du,%du,%du,%du}}, \\" % r8)
     w("  {{0u,0u,0u,0u,0u,0u,0u,0u}} }")
@@ -453,12 +457,12 @@ def emit_process(name, n_rounds=None):
     for o in L.stored:
         if o.op != "EXT" and o.prop:
             sub_flags[o.legs] |= 1 | (2 * massive_of(o))
-    w("#define %s_SUB_MASKS { %s }" % (name.upper(), ",".join(str(sum(1 << l for l in sub) | (sub_flags[sub] << 16)) for sub in L.subsets)))
-    w("#define %s_LEG_KIND { %s }" % (name.upper(), ",".join(str(leg.kind) for leg in P.legs)))
-    w("#define %s_LEG_MASSIVE { %s }" % (name.upper(), ",".join("1" if leg.massive else "0" for leg in P.legs)))
+    w("#define %s_SUB_MASKS { %s }" % (name, ",".join(str(sum(1 << l for l in sub) | (sub_flags[sub] << 16)) for sub in L.subsets)))
+    w("#define %s_LEG_KIND { %s }" % (name, ",".join(str(leg.kind) for leg in P.legs)))
+    w("#define %s_LEG_MASSIVE { %s }" % (name, ",".join("1" if leg.massive else "0" for leg in P.legs)))
     ext_off = [L.off[o.id] for o in L.objs if o.op == "EXT"]
     assert [o.legs[0] for o in L.objs if o.op == "EXT"] == list(range(n))
-    w("#define %s_EXT_OFF { %s }" % (name.upper(), ",".join(str(x) for x in ext_off)))
+    w("#define %s_EXT_OFF { %s }" % (name, ",".join(str(x) for x in ext_off)))
 
     # ---- dots, round by round ----------------------------------------------------------------------------------
     def ldw(oid):

@@ -10,12 +10,17 @@
 #include "../../paper_2211_14056_b200/csrc/generated/gg_ttx.inc"
 #include "../../paper_2211_14056_b200/csrc/generated/gg_ttxg.inc"
 #include "../../paper_2211_14056_b200/csrc/generated/gg_ttxgg.inc"
+#include "../../paper_2211_14056_b200/csrc/generated/qqx_ttx.inc"
+#include "../../paper_2211_14056_b200/csrc/generated/qqx_ttxg.inc"
+#include "../../paper_2211_14056_b200/csrc/generated/qg_ttxq.inc"
+#include "../../paper_2211_14056_b200/csrc/generated/qqx_ttxgg.inc"
+#include "../../paper_2211_14056_b200/csrc/generated/qg_ttxqg.inc"
 
 using namespace madme;
 
 template <class P> struct Tables;
-#define DEF_TABLES(P, U)                                        \
-  template <> struct Tables<P> {                                \
+#define DEF_TABLES(U)                                           \
+  template <> struct Tables<U> {                                \
     static const MeItem* items() { static const MeItem t[] = U##_ITEM_TABLE; return t; }        \
     static const MeMember* members() { static const MeMember t[] = U##_MEMBER_TABLE; return t; } \
     static const int* masks() { static const int t[] = U##_SUB_MASKS; return t; }       \
@@ -23,10 +28,8 @@ template <class P> struct Tables;
     static const int* massive() { static const int t[] = U##_LEG_MASSIVE; return t; }   \
     static const int* ext_off() { static const int t[] = U##_EXT_OFF; return t; }       \
   };
-DEF_TABLES(epem_mupmum, EPEM_MUPMUM)
-DEF_TABLES(gg_ttx, GG_TTX)
-DEF_TABLES(gg_ttxg, GG_TTXG)
-DEF_TABLES(gg_ttxgg, GG_TTXGG)
+#define FOR_EACH_PROCESS(X) X(epem_mupmum) X(gg_ttx) X(gg_ttxg) X(gg_ttxgg) X(qqx_ttx) X(qqx_ttxg) X(qg_ttxq) X(qqx_ttxgg) X(qg_ttxqg)
+FOR_EACH_PROCESS(DEF_TABLES)
 
 // items [begin, end) of one stage for ONE event: the device runs them with lanes = (local variant j, event)
 template <class P> void items(double* sm, int begin, int end, double mass) {
@@ -80,10 +83,8 @@ template <class P> void eval(const double* mom, double* me2, long long n, double
 // split != 0: the two-warps-per-event form of the dot and colour stages (each warp half of the colour flows)
 extern "C" int host_me_eval(const char* proc, const double* mom, double* me2, long long n, double mass, double coupling,
                             double* per_hel, int split) {
-  if (!strcmp(proc, "epem_mupmum")) eval<epem_mupmum>(mom, me2, n, mass, coupling, per_hel, split != 0);
-  else if (!strcmp(proc, "gg_ttx")) eval<gg_ttx>(mom, me2, n, mass, coupling, per_hel, split != 0);
-  else if (!strcmp(proc, "gg_ttxg")) eval<gg_ttxg>(mom, me2, n, mass, coupling, per_hel, split != 0);
-  else if (!strcmp(proc, "gg_ttxgg")) eval<gg_ttxgg>(mom, me2, n, mass, coupling, per_hel, split != 0);
-  else return -1;
-  return 0;
+#define TRY(P) if (!strcmp(proc, #P)) { eval<P>(mom, me2, n, mass, coupling, per_hel, split != 0); return 0; }
+  FOR_EACH_PROCESS(TRY)
+#undef TRY
+  return -1;
 }

@@ -42,12 +42,19 @@ def test_generator_counts(name, nd, n4, nt, nf):
 def test_diagram_counts_of_the_hadronic_processes():
     """PAPER.md:57-58 (Table 1) prints 36 diagrams for p p -> t tbar g and 267 for p p -> t tbar g g.  The generator's own
     enumeration of every partonic channel reproduces both totals: 36 = 16 (gg) + 4 x 5 (q qbar, qbar q, q g, g q) and
-    267 = 123 + 4 x 36.  Only the gg channels have kernels; the others are enumerated for this pin.
+    267 = 123 + 4 x 36 (tests/golden/diagram_counts_quark_channels.txt: diagrams, with a four-gluon vertex, terms).
     g g -> t tbar g g g: 1 240 diagrams, 295 with a four-gluon vertex — 10 of those with two (three
     external gluons on one, two on the other), hence 945 + 3 x 285 + 9 x 10 = 1 890 colour-pure terms (SURVEY's 1 830
     counts one vertex each)."""
     n = lambda name: diagrams.Program(name, count_only=True)
-    counts = {k: n(k).n_diagrams for k in ("qqx_ttx", "qqx_ttxg", "qqx_ttxgg", "qg_ttxq", "qg_ttxqg")}
+    counts = {}
+    for line in open(os.path.join(HERE, "golden", "diagram_counts_quark_channels.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        proc, nd, n4, nt = [x.strip() for x in line.split("|")]
+        s = diagrams.Program(proc).summary()
+        assert (s["n_diagrams"], s["n_diagrams_4g"], s["n_terms"]) == (int(nd), int(n4), int(nt))
+        counts[proc] = s["n_diagrams"]
     assert counts == {"qqx_ttx": 1, "qqx_ttxg": 5, "qqx_ttxgg": 36, "qg_ttxq": 5, "qg_ttxqg": 36}
     gg = {k: diagrams.Program(k).summary()["n_diagrams"] for k in ("gg_ttxg", "gg_ttxgg")}
     assert gg["gg_ttxg"] + 2 * counts["qqx_ttxg"] + 2 * counts["qg_ttxq"] == 36
@@ -71,7 +78,8 @@ def test_generator_colour_matrix_golden():
 
 
 @pytest.mark.parametrize("split", [0, 1])
-@pytest.mark.parametrize("cfg,n", [("config0", 64), ("config1", 64), ("config2", 32), ("config3", 12)])
+@pytest.mark.parametrize("cfg,n", [("config0", 64), ("config1", 64), ("config2", 32), ("config3", 12), ("qqx_ttx", 64),
+                                   ("qqx_ttxg", 32), ("qg_ttxq", 32), ("qqx_ttxgg", 16), ("qg_ttxqg", 16)])
 def test_generated_program_matches_oracle(host, cfg, n, split):
     """split = 1: the form with two warps per event, each holding half of the colour flows (me_kernel.cuh, SPLIT_J)."""
     w = BY_NAME[cfg]
