@@ -48,17 +48,17 @@ template <class P> struct EventSmem {
   static constexpr int DOUBLES = ((RAW + 13) / 16) * 16 + 2;
 };
 
-constexpr int ME_W = 8;  // events per CTA (gen/emit.py::W_EVENTS: the item tables are laid out for it); a CTA has P::N_WARPS >= ME_W
-                         // warps: all of them run items, the first ME_W own one event each in the dot stages
+// Events per CTA: P::W_EVENTS (gen/emit.py: the item tables are laid out for it; 8, or 4 for g g -> t tbar g g g).  A CTA
+// has P::N_WARPS >= W_EVENTS warps: all of them run items, the first W_EVENTS own one event each in the dot stages.
 
 // J in tensor memory: warp w owns TMEM lanes 32 (w % 4) .. +31 and the column block w / 4 (REGS columns: 4 per colour
 // flow it holds).  With P::SPLIT_J an event has TWO warps (w and w + 8, same lanes, neighbouring blocks), each holding
 // the flows of one half; the halves meet once, for J^dagger CF J, by reading the partner's block.
 template <class P> struct JPark {
   static constexpr int NFW = P::SPLIT_J ? P::N_FLOW_HALF : P::N_FLOW;   // flows per warp
-  static constexpr bool ON = P::N_ROUNDS > 1 || P::SPLIT_J;
+  static constexpr bool ON = P::N_ROUNDS > 1 || P::SPLIT_J || P::CHUNKED;
   static constexpr int REGS = 4 * NFW;                             // 32-bit columns per warp
-  static constexpr int COLS = tmem_cols((P::N_WARPS / 4) * REGS);  // allocation: a power of two >= 32
+  static constexpr int COLS = tmem_cols(P::CHUNKED ? REGS : (P::N_WARPS / 4) * REGS);  // allocation: a power of two >= 32
   static __device__ __forceinline__ uint32_t addr(uint32_t base, int warp) {
     return base + (static_cast<uint32_t>(32 * (warp & 3)) << 16) + (warp >> 2) * REGS;
   }
@@ -86,10 +86,15 @@ template <class P> struct JPark {
 // |M|^2 of the 8 events whose momenta sit at the head of each event slice ([n_ext][4]).  Returns, on every lane of
 // warp w < 8, the helicity- and colour-summed, averaged value of event w.  hel_out (optional, global [N_HEL], per warp)
 // receives each helicity combination's share.  tmem: base address of the CTA's tensor-memory allocation.
+template <class P> __device__ __forceinline__ double cta_me2_chunked(double* smem, double mass, double scale, double* hel_out, uint32_t tmem);
+
 template <class P>
 __device__ __forceinline__ double cta_me2(double* smem, double mass, double scale, double* hel_out, uint32_t tmem) {
+  if constexpr (P::CHUNKED) {
+    return cta_me2_chunked<P>(smem, mass, scale, hel_out, tmem);
+  } else {
   constexpr int STRIDE = EventSmem<P>::DOUBLES;
-  constexpr int W = ME_W;
+  constexpr int W = P::W_EVENTS;
   constexpr bool SPLIT = P::SPLIT_J;
   static_assert(!SPLIT || P::N_WARPS == 2 * W, "two warps per event");
   // the warp index through a shuffle: the compiler then knows it is warp-uniform, so the item loop (table reads, op
@@ -100,11 +105,12 @@ __device__ __forceinline__ double cta_me2(double* smem, double mass, double scal
   {
     const int t = threadIdx.x, ev = t % W;
     double* mom_s = smem + ev * STRIDE;
-    me_phase0(t / W, 4 * P::N_WARPS, mom_s + 4 * P::N_EXT, mom_s, P::N_EXT, P::N_SUB, d_masks, d_kind, d_massive, d_extoff, mass);
+    me_phase0(t / W, 32 * P::N_WARPS / W, mom_s + 4 * P::N_EXT, mom_s, P::N_EXT, P::N_SUB, d_masks, d_kind, d_massive, d_extoff, mass);
   }
   __syncthreads();
   double* base = smem + 4 * P::N_EXT;  // event e's scratch = base + e * STRIDE
   static_assert(P::N_HEL_EVAL <= 32, "one helicity combination per lane");
+  static_assert(P::VPI == 4 && P::N_PASS == 1, "the register-resident form is laid out for eight events per CTA");
   constexpr int NFW = JPark<P>::NFW;
   double jr[NFW], ji[NFW];
   const double* my = base + ev_w * STRIDE;
@@ -189,15 +195,125 @@ __device__ __forceinline__ double cta_me2(double* smem, double mass, double scal
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
   return 2.0 * v * scale;
+  }
 }
 
-// 8 events per CTA (blockDim.x = 32 P::N_WARPS); persistent grid, batches of 8 consecutive events.
+// The same for a process whose colour-flow vector does not fit a lane's registers (g g -> t tbar g g g: 120 flows; SURVEY.md
+// §8(f) N2).  The event is evaluated in P::N_PASS passes with the helicities of the frozen legs fixed, so that a lane still
+// holds one helicity combination; J of a pass lives in TENSOR MEMORY (4 N_FLOW 32-bit columns of the warp's 32 lanes) and
+// the dot stages load, update and store it P::CHUNK flows at a time; J^dagger CF J is summed over pairs of chunks.
+// Items: the 32 lanes are W_EVENTS events x VPI helicity variants (lane = event * VPI + variant: the lanes of one event
+// read one 128-byte line).
+template <class P>
+__device__ __forceinline__ double cta_me2_chunked(double* smem, double mass, double scale, double* hel_out, uint32_t tmem) {
+  constexpr int STRIDE = EventSmem<P>::DOUBLES;
+  constexpr int W = P::W_EVENTS, VPI = P::VPI, CH = P::CHUNK, NC = P::N_CHUNK;
+  static_assert(W * VPI == 32 && W <= 4 && P::N_HEL_EVAL <= 32 && 4 * CH * NC <= 512, "one event per tensor-memory sub-partition");
+  const int lane = threadIdx.x & 31, warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
+  double* base = smem + 4 * P::N_EXT;
+  const double* my = base + (warp & (W - 1)) * STRIDE;
+  double* sm_e = base + (lane / VPI) * STRIDE;
+  const int j = lane % VPI;
+  const bool dot_warp = warp < W;
+  const uint32_t tj = tmem + (static_cast<uint32_t>(32 * (warp & 3)) << 16);   // this warp's lanes, column 0
+  double v = 0.0;
+#pragma unroll 1
+  for (int pass = 0; pass < P::N_PASS; ++pass) {
+    {
+      const int t = threadIdx.x, ev = t % W;
+      double* mom_s = smem + ev * STRIDE;
+      me_phase0(t / W, 32 * P::N_WARPS / W, mom_s + 4 * P::N_EXT, mom_s, P::N_EXT, P::N_SUB, d_masks, d_kind, d_massive, d_extoff, mass,
+                P::FROZEN_MASK, P::frozen_helicities(pass));
+    }
+    if (dot_warp) {   // J = 0
+      uint32_t z[4 * CH];
+#pragma unroll
+      for (int k = 0; k < 4 * CH; ++k) z[k] = 0u;
+#pragma unroll 1
+      for (int c = 0; c < NC; ++c) tmem_store<4 * CH>(tj + 4 * CH * c, z);
+    }
+    __syncthreads();
+    int it = 0;
+#pragma unroll 1
+    for (int p = 0; p < P::N_STAGES; ++p) {
+      const int end = P::stage_end(p);
+#pragma unroll 1
+      for (int i = it + warp; i < end; i += P::N_WARPS) me_run_item<true, VPI>(c_items[i], c_members, j, sm_e, mass);
+      it = end;
+      __syncthreads();
+      const int r = P::stage_dots(p);
+      if (r >= 0) {
+        if (dot_warp) {
+#pragma unroll 1
+          for (int c = 0; c < NC; ++c) {
+            if (!P::has_dots(r, c)) continue;
+            double jr[CH], ji[CH];
+            {
+              uint32_t q[4 * CH];
+              tmem_load<4 * CH>(tj + 4 * CH * c, q);
+#pragma unroll
+              for (int f = 0; f < CH; ++f) { jr[f] = __hiloint2double(q[4 * f + 1], q[4 * f]); ji[f] = __hiloint2double(q[4 * f + 3], q[4 * f + 2]); }
+            }
+            if (lane < P::N_HEL_EVAL) P::dots(r, c, my, lane, jr, ji);
+            {
+              uint32_t q[4 * CH];
+#pragma unroll
+              for (int f = 0; f < CH; ++f) {
+                q[4 * f] = __double2loint(jr[f]); q[4 * f + 1] = __double2hiint(jr[f]);
+                q[4 * f + 2] = __double2loint(ji[f]); q[4 * f + 3] = __double2hiint(ji[f]);
+              }
+              tmem_store<4 * CH>(tj + 4 * CH * c, q);
+            }
+          }
+        }
+        __syncthreads();   // the next round's items (or the next pass) overwrite the round region
+      }
+    }
+    // a9, a10: J^dagger CF J over chunks and pairs of chunks; this pass's helicities
+    if (dot_warp) {
+      double vp = 0.0;
+#pragma unroll 1
+      for (int ca = 0; ca < NC; ++ca) {
+        double ar[CH], ai[CH];
+        {
+          uint32_t q[4 * CH];
+          tmem_load<4 * CH>(tj + 4 * CH * ca, q);
+#pragma unroll
+          for (int f = 0; f < CH; ++f) { ar[f] = __hiloint2double(q[4 * f + 1], q[4 * f]); ai[f] = __hiloint2double(q[4 * f + 3], q[4 * f + 2]); }
+        }
+        vp += P::colour_diag(ca, ar, ai);
+#pragma unroll 1
+        for (int cb = ca + 1; cb < NC; ++cb) {
+          double br[CH], bi[CH];
+          uint32_t q[4 * CH];
+          tmem_load<4 * CH>(tj + 4 * CH * cb, q);
+#pragma unroll
+          for (int f = 0; f < CH; ++f) { br[f] = __hiloint2double(q[4 * f + 1], q[4 * f]); bi[f] = __hiloint2double(q[4 * f + 3], q[4 * f + 2]); }
+          vp += P::colour_pair(ca, cb, ar, ai, br, bi);
+        }
+      }
+      if (lane >= P::N_HEL_EVAL) vp = 0.0;
+      if (hel_out && lane < P::N_HEL_EVAL) {   // the parity partner has every helicity flipped
+        const int hf = P::full_helicity(lane, pass);
+        hel_out[hf] = vp * scale;
+        hel_out[(P::N_HEL - 1) ^ hf] = vp * scale;
+      }
+      v += vp;
+    }
+  }
+  if (!dot_warp) return 0.0;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return 2.0 * v * scale;
+}
+
+// W_EVENTS events per CTA (blockDim.x = 32 P::N_WARPS); persistent grid, batches of W_EVENTS consecutive events.
 template <class P>
 __global__ void __launch_bounds__(32 * P::N_WARPS, 1) me_eval_kernel(const double* __restrict__ momenta, double* __restrict__ me2,
                                                               double* __restrict__ me2_hel, long long n_ev, double mass, double scale) {
   extern __shared__ __align__(16) double smem[];
   constexpr int STRIDE = EventSmem<P>::DOUBLES;
-  constexpr int W = ME_W;
+  constexpr int W = P::W_EVENTS;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t tmem = JPark<P>::ON ? tmem_alloc<JPark<P>::COLS>() : 0u;
   const long long n_batches = (n_ev + W - 1) / W;

@@ -84,8 +84,11 @@ ME_HD vec4 ld_k(const double* p) {
 // physical momenta; legs 0,1 incoming.  sub_masks[s] = bitmask of legs of subset s (block s at sm + 8 s) | flags << 16:
 // flag 1 = some propagated current lives on S (the denominator is needed), flag 2 = that line is massive.
 // Work items idx, idx + step, ... (subsets, then legs) of ONE event.
+// frozen_mask: legs whose helicity is fixed (leg 0 by parity; more for processes evaluated in passes); their fixed
+// helicities are the bits of frozen_hel at the leg positions, and only that wavefunction is stored.
 ME_HD void me_phase0(int idx, int step, double* sm, const double* mom, int n_ext, int n_sub, const int* sub_masks,
-                     const int* leg_kind, const int* leg_massive, const int* ext_off, double mass) {
+                     const int* leg_kind, const int* leg_massive, const int* ext_off, double mass,
+                     unsigned frozen_mask = 1u, unsigned frozen_hel = 1u) {
   // rolled: this runs once per event and must not crowd the instruction cache of the item and dot stages
 #if defined(__CUDA_ARCH__)
 #pragma unroll 1
@@ -111,8 +114,8 @@ ME_HD void me_phase0(int idx, int step, double* sm, const double* mom, int n_ext
   for (int l = idx; l < n_ext; l += step) {
     wf4 w[2];
     external_wavefunction(leg_kind[l], mom + 4 * l, leg_massive[l] ? mass : 0.0, w);
-    if (l == 0) {
-      st_wf(sm + ext_off[0], w[1]);  // leg 0: helicity +1 only (parity)
+    if ((frozen_mask >> l) & 1u) {
+      st_wf(sm + ext_off[l], w[(frozen_hel >> l) & 1u]);  // one helicity only (leg 0: +1, parity)
     } else {
       st_wf(sm + ext_off[l], w[0]);
       st_wf(sm + ext_off[l] + 2, w[1]);
@@ -157,37 +160,46 @@ ME_HD void acc_term(wf4 (&acc)[ME_NSLOT], const wf4& x, unsigned code, bool wide
 
 // a6: one item for local variant j (0 .. VPI-1) of one event (scratch at sm).  PREFETCH: fetch the operands of member
 // i + 1 before member i is evaluated (32 more registers; for CTAs with two warps per scheduler).
-template <bool PREFETCH>
+// double offset of helicity variant v inside a stored object (gen/emit.py::voff): 16-byte slots of a 128-byte line; an
+// object with 16 variants continues in the next group of four lines
+// (VPI = 4, eight events per CTA: the generator asserts that no object has more than 8 variants, so this is 2 v)
+template <int VPI> ME_HD int me_voff(unsigned v) { return VPI == 4 ? static_cast<int>(2u * v) : static_cast<int>(2u * (v & 7u) + 64u * (v >> 3)); }
+// the variant of an argument that enters local variant j of the item: 4-bit entries; VPI = 4: a and b share word 3, c
+// sits in the high half of word 2; VPI = 8: words 3, 5, 6
+template <int VPI> ME_HD unsigned me_vmap_a(const MeMember* m, int j) { return VPI == 4 ? (m->w[3] >> (4 * j)) & 15u : (m->w[3] >> (4 * j)) & 15u; }
+template <int VPI> ME_HD unsigned me_vmap_b(const MeMember* m, int j) { return VPI == 4 ? (m->w[3] >> (16 + 4 * j)) & 15u : (m->w[5] >> (4 * j)) & 15u; }
+template <int VPI> ME_HD unsigned me_vmap_c(const MeMember* m, int j) { return VPI == 4 ? (m->w[2] >> (16 + 4 * j)) & 15u : (m->w[6] >> (4 * j)) & 15u; }
+
+template <bool PREFETCH, int VPI = 4>
 ME_HD void me_run_item(const MeItem H, const MeMember* __restrict__ members, int j, double* __restrict__ sm, double mass) {
   const int n_mem = H.w0 & 0xff;
   const int nv = (H.w0 >> 16) & 0xff, v = static_cast<int>(H.w0 >> 24) + j;
   if (n_mem == 0 || v >= nv) return;
   const int n_out = (H.w0 >> 8) & 0xf, kind = (H.w0 >> 12) & 7;
   const bool wide = n_out > 2;
-  const int sh = 4 * j;
   wf4 acc[ME_NSLOT];
   for (int s = 0; s < ME_NSLOT; ++s)
     for (int c = 0; c < 4; ++c) acc[s].c[c] = mk(0.0, 0.0);
   const MeMember* m = members + (H.w1 & 0xffff);
-  unsigned w0 = m->w[0], w2 = m->w[2], w4 = m->w[4];
+  unsigned w0 = m->w[0], w2 = m->w[2], w4 = m->w[4], vc = VPI == 4 ? 0u : me_vmap_c<VPI>(m, j);
   wf4 A, B;
   {
-    const unsigned w1 = m->w[1], w3 = m->w[3];
-    A = ld_wf(sm + (w1 & 0xffff) + 2 * ((w3 >> sh) & 15u));
-    B = ld_wf(sm + (w1 >> 16) + 2 * ((w3 >> (16 + sh)) & 15u));
+    const unsigned w1 = m->w[1];
+    A = ld_wf(sm + (w1 & 0xffff) + me_voff<VPI>(me_vmap_a<VPI>(m, j)));
+    B = ld_wf(sm + (w1 >> 16) + me_voff<VPI>(me_vmap_b<VPI>(m, j)));
   }
 #if defined(__CUDA_ARCH__)
 #pragma unroll 1
 #endif
   for (int i = 0; i < n_mem; ++i) {
-    const unsigned c0 = w0, c2 = w2, c4 = w4;
+    const unsigned c0 = w0, c2 = w2, c4 = w4, cvc = vc;
     const wf4 a = A, b = B;
     if (PREFETCH ? (i + 1 < n_mem) : false) {
       ++m;
-      const unsigned w1 = m->w[1], w3 = m->w[3];
-      w0 = m->w[0]; w2 = m->w[2]; w4 = m->w[4];
-      A = ld_wf(sm + (w1 & 0xffff) + 2 * ((w3 >> sh) & 15u));
-      B = ld_wf(sm + (w1 >> 16) + 2 * ((w3 >> (16 + sh)) & 15u));
+      const unsigned w1 = m->w[1];
+      w0 = m->w[0]; w2 = m->w[2]; w4 = m->w[4]; vc = VPI == 4 ? 0u : me_vmap_c<VPI>(m, j);
+      A = ld_wf(sm + (w1 & 0xffff) + me_voff<VPI>(me_vmap_a<VPI>(m, j)));
+      B = ld_wf(sm + (w1 >> 16) + me_voff<VPI>(me_vmap_b<VPI>(m, j)));
     }
     const int op = c0 & 0xff;
     if (op == OP_SLASH_ROW) {
@@ -199,7 +211,7 @@ ME_HD void me_run_item(const MeItem H, const MeMember* __restrict__ members, int
     } else if (op == OP_VVV) {
       acc_term(acc, vvv_vec_bare(a, ld_k(sm + 8 * ((c0 >> 8) & 0xff)), b, ld_k(sm + 8 * ((c0 >> 16) & 0xff))), c4 & 0x1ffu, wide);
     } else {
-      const wf4 C = ld_wf(sm + (c2 & 0xffff) + 2 * ((c2 >> (16 + sh)) & 15u));
+      const wf4 C = ld_wf(sm + (c2 & 0xffff) + me_voff<VPI>(VPI == 4 ? (c2 >> (16 + 4 * j)) & 15u : cvc));
       wf4 t1, t2, t3;
       vvvv_vec_bare(a, b, C, t1, t2, t3);
       acc_term(acc, t1, c4 & 0x1ffu, wide);
@@ -208,10 +220,10 @@ ME_HD void me_run_item(const MeItem H, const MeMember* __restrict__ members, int
     }
     if (!PREFETCH && i + 1 < n_mem) {
       ++m;
-      const unsigned w1 = m->w[1], w3 = m->w[3];
-      w0 = m->w[0]; w2 = m->w[2]; w4 = m->w[4];
-      A = ld_wf(sm + (w1 & 0xffff) + 2 * ((w3 >> sh) & 15u));
-      B = ld_wf(sm + (w1 >> 16) + 2 * ((w3 >> (16 + sh)) & 15u));
+      const unsigned w1 = m->w[1];
+      w0 = m->w[0]; w2 = m->w[2]; w4 = m->w[4]; vc = VPI == 4 ? 0u : me_vmap_c<VPI>(m, j);
+      A = ld_wf(sm + (w1 & 0xffff) + me_voff<VPI>(me_vmap_a<VPI>(m, j)));
+      B = ld_wf(sm + (w1 >> 16) + me_voff<VPI>(me_vmap_b<VPI>(m, j)));
     }
   }
   // the common propagator, once per colour-ordered current
@@ -219,14 +231,14 @@ ME_HD void me_run_item(const MeItem H, const MeMember* __restrict__ members, int
   const unsigned outs[ME_NSLOT] = {H.w2 & 0xffff, H.w2 >> 16, H.w3 & 0xffff, H.w3 >> 16};
   if (kind == KIND_OPEN) {
     for (int s = 0; s < ME_NSLOT; ++s)
-      if (s < n_out) st_wf(sm + outs[s] + 2 * v, acc[s]);
+      if (s < n_out) st_wf(sm + outs[s] + me_voff<VPI>(v), acc[s]);
   } else if (kind == KIND_VEC) {
     const double f = ks[4];
     for (int s = 0; s < ME_NSLOT; ++s)
       if (s < n_out) {
         wf4 y;
         for (int c = 0; c < 4; ++c) y.c[c] = f * acc[s].c[c];
-        st_wf(sm + outs[s] + 2 * v, y);
+        st_wf(sm + outs[s] + me_voff<VPI>(v), y);
       }
   } else {
     const bool massive = (H.w0 >> 15) & 1;
@@ -234,10 +246,10 @@ ME_HD void me_run_item(const MeItem H, const MeMember* __restrict__ members, int
     const vec4 K = ld_k(ks);
     if (kind == KIND_ROW) {
       for (int s = 0; s < ME_NSLOT; ++s)
-        if (s < n_out) st_wf(sm + outs[s] + 2 * v, prop_row(K, -1.0, mm, f, acc[s]));
+        if (s < n_out) st_wf(sm + outs[s] + me_voff<VPI>(v), prop_row(K, -1.0, mm, f, acc[s]));
     } else {
       for (int s = 0; s < ME_NSLOT; ++s)
-        if (s < n_out) st_wf(sm + outs[s] + 2 * v, prop_col(K, 1.0, mm, f, acc[s]));
+        if (s < n_out) st_wf(sm + outs[s] + me_voff<VPI>(v), prop_col(K, 1.0, mm, f, acc[s]));
     }
   }
 }

@@ -18,14 +18,14 @@ using P = MADME_PROC;
 int geom(me_handle* h) {
   cudaFuncAttributes fa;
   CU(cudaFuncGetAttributes(&fa, me_eval_kernel<P>));
-  const int bytes = ME_W * EventSmem<P>::DOUBLES * 8;
+  const int bytes = P::W_EVENTS * EventSmem<P>::DOUBLES * 8;
   CU(cudaFuncSetAttribute(me_eval_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
   int ctas = 0;
   CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas, me_eval_kernel<P>, 32 * P::N_WARPS, bytes));
   if (ctas < 1) return fail(ME_ECUDA, "me_eval kernel does not fit on an SM%s%s");
   // tensor memory: 512 columns per SM shared by the resident CTAs
   if (JPark<P>::ON && ctas * JPark<P>::COLS > 512) ctas = 512 / JPark<P>::COLS;
-  h->warps = ME_W;
+  h->warps = P::W_EVENTS;
   h->regs = fa.numRegs;
   h->ctas_per_sm = ctas;
   h->smem_bytes = bytes;
@@ -52,7 +52,7 @@ int fill(me_handle* h) {
 }
 
 int eval(me_handle* h, const double* mom, double* me2, double* hel, long long n, cudaStream_t s) {
-  const long long need = (n + ME_W - 1) / ME_W;
+  const long long need = (n + P::W_EVENTS - 1) / P::W_EVENTS;
   const int grid = static_cast<int>(need < h->grid ? need : h->grid);
   me_eval_kernel<P><<<grid, 32 * P::N_WARPS, h->smem_bytes, s>>>(mom, me2, hel, n, h->mass, h->scale);
   CU(cudaGetLastError());

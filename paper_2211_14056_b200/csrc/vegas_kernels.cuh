@@ -16,7 +16,7 @@ template <class P>
 __global__ void __launch_bounds__(32 * P::N_WARPS, 1) vegas_integrand_kernel(VegasArgs a, double* __restrict__ f_out,
                                                                  unsigned long long* __restrict__ idx_out, int idx_words,
                                                                  double* __restrict__ stage_all) {
-  constexpr int NF = P::N_EXT - 2, W = ME_W, NW = P::N_WARPS;
+  constexpr int NF = P::N_EXT - 2, W = P::W_EVENTS, NW = P::N_WARPS;
   constexpr int STRIDE = EventSmem<P>::DOUBLES;
   constexpr int SLOT = 4 * NF + 4;  // final momenta, weight, event index, beam energy, pad
   extern __shared__ __align__(16) double smem[];

@@ -67,9 +67,11 @@ PROCESSES["qqx_ttxg"] = (_QQX + [_G_OUT], "gs", 4 * 9)
 PROCESSES["qg_ttxq"] = (_QG, "gs", 4 * 24)
 PROCESSES["qqx_ttxgg"] = (_QQX + [_G_OUT, _G_OUT], "gs", 4 * 9 * 2)
 PROCESSES["qg_ttxqg"] = (_QG + [_G_OUT], "gs", 4 * 24)
-# Processes whose diagrams are ENUMERATED only (counts pinned in tests/test_generated_host.py against SURVEY.md §8(f)
-# N2); no kernels are generated: g g -> t tbar g g g needs J in tensor memory.
-COUNT_ONLY = {"gg_ttxggg": PROCESSES["gg_ttxgg"][0] + [_G_OUT]}
+# Processes whose diagrams are ENUMERATED only (Program(name, count_only=True)): none at present.
+COUNT_ONLY = {}
+# g g -> t tbar g g g (1 240 diagrams, 120 colour flows; the gap to the
+# tensorised generator widens with the number of diagrams).  1/4 spins x 1/64 colours x 1/3! identical gluons.
+PROCESSES["gg_ttxggg"] = (PROCESSES["gg_ttxgg"][0] + [_G_OUT], "gs", 4 * 64 * 6)
 VECTOR_OF = {"t": "g", "q": "g", "e": "a", "mu": "a"}
 CUT_ALL = True   # every diagram is the contraction of an open current U with a propagated current C (see _pick_cut)
 
@@ -148,9 +150,11 @@ def _set_partitions(items, k):
 class Program:
     """The evaluated-closed-at-centroid diagram list of one process."""
 
-    def __init__(self, name, count_only=False):
-        """count_only: enumerate the diagrams of a COUNT_ONLY process (no colour flows, no factorisation)."""
+    def __init__(self, name, count_only=False, frozen=(0,)):
+        """count_only: enumerate the diagrams only (no colour flows, no factorisation).  frozen: legs whose helicity is
+        fixed while the others are summed (leg 0: parity; emit.py freezes more legs for processes evaluated in passes)."""
         self.name = name
+        self.frozen = tuple(frozen)
         self.legs, self.coupling, self.avg = (COUNT_ONLY[name], "gs", 1) if name in COUNT_ONLY else PROCESSES[name]
         self.n = len(self.legs)
         self.objs = []
@@ -319,7 +323,8 @@ class Program:
             cands = [o for o in cands if 2 * len(o.legs) == self.n]
         if not cands:
             return None
-        return max(cands, key=lambda o: (len(o.legs), max(o.legs)))
+        # among equally large ones, one without a frozen leg: U then holds them all and has the fewest variants
+        return max(cands, key=lambda o: (len(o.legs), not any(l in o.legs for l in self.frozen), max(o.legs)))
 
     def _close3(self, A, B, C):
         objs = (A, B, C)
@@ -444,18 +449,32 @@ class Program:
                             ops.append(np.eye(3, dtype=complex))
                             lab[cols[pairing[k]]] = nxt
                     out = "".join(lab[l] for l in col_legs)
-                    basis.append(np.einsum(",".join(expr_in) + "->" + out, *ops))
+                    basis.append(np.einsum(",".join(expr_in) + "->" + out, *ops, optimize=True))
                     perms.append((tuple(pairing), tuple(strings)) if nl > 1 else tuple(s))
         self.flow_perms = perms
         nb = len(basis)
         Bm = np.array([b.ravel() for b in basis])
-        cfi0 = np.linalg.inv(Bm.conj() @ Bm.T)
+        del basis
+        # A term's flow coefficients solve  sum_f c_f B_f = (its colour tensor): an overdetermined consistent system.
+        # Small tensors use every entry; for g g -> t tbar g g g (8^5 x 9 entries, 120 flows, 1 890 terms) a fixed random
+        # sample of the entries determines c and a second, disjoint sample checks it.
+        size = Bm.shape[1]
+        if size > 40000:
+            pick = np.random.default_rng(20221114).permutation(size)
+            sel, chk = np.sort(pick[:12288]), np.sort(pick[12288:24576])
+        else:
+            sel = chk = np.arange(size)
+        Bs, Bc = Bm[:, sel], Bm[:, chk]
+        gram = Bs.conj() @ Bs.T
+        assert np.linalg.cond(gram) < 1e8, "the sampled colour basis is not independent"
+        cfi0 = np.linalg.inv(gram) @ Bs.conj()
         arrs = []
         for t in self.terms:
             arr, labels = self._term_colour(t)
             assert labels == col_legs, (labels, col_legs)
-            c = cfi0 @ (Bm.conj() @ arr.ravel())
-            assert np.allclose(Bm.T @ c, arr.ravel(), atol=1e-9), "colour factor outside the flow basis"
+            flat = arr.ravel()
+            c = cfi0 @ flat[sel]
+            assert np.allclose(Bc.T @ c, flat[chk], atol=1e-9), "colour factor outside the flow basis"
             arrs.append(c)
         # one magnitude per flow (1 with one line): scale the basis tensor by it
         mag = np.ones(nb)
@@ -469,18 +488,14 @@ class Program:
         cf = (Bm.conj() @ Bm.T)
         assert np.allclose(cf.imag, 0)
         cf = cf.real
-        den = next(d for d in range(1, 4000) if np.allclose(np.rint(cf * d), cf * d, atol=1e-9))
+        den = next(d for d in range(1, 4000) if np.allclose(np.rint(cf * d), cf * d, atol=1e-7))
         if nl == 1:
-            assert den == {2: 3, 3: 9, 4: 54}.get(len(glu), den)
+            assert den == {2: 3, 3: 9, 4: 54, 5: 324}.get(len(glu), den)
         num = np.rint(cf * den)
         self.cf_num = num.astype(np.int64)
         self.cf_den = den
-        cfi = np.linalg.inv(cf)
-        for t in self.terms:
-            arr, _ = self._term_colour(t)
-            c = cfi @ (Bm.conj() @ arr.ravel())
-            assert np.allclose(Bm.T @ c, arr.ravel(), atol=1e-9), "colour factor outside the flow basis"
-            c = c * t.phase
+        for t, c in zip(self.terms, arrs):
+            c = c / mag * t.phase
             flows = []
             for f in range(nb):
                 if abs(c[f]) < 1e-9:

@@ -26,14 +26,33 @@ from .diagrams import PROCESSES, Program
 HERE = os.path.dirname(os.path.abspath(__file__))
 OUT_DIR = os.path.join(os.path.dirname(HERE), "csrc", "generated")
 NSLOT = 4            # accumulators (colour-ordered currents) per item
-W_EVENTS = 8         # events per CTA = warps per CTA
-VPI = 32 // W_EVENTS  # helicity variants per item (lanes = VPI variants x W_EVENTS events)
-N_WARPS = int(os.environ.get("MADME_GEN_WARPS", "8"))
-DOTS_C_PER_U = N_WARPS > W_EVENTS
-DYNAMIC = False      # True: items listed longest first for a shared work counter (measured, lost 4 %; the kernel uses the fixed map)   # warps per CTA: W_EVENTS own an event in the dot stages, all run items
-# shared-memory budget: doubles per event so that W_EVENTS events fit in the 227 KB a CTA can own
-SMEM_BUDGET_DOUBLES = int(os.environ.get("MADME_GEN_SMEM_DOUBLES", str((232448 // (8 * W_EVENTS)) - 32 - 16)))
+W_EVENTS = 8         # events per CTA (default geometry)
+N_WARPS = int(os.environ.get("MADME_GEN_WARPS", "8"))   # warps per CTA: W_EVENTS own an event in the dot stages, all run items
+DYNAMIC = False      # True: items listed longest first for a shared work counter (measured, lost 4 %; the kernel uses the fixed map)
 N_ROUNDS = int(os.environ.get("MADME_GEN_ROUNDS", "0"))   # 0: the fewest rounds that fit the budget
+# Per-process geometry.  w_events: events per CTA (32 / w_events helicity variants per item); frozen: legs whose helicity
+# is fixed during one PASS over the event (leg 0 always: parity; more legs = 2^(len-1) passes, each summing the other
+# helicities, so that one lane still holds one helicity combination and J of one pass fits tensor memory); chunk: colour
+# flows held in registers at a time by the dot stages (0: all of them), the others wait in tensor memory.
+GEOMETRY = {"gg_ttxggg": dict(w_events=4, frozen=(0, 6), chunk=int(os.environ.get("MADME_GEN_CHUNK", "20")))}
+FROZEN = (0,)        # set per process by emit_process
+
+
+def geometry(name):
+    g = dict(w_events=W_EVENTS, frozen=(0,), chunk=0)
+    g.update(GEOMETRY.get(name, {}))
+    return g
+
+
+def smem_budget_doubles(w_events):
+    """doubles per event so that w_events events fit in the 227 KB a CTA can own"""
+    return int(os.environ.get("MADME_GEN_SMEM_DOUBLES", str((232448 // (8 * w_events)) - 32 - 16)))
+
+
+def voff(v):
+    """double offset of helicity variant v inside a stored object: 16-byte slots of one 128-byte line, objects with 16
+    variants continue in the next group of four lines"""
+    return 2 * (v & 7) + 64 * (v >> 3)
 
 OP_SLASH_ROW, OP_SLASH_COL, OP_FFV_VEC, OP_VVV, OP_VVVV = range(5)
 KIND_VEC, KIND_ROW, KIND_COL, KIND_OPEN = range(4)
@@ -48,8 +67,9 @@ FLOPS_DOT, FLOPS_EXT = 4 * 8, 45
 
 
 def bits_of(legs):
-    """Legs that carry a helicity label (leg 0 is fixed at +1 by parity, see diagrams.py)."""
-    return [l for l in legs if l != 0]
+    """Legs that carry a helicity label inside one pass (leg 0 is fixed at +1 by parity, see diagrams.py; the other frozen
+    legs are fixed by the pass)."""
+    return [l for l in legs if l not in FROZEN]
 
 
 def variant_index(sub_legs, sup_legs, v):
@@ -112,7 +132,9 @@ class Layout:
     open side U | the rest); the operands of a split's dot products live in the round region while that split's
     round is processed."""
 
-    def __init__(self, P, n_rounds):
+    def __init__(self, P, n_rounds, cap=None):
+        """cap: the most doubles the operands of one leg split may take in the round region; a larger split is divided
+        into PARTS (its open currents U in groups, each with the dot products they enter) that go to different rounds."""
         self.P = P
         objs = P.used_objects()
         self.objs = objs
@@ -132,25 +154,42 @@ class Layout:
         self.sub_index = {s: i for i, s in enumerate(subsets)}
         # split of every stored object outside the base: U side -> its own legs; C side -> the complement
         u_sets = {P.objs[d[1]].legs for d in P.dots}
-        self.split_of = {}
+        self.split_of = {}      # stored object outside the base -> (legs of the U side, part)
         for o in self.stored:
             if o.id in base_ids:
                 continue
             comp = tuple(l for l in all_legs if l not in o.legs)
-            self.split_of[o.id] = o.legs if (0 in o.legs) else comp
-            assert self.split_of[o.id] in u_sets, o.legs
-        self.splits = sorted(u_sets, key=lambda s: (len(s), s))
-        size = {s: 0 for s in self.splits}
+            self.split_of[o.id] = (o.legs if (0 in o.legs) else comp, 0)
+            assert self.split_of[o.id][0] in u_sets, o.legs
+        size = {(s, 0): 0 for s in sorted(u_sets, key=lambda s: (len(s), s))}
         for o in self.stored:
             if o.id in self.split_of:
                 size[self.split_of[o.id]] += 8 * self.nv(o)
+        if cap:
+            for key in sorted(k for k, v in size.items() if v > cap):
+                mine = [o for o in self.stored if self.split_of.get(o.id) == key]
+                us = [o for o in mine if o.legs == key[0]]
+                # the C side must already be resident (base), so that a part is just a group of U's
+                assert len(us) == len(mine), "a split that is too large has C operands outside the base"
+                # neighbours share bare vertices: order by the members so that a part keeps them together
+                us.sort(key=lambda o: (sorted(self.unit_key(m) for m, _ in self.members_of(o)), o.id))
+                part, used = 0, 0
+                for o in us:
+                    need = 8 * self.nv(o)
+                    if used + need > cap:
+                        part, used = part + 1, 0
+                    used += need
+                    self.split_of[o.id] = (key[0], part)
+                    size[(key[0], part)] = used
+        self.part_of_u = {oid: k[1] for oid, k in self.split_of.items() if P.objs[oid].legs == k[0]}
+        self.splits = sorted(size, key=lambda k: (len(k[0]), k))
         bins = [[0, []] for _ in range(max(1, min(n_rounds, len(self.splits))))]
         for s_, sz in sorted(size.items(), key=lambda kv: -kv[1]):
             b = min(bins, key=lambda x: x[0])
             b[0] += sz
             b[1].append(s_)
         bins = [b for b in bins if b[1]]
-        self.rounds = [sorted(b[1], key=lambda s: (len(s), s)) for b in bins]
+        self.rounds = [sorted(b[1], key=lambda k: (len(k[0]), k)) for b in bins]
         self.round_of = {s_: r for r, b in enumerate(self.rounds) for s_ in b}
         # Fixed-stride storage: a GROUP is 4 lines of 128 B (one line per wavefunction component); an object with nv
         # variants owns nv consecutive 16-byte slots (aligned to nv) in each line, so component c of variant v sits at
@@ -164,7 +203,12 @@ class Layout:
             groups = []          # free slot bitmaps
             for o in sorted(obj_list, key=lambda o: (-self.nv(o), o.id)):
                 nv = self.nv(o)
-                assert nv <= 8, "objects with more than 8 helicity variants need a wider storage group"
+                assert nv <= (8 if len(FROZEN) == 1 else 16), "objects with more helicity variants need a wider storage"
+                if nv == 16:    # two whole groups, consecutive
+                    groups.append([True] * 8)
+                    groups.append([True] * 8)
+                    self.off[o.id] = first_group_off + (len(groups) - 2) * 64
+                    continue
                 for gi, used in enumerate(groups):
                     slot = next((s0 for s0 in range(0, 8, nv) if not any(used[s0:s0 + nv])), None)
                     if slot is not None:
@@ -189,6 +233,10 @@ class Layout:
 
     def round_objs(self, r):
         return [o for o in self.stored if o.id in self.split_of and self.round_of[self.split_of[o.id]] == r]
+
+    def dot_key(self, d):
+        """(legs of the U side, part) of a dot product (flow, u, c, phase, kind)"""
+        return (self.P.objs[d[1]].legs, self.part_of_u.get(d[1], 0))
 
     # ---- tasks -------------------------------------------------------------------------------------------------
     def members_of(self, o):
@@ -292,20 +340,39 @@ def split_flows(P, nf):
     return best[1]
 
 
-def pick_rounds(P):
+def pick_rounds(P, budget):
     if N_ROUNDS:
         return Layout(P, N_ROUNDS)
-    for n in range(1, 17):
-        L = Layout(P, n)
-        if 4 * P.n + L.smem_doubles <= SMEM_BUDGET_DOUBLES or n >= len(L.splits):
+    L = Layout(P, 1)
+    if 4 * P.n + L.smem_doubles <= budget:
+        return L
+    cap = ((budget - 4 * P.n - L.base_doubles) // 64) * 64 - 64     # whole storage groups, one spare for fragmentation
+    assert cap >= 512, "the base region leaves no room for a round"
+    for n in range(2, 129):
+        L = Layout(P, n, cap)
+        if 4 * P.n + L.smem_doubles <= budget or n >= len(L.splits):
             return L
     return L
 
 
 def emit_process(name, n_rounds=None):
-    P = Program(name)
+    global FROZEN
+    geo = geometry(name)
+    FROZEN = tuple(geo["frozen"])
+    try:
+        return _emit_process(name, n_rounds, geo)
+    finally:
+        FROZEN = (0,)
+
+
+def _emit_process(name, n_rounds, geo):
+    W_EV, CHUNK = geo["w_events"], geo["chunk"]
+    VPI = 32 // W_EV
+    DOTS_C_PER_U = N_WARPS > W_EV and not CHUNK
+    P = Program(name, frozen=FROZEN)
     assert all(t.op.startswith("DOT") for t in P.terms), "every diagram must be a propagator-cut contraction"
-    L = Layout(P, n_rounds) if n_rounds else pick_rounds(P)
+    L = Layout(P, n_rounds) if n_rounds else pick_rounds(P, smem_budget_doubles(W_EV))
+    assert 4 * P.n + L.smem_doubles <= smem_budget_doubles(W_EV), "the event does not fit the CTA's shared memory"
     n = P.n
     nf = len(P.flow_perms)
     W = []
@@ -381,8 +448,13 @@ def emit_process(name, n_rounds=None):
             assert max(offs) < 65536
             ks = [sub_i(a.legs) for a in args[:2]]
             code = lambda term: u.swap[term] | (sum(c << (2 * sl) for sl, c in enumerate(u.sign[term])) << 1)
-            members.append((u.op | (ks[0] << 8) | (ks[1] << 16), offs[0] | (offs[1] << 16), offs[2] | (vmaps[2] << 16),
-                            vmaps[0] | (vmaps[1] << 16), code(0) | (code(1) << 9) | (code(2) << 18), 0, 0, 0))
+            if VPI == 4:    # four 4-bit entries per argument
+                members.append((u.op | (ks[0] << 8) | (ks[1] << 16), offs[0] | (offs[1] << 16), offs[2] | (vmaps[2] << 16),
+                                vmaps[0] | (vmaps[1] << 16), code(0) | (code(1) << 9) | (code(2) << 18), 0, 0, 0))
+            else:           # eight 4-bit entries per argument: a word each (w3, w5, w6)
+                assert VPI == 8
+                members.append((u.op | (ks[0] << 8) | (ks[1] << 16), offs[0] | (offs[1] << 16), offs[2],
+                                vmaps[0], code(0) | (code(1) << 9) | (code(2) << 18), vmaps[1], vmaps[2], 0))
         outs = [L.off[x.id] for x in t.outputs] + [0] * NSLOT
         assert first < 65536 and len(t.units) < 256 and nv < 256
         w0 = len(t.units) | (len(t.outputs) << 8) | (L.kind_of(o) << 12) | (massive_of(o) << 15) | (nv << 16) | (vbase << 24)
@@ -412,12 +484,32 @@ def emit_process(name, n_rounds=None):
       % (sum(1 for o in L.stored if o.op != "EXT"), n_tasks, n_units, s["n_dots"]))
     w("// helicity combination over %d leg splits in %d rounds; %d of %d combinations evaluated (parity, leg 0 at +1)"
       % (len(L.splits), len(L.rounds), 1 << (n - 1), 1 << n))
+    n_pass = 1 << (len(FROZEN) - 1)
+    hel_legs = bits_of(range(n))            # bit k of a lane's helicity index h is the helicity of leg hel_legs[k]
+    if n_pass > 1:
+        w("// in %d passes: legs %s are fixed during a pass, a lane holds one combination of the helicities of legs %s"
+          % (n_pass, list(FROZEN[1:]), hel_legs))
     w("#pragma once")
     w('#include "../me_tasks.cuh"')
     w("namespace madme {")
     w("struct %s {" % name)
     w("  static constexpr int N_EXT = %d, N_HEL = %d, N_HEL_EVAL = %d, N_FLOW = %d, N_SUB = %d;"
-      % (n, 1 << n, 1 << (n - 1), nf, len(L.subsets)))
+      % (n, 1 << n, 1 << len(hel_legs), nf, len(L.subsets)))
+    w("  // geometry: events per CTA; passes over the event with the helicities of the FROZEN legs fixed (leg 0: +1, the")
+    w("  // others by the pass index, bit k-1 of it for the k-th frozen leg); colour flows per register chunk (0: all)")
+    w("  static constexpr int W_EVENTS = %d, VPI = %d, N_PASS = %d, CHUNK = %d, N_CHUNK = %d;"
+      % (W_EV, VPI, n_pass, CHUNK, (nf + CHUNK - 1) // CHUNK if CHUNK else 1))
+    w("  static constexpr bool CHUNKED = %s;" % ("true" if CHUNK else "false"))
+    w("  static constexpr unsigned FROZEN_MASK = %d;" % sum(1 << l for l in FROZEN))
+    w("  // helicity of every leg (bit l) for lane index h of pass p; leg 0 at +1")
+    w("  static ME_HD int full_helicity(int h, int p) {")
+    w("    return 1 | %s;" % " | ".join(["(((h >> %d) & 1) << %d)" % (k, l) for k, l in enumerate(hel_legs)]
+                                        + ["(((p >> %d) & 1) << %d)" % (k, l) for k, l in enumerate(FROZEN[1:])]))
+    w("  }")
+    w("  // fixed helicities of the frozen legs in pass p, as bits at the leg positions")
+    w("  static ME_HD unsigned frozen_helicities(int p) {")
+    w("    return 1u%s;" % "".join(" | (((unsigned(p) >> %d) & 1u) << %d)" % (k, l) for k, l in enumerate(FROZEN[1:])))
+    w("  }")
     w("  static constexpr int N_DIAGRAMS = %d, N_DIAGRAMS_4G = %d, N_TERMS = %d, N_CURRENTS = %d, N_COMBOS = %d, N_DOTS = %d;"
       % (s["n_diagrams"], s["n_diagrams_4g"], s["n_terms"], s["n_currents"], s["n_combos"], s["n_dots"]))
     w("  static constexpr int SMEM_DOUBLES = %d, BASE_DOUBLES = %d;" % (L.smem_doubles, L.base_doubles))
@@ -467,61 +559,73 @@ def emit_process(name, n_rounds=None):
     # ---- dots, round by round ----------------------------------------------------------------------------------
     def ldw(oid):
         o = P.objs[oid]
-        terms = ["%d * b%d" % (2 << k, l) for k, l in enumerate(bits_of(o.legs))]
+        terms = ["%d * b%d" % (voff(1 << k), l) for k, l in enumerate(bits_of(o.legs))]
         return "ld_wf(sm + %s)" % " + ".join([str(L.off[oid])] + terms)
 
     zcode = {1: 0, 1j: 1, -1: 2, -1j: 3}
     by_split = {}
     for d in P.dots:
-        by_split.setdefault(P.objs[d[1]].legs, []).append(d)
+        by_split.setdefault(L.dot_key(d), []).append(d)
+    def emit_round_body(r, keep, local, ind):
+        """the dot products of round r that feed the flows in `keep` (global flow -> index into jr/ji given by `local`);
+        returns (flop count, number of contractions)"""
+        flops = ncon = 0
+        for key in L.rounds[r]:
+            dots = [d for d in by_split.get(key, []) if d[0] in keep]
+            if not dots:
+                continue
+            w(ind + "{  // split %s | rest%s: %d dot products" % ("".join(str(l) for l in key[0]), " (part %d)" % key[1] if key[1] else "", len(dots)))
+            if not DOTS_C_PER_U:
+                for c in sorted({d[2] for d in dots}):
+                    w(ind + "  const wf4 c%d = %s;" % (c, ldw(c)))
+            for u in sorted({d[1] for d in dots}):
+                w(ind + "  { const wf4 u = %s;" % ldw(u))
+                by_c = {}
+                for (f, uu, c, z, kind) in dots:
+                    if uu == u:     # the phases i^a of the stored operands go into the dot product's phase
+                        by_c.setdefault((c, kind), []).append((local[f], (zcode[z] + out_phase.get(u, 0) + out_phase.get(c, 0)) % 4))
+                for (c, kind), fl in sorted(by_c.items()):
+                    mink = "true" if kind == "V" else "false"
+                    if DOTS_C_PER_U:     # one C operand live at a time
+                        w(ind + "    { const wf4 c%d = %s;" % (c, ldw(c)))
+                    ncon += 1
+                    if len(fl) == 1:
+                        w(ind + "    dot_acc<%d, %s>(jr[%d], ji[%d], u, c%d);" % (fl[0][1], mink, fl[0][0], fl[0][0], c))
+                        flops += FLOPS_DOT
+                    else:   # one contraction feeds several colour flows: computed once, added with each flow's phase
+                        w(ind + "    { const cplx t = dot_val<%s>(u, c%d);" % (mink, c))
+                        for f, zc in fl:
+                            w(ind + "      jadd<%d>(jr[%d], ji[%d], t);" % (zc, f, f))
+                        w(ind + "    }")
+                        flops += FLOPS_DOT - 4 + 2 * len(fl)
+                    if DOTS_C_PER_U:
+                        w(ind + "    }")
+                w(ind + "  }")
+            w(ind + "}")
+        return flops, ncon
+
+    def hel_bits():
+        for k, l in enumerate(hel_legs):
+            w("    const int b%d = (h >> %d) & 1; (void)b%d;" % (l, k, l))
+
     def emit_dots(fname, keep, local):
-        """dots of the flows in `keep` (global flow -> index into jr/ji given by `local`); returns the flop count"""
         flops = 0
         w("  static ME_HD void %s(int r, const double* __restrict__ sm, int h, double* __restrict__ jr, double* __restrict__ ji) {" % fname)
-        for l in range(1, n):
-            w("    const int b%d = (h >> %d) & 1; (void)b%d;" % (l, l - 1, l))
+        hel_bits()
         w("    switch (r) {")
-        for r, split_list in enumerate(L.rounds):
+        for r in range(len(L.rounds)):
             w("      case %d: {" % r)
-            for legs in split_list:
-                dots = [d for d in by_split[legs] if d[0] in keep]
-                if not dots:
-                    continue
-                w("        {  // split %s | rest: %d dot products" % ("".join(str(l) for l in legs), len(dots)))
-                if not DOTS_C_PER_U:
-                    for c in sorted({d[2] for d in dots}):
-                        w("          const wf4 c%d = %s;" % (c, ldw(c)))
-                for u in sorted({d[1] for d in dots}):
-                    w("          { const wf4 u = %s;" % ldw(u))
-                    by_c = {}
-                    for (f, uu, c, z, kind) in dots:
-                        if uu == u:     # the phases i^a of the stored operands go into the dot product's phase
-                            by_c.setdefault((c, kind), []).append((local[f], (zcode[z] + out_phase.get(u, 0) + out_phase.get(c, 0)) % 4))
-                    for (c, kind), fl in sorted(by_c.items()):
-                        mink = "true" if kind == "V" else "false"
-                        if DOTS_C_PER_U:     # one C operand live at a time
-                            w("            { const wf4 c%d = %s;" % (c, ldw(c)))
-                        if len(fl) == 1:
-                            w("            dot_acc<%d, %s>(jr[%d], ji[%d], u, c%d);" % (fl[0][1], mink, fl[0][0], fl[0][0], c))
-                            flops += FLOPS_DOT
-                        else:   # one contraction feeds several colour flows: computed once, added with each flow's phase
-                            w("            { const cplx t = dot_val<%s>(u, c%d);" % (mink, c))
-                            for f, zc in fl:
-                                w("              jadd<%d>(jr[%d], ji[%d], t);" % (zc, f, f))
-                            w("            }")
-                            flops += FLOPS_DOT - 4 + 2 * len(fl)
-                        if DOTS_C_PER_U:
-                            w("            }")
-                    w("          }")
-                w("        }")
+            flops += emit_round_body(r, keep, local, "        ")[0]
             w("      } break;")
         w("      default: break;")
         w("    }")
         w("  }")
         return flops
 
-    w("  // a7-a8: the dot products of round r for helicity combination h (leg 0 has helicity +1; bit l-1 of h is the")
-    w("  // helicity of leg l, 0 <-> -1, 1 <-> +1), accumulated into the colour-flow vector J = (jr, ji).")
+    w("  // a7-a8: the dot products of round r for helicity combination h (bit k of h is the helicity of the k-th leg that")
+    w("  // is not frozen, 0 <-> -1, 1 <-> +1), accumulated into the colour-flow vector J = (jr, ji).")
+    if CHUNK:
+        return _emit_chunked(W, w, P, L, nf, CHUNK, n_pass, n, cur_flops, emit_round_body, hel_bits)
     amp_flops = emit_dots("dots", set(range(nf)), {f: f for f in range(nf)})
 
     # ---- colour contraction grouped by distinct CF numerator (SURVEY §8(c) E: 9 distinct values for 4 gluons) ----
@@ -591,11 +695,12 @@ def emit_process(name, n_rounds=None):
     fca = emit_colour("colour_cross_a(%s)" % four, cross_a)
     fcb0 = emit_colour("colour_cross_b0(%s)" % four, cross_b0)
     fcb1 = emit_colour("colour_cross_b1(%s)" % four, cross_b1)
-    w("  static constexpr bool SPLIT_J = %s;" % ("true" if N_WARPS == 2 * W_EVENTS else "false"))
-    if N_WARPS == 2 * W_EVENTS:
+    w("  static constexpr bool SPLIT_J = %s;" % ("true" if N_WARPS == 2 * W_EV else "false"))
+    if N_WARPS == 2 * W_EV:
         amp_flops, col_flops = flops_a + flops_b, fa_ + fb_ + fca + fcb0 + fcb1
     ext_flops = FLOPS_EXT * 2 * n
-    nh = 1 << (n - 1)
+    nh = 1 << len(hel_legs)
+    assert n_pass == 1
     per_event = ext_flops + cur_flops + nh * (amp_flops + col_flops)
     w("  // nominal fp64 flops per event as emitted (FMA = 2): externals %d + currents %d + %d helicities x"
       % (ext_flops, cur_flops, nh))
@@ -606,22 +711,134 @@ def emit_process(name, n_rounds=None):
     return "\n".join(W) + "\n"
 
 
-def emit_all(out_dir=OUT_DIR, only=None):
+def _emit_chunked(W, w, P, L, nf, CHUNK, n_pass, n, cur_flops, emit_round_body, hel_bits):
+    """The dot and colour stages of a process whose colour-flow vector does not fit the registers of a lane: J lives in
+    tensor memory (4 N_FLOW 32-bit columns of the warp's lanes), CHUNK flows at a time are loaded, updated by the dot
+    products of the round that feed them, and stored back; J^dagger CF J is summed over pairs of chunks."""
+    nc = (nf + CHUNK - 1) // CHUNK
+    chunk_of = lambda f: f // CHUNK
+    flops = ncon = 0
+    has = []
+    w("  // dot products of round r that feed the colour flows of chunk c (flow f = c * CHUNK + index into jr / ji)")
+    w("  static ME_HD void dots(int r, int c, const double* __restrict__ sm, int h, double* __restrict__ jr, double* __restrict__ ji) {")
+    hel_bits()
+    w("    switch (r * N_CHUNK + c) {")
+    for r in range(len(L.rounds)):
+        for c in range(nc):
+            keep = {f for f in range(nf) if chunk_of(f) == c}
+            mark = len(W)
+            w("      case %d: {  // round %d, flows %d..%d" % (r * nc + c, r, c * CHUNK, min(nf, (c + 1) * CHUNK) - 1))
+            fl, k = emit_round_body(r, keep, {f: f - c * CHUNK for f in keep}, "        ")
+            if k == 0:
+                del W[mark:]
+                continue
+            w("      } break;")
+            flops += fl
+            ncon += k
+            has.append(r * nc + c)
+    w("      default: break;")
+    w("    }")
+    w("  }")
+    w("  static ME_HD bool has_dots(int r, int c) {")
+    w("    switch (r * N_CHUNK + c) {")
+    for k in has:
+        w("      case %d:" % k)
+    w("        return true;")
+    w("      default: return false;")
+    w("    }")
+    w("  }")
+    w("  static constexpr int N_CONTRACTIONS = %d;  // per helicity combination (a contraction shared by flows of different chunks counts twice)" % ncon)
+    cf = P.cf_num
+
+    def body(pairs):
+        """sum of wt CF (re re + im im) over pairs, grouped by value so that few partial sums are live at a time"""
+        fl = 0
+        by_val = {}
+        for (fa, ga, v, wt) in pairs:
+            by_val.setdefault(v * wt, []).append((fa, ga))
+        re = lambda a: ("or_[%d]" if a[0] == "o" else "jr[%d]") % a[1]
+        im = lambda a: ("oi[%d]" if a[0] == "o" else "ji[%d]") % a[1]
+        w("        double tot = 0.0;")
+        for v in sorted(by_val, key=lambda v: -abs(v)):
+            if v == 0:
+                continue
+            lst = by_val[v]
+            w("        { double s0 = 0.0, s1 = 0.0;")
+            for k, (fa, ga) in enumerate(lst):
+                nm = "s%d" % (k & 1)
+                w("          %s = fma(%s, %s, fma(%s, %s, %s));" % (nm, re(fa), re(ga), im(fa), im(ga), nm))
+                fl += 4
+            w("          tot = fma(%d.0, s0 + s1, tot); }" % v)
+            fl += 3
+        w("        return tot;")
+        return fl
+
+    col_flops = 0
+    w("  // a9: sum_{f,f'} J_f^* CFnum_{ff'} J_f' as a sum over chunks (diagonal blocks) and pairs of chunks (x 2)")
+    w("  static ME_HD double colour_diag(int c, const double* __restrict__ jr, const double* __restrict__ ji) {")
+    w("    switch (c) {")
+    for c in range(nc):
+        fl_ = [f for f in range(nf) if chunk_of(f) == c]
+        w("      case %d: {" % c)
+        col_flops += body([(("j", f - c * CHUNK), ("j", g - c * CHUNK), int(cf[f, g]), 1 if f == g else 2) for i, f in enumerate(fl_) for g in fl_[i:]])
+        w("      }")
+    w("      default: return 0.0;")
+    w("    }")
+    w("  }")
+    w("  // chunk ca in (jr, ji), chunk cb > ca in (or_, oi)")
+    w("  static ME_HD double colour_pair(int ca, int cb, const double* __restrict__ jr, const double* __restrict__ ji,")
+    w("                                  const double* __restrict__ or_, const double* __restrict__ oi) {")
+    w("    switch (ca * N_CHUNK + cb) {")
+    for ca in range(nc):
+        for cb in range(ca + 1, nc):
+            fa_ = [f for f in range(nf) if chunk_of(f) == ca]
+            fb_ = [f for f in range(nf) if chunk_of(f) == cb]
+            w("      case %d: {" % (ca * nc + cb))
+            col_flops += body([(("j", f - ca * CHUNK), ("o", g - cb * CHUNK), int(cf[f, g]), 2) for f in fa_ for g in fb_])
+            w("      }")
+    w("      default: return 0.0;")
+    w("    }")
+    w("  }")
+    w("  static constexpr bool SPLIT_J = false;")
+    w("  static constexpr int N_FLOW_HALF = N_FLOW;")
+    ext_flops = FLOPS_EXT * 2 * n
+    nh = 1 << len(bits_of(range(n)))
+    per_event = n_pass * (ext_flops + cur_flops + nh * (flops + col_flops))
+    w("  // nominal fp64 flops per event as emitted (FMA = 2): %d passes x (externals %d + currents %d + %d helicities x"
+      % (n_pass, ext_flops, cur_flops, nh))
+    w("  // (dot products %d + colour %d))" % (flops, col_flops))
+    w("  static constexpr double FLOPS_PER_EVENT = %d.0;" % per_event)
+    w("};")
+    w("}  // namespace madme")
+    return "\n".join(W) + "\n"
+
+
+def emit_all(out_dir=OUT_DIR, only=None, force=False):
+    """Regenerate the programs that are older than the generator's sources (g g -> t tbar g g g alone takes half a minute);
+    force, or any MADME_GEN_* override in the environment, regenerates everything."""
     os.makedirs(out_dir, exist_ok=True)
     paths = []
+    newest = max(os.path.getmtime(os.path.join(HERE, f)) for f in ("emit.py", "diagrams.py"))
+    force = force or any(k.startswith("MADME_GEN_") for k in os.environ)
     for name in PROCESSES:
         if only and name not in only:
             continue
-        src = emit_process(name)
         path = os.path.join(out_dir, name + ".inc")
+        if not force and os.path.exists(path) and os.path.getmtime(path) >= newest:
+            paths.append(path)
+            continue
+        src = emit_process(name)
         old = open(path).read() if os.path.exists(path) else None
         if old != src:
             with open(path, "w") as f:
                 f.write(src)
+        else:
+            os.utime(path)
         paths.append(path)
     return paths
 
 
 if __name__ == "__main__":
-    for p in emit_all():
+    import sys
+    for p in emit_all(force="--force" in sys.argv):
         print(p)

@@ -10,6 +10,7 @@
 #include "../../paper_2211_14056_b200/csrc/generated/gg_ttx.inc"
 #include "../../paper_2211_14056_b200/csrc/generated/gg_ttxg.inc"
 #include "../../paper_2211_14056_b200/csrc/generated/gg_ttxgg.inc"
+#include "../../paper_2211_14056_b200/csrc/generated/gg_ttxggg.inc"
 #include "../../paper_2211_14056_b200/csrc/generated/qqx_ttx.inc"
 #include "../../paper_2211_14056_b200/csrc/generated/qqx_ttxg.inc"
 #include "../../paper_2211_14056_b200/csrc/generated/qg_ttxq.inc"
@@ -28,19 +29,63 @@ template <class P> struct Tables;
     static const int* massive() { static const int t[] = U##_LEG_MASSIVE; return t; }   \
     static const int* ext_off() { static const int t[] = U##_EXT_OFF; return t; }       \
   };
-#define FOR_EACH_PROCESS(X) X(epem_mupmum) X(gg_ttx) X(gg_ttxg) X(gg_ttxgg) X(qqx_ttx) X(qqx_ttxg) X(qg_ttxq) X(qqx_ttxgg) X(qg_ttxqg)
+#define FOR_EACH_PROCESS(X) X(epem_mupmum) X(gg_ttx) X(gg_ttxg) X(gg_ttxgg) X(gg_ttxggg) X(qqx_ttx) X(qqx_ttxg) X(qg_ttxq) X(qqx_ttxgg) X(qg_ttxqg)
 FOR_EACH_PROCESS(DEF_TABLES)
 
 // items [begin, end) of one stage for ONE event: the device runs them with lanes = (local variant j, event)
 template <class P> void items(double* sm, int begin, int end, double mass) {
   for (int it = begin; it < end; ++it)
-    for (int j = 0; j < 4; ++j) {
-      if (it & 1) me_run_item<true>(Tables<P>::items()[it], Tables<P>::members(), j, sm, mass);   // both forms of the member loop
-      else me_run_item<false>(Tables<P>::items()[it], Tables<P>::members(), j, sm, mass);
+    for (int j = 0; j < P::VPI; ++j) {
+      if (it & 1) me_run_item<true, P::VPI>(Tables<P>::items()[it], Tables<P>::members(), j, sm, mass);   // both forms of the member loop
+      else me_run_item<false, P::VPI>(Tables<P>::items()[it], Tables<P>::members(), j, sm, mass);
     }
 }
 
+// the chunked form (me_kernel.cuh::cta_me2_chunked): passes over the frozen helicities, J held whole here (the device keeps
+// it in tensor memory), dots and colour called chunk by chunk exactly as the device does
+template <class P> void eval_chunked(const double* mom, double* me2, long long n, double mass, double coupling, double* per_hel) {
+  std::vector<double> sm(P::SMEM_DOUBLES);
+  double g2 = 1;
+  for (int i = 0; i < P::COUPLING_POWER; ++i) g2 *= coupling;
+  const double scale = g2 / (double(P::CF_DEN) * double(P::AVG_DEN));
+  constexpr int CH = P::CHUNK, NC = P::N_CHUNK;
+  for (long long e = 0; e < n; ++e) {
+    double s = 0;
+    for (int pass = 0; pass < P::N_PASS; ++pass) {
+      for (int lane = 0; lane < 32; ++lane)
+        me_phase0(lane, 32, sm.data(), mom + e * 4 * P::N_EXT, P::N_EXT, P::N_SUB, Tables<P>::masks(), Tables<P>::kind(),
+                  Tables<P>::massive(), Tables<P>::ext_off(), mass, P::FROZEN_MASK, P::frozen_helicities(pass));
+      std::vector<double> jr(size_t(P::N_HEL_EVAL) * CH * NC, 0.0), ji(size_t(P::N_HEL_EVAL) * CH * NC, 0.0);
+      int it = 0;
+      for (int p = 0; p < P::N_STAGES; ++p) {
+        items<P>(sm.data(), it, P::stage_end(p), mass);
+        it = P::stage_end(p);
+        const int r = P::stage_dots(p);
+        if (r >= 0)
+          for (int h = 0; h < P::N_HEL_EVAL; ++h)
+            for (int c = 0; c < NC; ++c)
+              if (P::has_dots(r, c)) P::dots(r, c, sm.data(), h, &jr[(size_t(h) * NC + c) * CH], &ji[(size_t(h) * NC + c) * CH]);
+      }
+      for (int h = 0; h < P::N_HEL_EVAL; ++h) {
+        double v = 0;
+        for (int ca = 0; ca < NC; ++ca) {
+          const double* ar = &jr[(size_t(h) * NC + ca) * CH]; const double* ai = &ji[(size_t(h) * NC + ca) * CH];
+          v += P::colour_diag(ca, ar, ai);
+          for (int cb = ca + 1; cb < NC; ++cb) v += P::colour_pair(ca, cb, ar, ai, &jr[(size_t(h) * NC + cb) * CH], &ji[(size_t(h) * NC + cb) * CH]);
+        }
+        if (per_hel) per_hel[e * P::N_HEL + P::full_helicity(h, pass)] = v * scale;
+        s += v;
+      }
+    }
+    me2[e] = 2.0 * s * scale;
+  }
+}
+
 template <class P> void eval(const double* mom, double* me2, long long n, double mass, double coupling, double* per_hel, bool split) {
+  if constexpr (P::CHUNKED) {
+    eval_chunked<P>(mom, me2, n, mass, coupling, per_hel);
+    return;
+  } else {
   std::vector<double> sm(P::SMEM_DOUBLES);
   double g2 = 1;
   for (int i = 0; i < P::COUPLING_POWER; ++i) g2 *= coupling;
@@ -77,6 +122,7 @@ template <class P> void eval(const double* mom, double* me2, long long n, double
       s += v;
     }
     me2[e] = 2.0 * s * scale;
+  }
   }
 }
 

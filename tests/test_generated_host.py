@@ -64,6 +64,20 @@ def test_diagram_counts_of_the_hadronic_processes():
     assert len(big.terms) == (1240 - 295) + 3 * 285 + 9 * 10
 
 
+def test_gg_ttxggg_generated_program_matches_oracle(host):
+    """the chunked form (two passes over the helicity of the last gluon, 120 flows in chunks of 20, splits
+    divided into parts over 9 rounds) on the CPU harness against the oracle's tier 1."""
+    w = BY_NAME["gg_ttxggg"]
+    mom = _momenta("gg_ttxggg", 6)
+    out = np.empty(6)
+    hel = np.zeros((6, 128))
+    g = np.sqrt(4 * np.pi * PARAMS["alpha_s"])
+    assert host.host_me_eval(b"gg_ttxggg", mom.ctypes.data, out.ctypes.data, 6, PARAMS["m_top"], g, hel.ctypes.data, 0) == 0
+    expect = ref.MatrixElementRef("gg_ttxggg").eval(mom)
+    assert np.max(np.abs(out / expect - 1)) < 1e-11
+    assert np.max(np.abs(2 * hel.sum(1) / expect - 1)) < 1e-11      # the harness stores each evaluated combination once
+
+
 def test_generator_colour_matrix_golden():
     rows = {}
     for line in open(os.path.join(HERE, "golden", "colour_matrix_rows.txt")):
