@@ -58,7 +58,8 @@ template <class P> struct JPark {
   static constexpr int NFW = P::SPLIT_J ? P::N_FLOW_HALF : P::N_FLOW;   // flows per warp
   static constexpr bool ON = P::N_ROUNDS > 1 || P::SPLIT_J || P::CHUNKED;
   static constexpr int REGS = 4 * NFW;                             // 32-bit columns per warp
-  static constexpr int COLS = tmem_cols(P::CHUNKED ? REGS : (P::N_WARPS / 4) * REGS);  // allocation: a power of two >= 32
+  // allocation: a power of two >= 32; chunked form: one column block per event of a sub-partition
+  static constexpr int COLS = tmem_cols(P::CHUNKED ? ((P::W_EVENTS + 3) / 4) * 4 * P::CHUNK * P::N_CHUNK : (P::N_WARPS / 4) * REGS);
   static __device__ __forceinline__ uint32_t addr(uint32_t base, int warp) {
     return base + (static_cast<uint32_t>(32 * (warp & 3)) << 16) + (warp >> 2) * REGS;
   }
@@ -198,110 +199,140 @@ __device__ __forceinline__ double cta_me2(double* smem, double mass, double scal
   }
 }
 
-// The same for a process whose colour-flow vector does not fit a lane's registers (g g -> t tbar g g g: 120 flows; SURVEY.md
-// §8(f) N2).  The event is evaluated in P::N_PASS passes with the helicities of the frozen legs fixed, so that a lane still
-// holds one helicity combination; J of a pass lives in TENSOR MEMORY (4 N_FLOW 32-bit columns of the warp's 32 lanes) and
-// the dot stages load, update and store it P::CHUNK flows at a time; J^dagger CF J is summed over pairs of chunks.
-// Items: the 32 lanes are W_EVENTS events x VPI helicity variants (lane = event * VPI + variant: the lanes of one event
-// read one 128-byte line).
+// The form with the colour-flow vector in TENSOR MEMORY (P::CHUNKED).  For processes whose J does not fit a lane's registers
+// (g g -> t tbar g g g: 120 flows), and for CTAs with more warps than events, where no warp can afford
+// to keep J in registers.  The event is evaluated in P::N_PASS passes with the helicities of the frozen legs fixed, so that
+// a lane holds one helicity combination; J of a pass occupies 4 N_FLOW 32-bit columns of 32 tensor-memory lanes per event
+// (event e: lanes 32 (e % 4).., column block e / 4).  The unit of work of the dot stages is (event, chunk of P::CHUNK flows):
+// load the chunk, add the round's dot products that feed it, store it back; of the colour stage (event, pair of chunks).
+// A warp reaches only the lanes of its own sub-partition (warp % 4), so the N_WARPS / 4 warps of a sub-partition share the
+// units of its W_EVENTS / 4 events.
+// Items: the 32 lanes are W_EVENTS events x VPI helicity variants.
+template <class P> struct ChunkIO {
+  static constexpr int CH = P::CHUNK;
+  static __device__ __forceinline__ void load(uint32_t taddr, double* jr, double* ji) {
+    uint32_t q[4 * CH];
+    tmem_load<4 * CH>(taddr, q);
+#pragma unroll
+    for (int f = 0; f < CH; ++f) { jr[f] = __hiloint2double(q[4 * f + 1], q[4 * f]); ji[f] = __hiloint2double(q[4 * f + 3], q[4 * f + 2]); }
+  }
+  static __device__ __forceinline__ void store(uint32_t taddr, const double* jr, const double* ji) {
+    uint32_t q[4 * CH];
+#pragma unroll
+    for (int f = 0; f < CH; ++f) {
+      q[4 * f] = __double2loint(jr[f]); q[4 * f + 1] = __double2hiint(jr[f]);
+      q[4 * f + 2] = __double2loint(ji[f]); q[4 * f + 3] = __double2hiint(ji[f]);
+    }
+    tmem_store<4 * CH>(taddr, q);
+  }
+};
+
 template <class P>
 __device__ __forceinline__ double cta_me2_chunked(double* smem, double mass, double scale, double* hel_out, uint32_t tmem) {
   constexpr int STRIDE = EventSmem<P>::DOUBLES;
-  constexpr int W = P::W_EVENTS, VPI = P::VPI, CH = P::CHUNK, NC = P::N_CHUNK;
-  static_assert(W * VPI == 32 && W <= 4 && P::N_HEL_EVAL <= 32 && 4 * CH * NC <= 512, "one event per tensor-memory sub-partition");
+  constexpr int W = P::W_EVENTS, VPI = P::VPI, CH = P::CHUNK, NC = P::N_CHUNK, NW = P::N_WARPS;
+  constexpr int EG = (W + 3) / 4, WG = NW / 4;   // events and warps per tensor-memory sub-partition
+  constexpr int NPAIR = NC * (NC + 1) / 2;
+  static_assert(W * VPI == 32 && (W == 4 || W == 8) && NW % 4 == 0 && P::N_HEL_EVAL <= 32 && EG * 4 * CH * NC <= 512, "geometry");
+  __shared__ double v_part[WG][W][32];
   const int lane = threadIdx.x & 31, warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0);
   double* base = smem + 4 * P::N_EXT;
-  const double* my = base + (warp & (W - 1)) * STRIDE;
-  double* sm_e = base + (lane / VPI) * STRIDE;
-  const int j = lane % VPI;
-  const bool dot_warp = warp < W;
-  const uint32_t tj = tmem + (static_cast<uint32_t>(32 * (warp & 3)) << 16);   // this warp's lanes, column 0
+  // items: eight events -> the lanes of a quarter warp are eight events (their stride is 16 B mod 128 B: no bank
+  // conflict); four events -> the eight lanes of an event read one 128-byte line
+  double* sm_e = base + (VPI == 4 ? lane % W : lane / VPI) * STRIDE;
+  const int j = VPI == 4 ? lane / W : lane % VPI;
+  const int sub = warp & 3, k_w = warp >> 2;
+  const uint32_t tsub = tmem + (static_cast<uint32_t>(32 * sub) << 16);   // this sub-partition's lanes, column 0
   double v = 0.0;
 #pragma unroll 1
   for (int pass = 0; pass < P::N_PASS; ++pass) {
     {
       const int t = threadIdx.x, ev = t % W;
       double* mom_s = smem + ev * STRIDE;
-      me_phase0(t / W, 32 * P::N_WARPS / W, mom_s + 4 * P::N_EXT, mom_s, P::N_EXT, P::N_SUB, d_masks, d_kind, d_massive, d_extoff, mass,
+      me_phase0(t / W, 32 * NW / W, mom_s + 4 * P::N_EXT, mom_s, P::N_EXT, P::N_SUB, d_masks, d_kind, d_massive, d_extoff, mass,
                 P::FROZEN_MASK, P::frozen_helicities(pass));
     }
-    if (dot_warp) {   // J = 0
-      uint32_t z[4 * CH];
+    {   // J = 0
+      double zr[CH], zi[CH];
 #pragma unroll
-      for (int k = 0; k < 4 * CH; ++k) z[k] = 0u;
+      for (int f = 0; f < CH; ++f) { zr[f] = 0.0; zi[f] = 0.0; }
 #pragma unroll 1
-      for (int c = 0; c < NC; ++c) tmem_store<4 * CH>(tj + 4 * CH * c, z);
+      for (int u = k_w; u < EG * NC; u += WG) ChunkIO<P>::store(tsub + (u / NC) * 4 * CH * NC + 4 * CH * (u % NC), zr, zi);
     }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     int it = 0;
 #pragma unroll 1
     for (int p = 0; p < P::N_STAGES; ++p) {
       const int end = P::stage_end(p);
 #pragma unroll 1
-      for (int i = it + warp; i < end; i += P::N_WARPS) me_run_item<true, VPI>(c_items[i], c_members, j, sm_e, mass);
+      for (int i = it + warp; i < end; i += NW) me_run_item<(NW <= 12), VPI>(c_items[i], c_members, j, sm_e, mass);
       it = end;
       __syncthreads();
       const int r = P::stage_dots(p);
       if (r >= 0) {
-        if (dot_warp) {
+        // the (event, chunk) units of this sub-partition that the round feeds, dealt to its warps in turn
+        int n = 0;
 #pragma unroll 1
-          for (int c = 0; c < NC; ++c) {
-            if (!P::has_dots(r, c)) continue;
-            double jr[CH], ji[CH];
-            {
-              uint32_t q[4 * CH];
-              tmem_load<4 * CH>(tj + 4 * CH * c, q);
-#pragma unroll
-              for (int f = 0; f < CH; ++f) { jr[f] = __hiloint2double(q[4 * f + 1], q[4 * f]); ji[f] = __hiloint2double(q[4 * f + 3], q[4 * f + 2]); }
-            }
-            if (lane < P::N_HEL_EVAL) P::dots(r, c, my, lane, jr, ji);
-            {
-              uint32_t q[4 * CH];
-#pragma unroll
-              for (int f = 0; f < CH; ++f) {
-                q[4 * f] = __double2loint(jr[f]); q[4 * f + 1] = __double2hiint(jr[f]);
-                q[4 * f + 2] = __double2loint(ji[f]); q[4 * f + 3] = __double2hiint(ji[f]);
-              }
-              tmem_store<4 * CH>(tj + 4 * CH * c, q);
-            }
-          }
+        for (int u = 0; u < EG * NC; ++u) {
+          const int ei = u / NC, c = u % NC;
+          if (!P::has_dots(r, c)) continue;
+          if ((n++) % WG != k_w) continue;
+          if (4 * ei + sub >= W) continue;
+          const uint32_t ta = tsub + ei * 4 * CH * NC + 4 * CH * c;
+          double jr[CH], ji[CH];
+          ChunkIO<P>::load(ta, jr, ji);
+          if (lane < P::N_HEL_EVAL) P::dots(r, c, base + (4 * ei + sub) * STRIDE, lane, jr, ji);
+          ChunkIO<P>::store(ta, jr, ji);
         }
-        __syncthreads();   // the next round's items (or the next pass) overwrite the round region
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();   // the next round's items (or the next pass) overwrite the round region; J is complete
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
       }
     }
-    // a9, a10: J^dagger CF J over chunks and pairs of chunks; this pass's helicities
-    if (dot_warp) {
-      double vp = 0.0;
-#pragma unroll 1
-      for (int ca = 0; ca < NC; ++ca) {
-        double ar[CH], ai[CH];
-        {
-          uint32_t q[4 * CH];
-          tmem_load<4 * CH>(tj + 4 * CH * ca, q);
+    // a9, a10: J^dagger CF J over (event, pair of chunks) units; this pass's helicities
+    double vp[EG];
 #pragma unroll
-          for (int f = 0; f < CH; ++f) { ar[f] = __hiloint2double(q[4 * f + 1], q[4 * f]); ai[f] = __hiloint2double(q[4 * f + 3], q[4 * f + 2]); }
-        }
-        vp += P::colour_diag(ca, ar, ai);
+    for (int ei = 0; ei < EG; ++ei) vp[ei] = 0.0;
 #pragma unroll 1
-        for (int cb = ca + 1; cb < NC; ++cb) {
-          double br[CH], bi[CH];
-          uint32_t q[4 * CH];
-          tmem_load<4 * CH>(tj + 4 * CH * cb, q);
-#pragma unroll
-          for (int f = 0; f < CH; ++f) { br[f] = __hiloint2double(q[4 * f + 1], q[4 * f]); bi[f] = __hiloint2double(q[4 * f + 3], q[4 * f + 2]); }
-          vp += P::colour_pair(ca, cb, ar, ai, br, bi);
-        }
+    for (int u = k_w; u < EG * NPAIR; u += WG) {
+      const int ei = u / NPAIR;
+      int q = u % NPAIR, ca = 0;
+      while (q >= NC - ca) { q -= NC - ca; ++ca; }
+      const int cb = ca + q;
+      double ar[CH], ai[CH], t;
+      ChunkIO<P>::load(tsub + ei * 4 * CH * NC + 4 * CH * ca, ar, ai);
+      if (cb == ca) {
+        t = P::colour_diag(ca, ar, ai);
+      } else {
+        double br[CH], bi[CH];
+        ChunkIO<P>::load(tsub + ei * 4 * CH * NC + 4 * CH * cb, br, bi);
+        t = P::colour_pair(ca, cb, ar, ai, br, bi);
       }
-      if (lane >= P::N_HEL_EVAL) vp = 0.0;
+#pragma unroll
+      for (int e2 = 0; e2 < EG; ++e2) vp[e2] += (e2 == ei) ? t : 0.0;
+    }
+#pragma unroll
+    for (int ei = 0; ei < EG; ++ei)
+      if (4 * ei + sub < W) v_part[k_w][4 * ei + sub][lane] = (lane < P::N_HEL_EVAL) ? vp[ei] : 0.0;
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    if (warp < W) {
+      double t = 0.0;
+#pragma unroll
+      for (int k = 0; k < WG; ++k) t += v_part[k][warp][lane];
       if (hel_out && lane < P::N_HEL_EVAL) {   // the parity partner has every helicity flipped
         const int hf = P::full_helicity(lane, pass);
-        hel_out[hf] = vp * scale;
-        hel_out[(P::N_HEL - 1) ^ hf] = vp * scale;
+        hel_out[hf] = t * scale;
+        hel_out[(P::N_HEL - 1) ^ hf] = t * scale;
       }
-      v += vp;
+      v += t;
     }
+    if (pass + 1 < P::N_PASS) __syncthreads();   // v_part is rewritten by the next pass
   }
-  if (!dot_warp) return 0.0;
+  if (warp >= W) return 0.0;
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
   return 2.0 * v * scale;

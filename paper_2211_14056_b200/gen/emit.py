@@ -34,12 +34,15 @@ N_ROUNDS = int(os.environ.get("MADME_GEN_ROUNDS", "0"))   # 0: the fewest rounds
 # is fixed during one PASS over the event (leg 0 always: parity; more legs = 2^(len-1) passes, each summing the other
 # helicities, so that one lane still holds one helicity combination and J of one pass fits tensor memory); chunk: colour
 # flows held in registers at a time by the dot stages (0: all of them), the others wait in tensor memory.
-GEOMETRY = {"gg_ttxggg": dict(w_events=4, frozen=(0, 6), chunk=int(os.environ.get("MADME_GEN_CHUNK", "20")))}
+GEOMETRY = {"gg_ttxggg": dict(w_events=4, frozen=(0, 6), chunk=int(os.environ.get("MADME_GEN_CHUNK7", "15")),
+                              n_warps=int(os.environ.get("MADME_GEN_WARPS7", "12")))}
+if os.environ.get("MADME_GEN_CHUNK6"):      # g g -> t tbar g g with J in tensor memory and more warps than events
+    GEOMETRY["gg_ttxgg"] = dict(chunk=int(os.environ["MADME_GEN_CHUNK6"]), n_warps=int(os.environ.get("MADME_GEN_WARPS6", "12")))
 FROZEN = (0,)        # set per process by emit_process
 
 
 def geometry(name):
-    g = dict(w_events=W_EVENTS, frozen=(0,), chunk=0)
+    g = dict(w_events=W_EVENTS, frozen=(0,), chunk=0, n_warps=N_WARPS)
     g.update(GEOMETRY.get(name, {}))
     return g
 
@@ -366,9 +369,9 @@ def emit_process(name, n_rounds=None):
 
 
 def _emit_process(name, n_rounds, geo):
-    W_EV, CHUNK = geo["w_events"], geo["chunk"]
+    W_EV, CHUNK, NWARPS = geo["w_events"], geo["chunk"], geo["n_warps"]
     VPI = 32 // W_EV
-    DOTS_C_PER_U = N_WARPS > W_EV and not CHUNK
+    DOTS_C_PER_U = NWARPS > W_EV or bool(CHUNK)
     P = Program(name, frozen=FROZEN)
     assert all(t.op.startswith("DOT") for t in P.terms), "every diagram must be a propagator-cut contraction"
     L = Layout(P, n_rounds) if n_rounds else pick_rounds(P, smem_budget_doubles(W_EV))
@@ -412,7 +415,7 @@ def _emit_process(name, n_rounds, geo):
             for cost, t, vbase in pending:
                 items.append(encode_item(t, vbase))
         else:
-            queues = [[0, []] for _ in range(N_WARPS)]
+            queues = [[0, []] for _ in range(NWARPS)]
             for cost, t, vbase in pending:
                 q = min(queues, key=lambda x: x[0])
                 q[0] += cost
@@ -532,8 +535,8 @@ def _emit_process(name, n_rounds, geo):
 
     w("  static constexpr int N_ITEMS = %d, N_MEMBERS = %d, N_ROUNDS = %d, N_STAGES = %d, N_TASKS = %d, N_UNITS = %d;"
       % (len(items), len(members), len(L.rounds), len(stage_end), n_tasks, n_units))
-    w("  static constexpr int N_WARPS = %d;" % N_WARPS)
-    w("  // stage p: items up to stage_end(p) (warp w takes items w, w + %d, ...), barrier, then the dot products of round" % N_WARPS)
+    w("  static constexpr int N_WARPS = %d;" % NWARPS)
+    w("  // stage p: items up to stage_end(p) (warp w takes items w, w + %d, ...), barrier, then the dot products of round" % NWARPS)
     w("  // stage_dots(p) (if >= 0), barrier")
     table_fn("stage_end", stage_end)
     table_fn("stage_dots", stage_dots)
@@ -695,8 +698,8 @@ def _emit_process(name, n_rounds, geo):
     fca = emit_colour("colour_cross_a(%s)" % four, cross_a)
     fcb0 = emit_colour("colour_cross_b0(%s)" % four, cross_b0)
     fcb1 = emit_colour("colour_cross_b1(%s)" % four, cross_b1)
-    w("  static constexpr bool SPLIT_J = %s;" % ("true" if N_WARPS == 2 * W_EV else "false"))
-    if N_WARPS == 2 * W_EV:
+    w("  static constexpr bool SPLIT_J = %s;" % ("true" if NWARPS == 2 * W_EV else "false"))
+    if NWARPS == 2 * W_EV:
         amp_flops, col_flops = flops_a + flops_b, fa_ + fb_ + fca + fcb0 + fcb1
     ext_flops = FLOPS_EXT * 2 * n
     nh = 1 << len(hel_legs)
@@ -819,7 +822,13 @@ def emit_all(out_dir=OUT_DIR, only=None, force=False):
     os.makedirs(out_dir, exist_ok=True)
     paths = []
     newest = max(os.path.getmtime(os.path.join(HERE, f)) for f in ("emit.py", "diagrams.py"))
-    force = force or any(k.startswith("MADME_GEN_") for k in os.environ)
+    # the MADME_GEN_* overrides the existing files were generated with
+    stamp_path = os.path.join(out_dir, ".overrides")
+    stamp = repr(sorted((k, v) for k, v in os.environ.items() if k.startswith("MADME_GEN_")))
+    if (open(stamp_path).read() if os.path.exists(stamp_path) else "[]") != stamp:
+        force = True
+    with open(stamp_path, "w") as f:
+        f.write(stamp)
     for name in PROCESSES:
         if only and name not in only:
             continue
