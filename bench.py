@@ -313,6 +313,36 @@ def main():
                      "integral_pb_last": lastv["integral"], "sigma_pb_last": lastv["variance"] ** 0.5,
                      "integral_pb_combined": comb, "sigma_pb_combined": sum(wts) ** -0.5, "chi2_per_dof": chi2}
 
+    # SURVEY §8(f) N1 / N2 beside the headline: me_eval of the quark-initiated 2 -> 4 channels and of g g -> t tbar g g g
+    # (the paper's thesis: the gap grows with the number of diagrams), a short extra leg outside the timed
+    # region; device-resident RAMBO momenta of each workload's own stream
+    channels = None
+    if not vegas and world == 1 and wl.name == "config3" and not args.no_vegas_leg:
+        channels = {}
+        for name in ("qqx_ttxgg", "qg_ttxqg", "gg_ttxggg"):
+            wc = BY_NAME[name]
+            nc = min(wc.n_events, args.events or wc.n_events)
+            hc = api.me_init(wc.process, PARAMS)
+            rc = api.philox_uniform(wc.seed, 0, 0, wc.n_dim, nc)
+            mc, _ = api.rambo_generate(rc, wc.sqrt_s, wc.masses, wc.ps_mode)
+            oc = torch.empty(nc, dtype=torch.float64, device="cuda")
+            for _ in range(2):
+                api.me_eval(hc, mc, oc)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            for _ in range(3):
+                api.me_eval(hc, mc, oc)
+            b.record(stream)
+            torch.cuda.synchronize()
+            msc = a.elapsed_time(b) / 3
+            fl = api.me_flops_per_event(hc)
+            channels[name] = {"events": nc, "kernel_ms": msc, "events_per_s": nc / (msc * 1e-3), "flops_per_event": fl,
+                              "tflops": fl * nc / (msc * 1e-3) / 1e12, "frac_of_measured": fl * nc / (msc * 1e-3) / 1e12 / probe_tflops,
+                              "diagrams": api.me_info(hc, 0), "colour_flows": api.me_info(hc, 3), "regs_per_thread": api.me_info(hc, 8),
+                              "events_per_cta": api.me_info(hc, 7)}
+            del hc, rc, mc, oc
+            torch.cuda.empty_cache()
+
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -346,6 +376,8 @@ def main():
         out["vegas"] = last
     elif vegas_leg is not None:
         out["vegas"] = vegas_leg
+    if channels:
+        out["channels"] = channels
     print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()

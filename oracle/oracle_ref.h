@@ -13,7 +13,15 @@
  *   philox/rambo/cuts
  *   vegas_*            SURVEY.md §8(c) G6, G7 (Lepage's Vegas)
  * Parity status: every function below is pinned by tests/test_oracle_*.py (closed forms,
- * Ward identity, Lorentz/basis/Bose invariance, tier 0 <-> tier 1, RAMBO identities) except:
+ * Ward identity, Lorentz/basis/Bose invariance, tier 0 <-> tier 1, RAMBO identities).  The quark-initiated channels
+ * (tier 0 with two fermion lines, tier 1 in the diagram basis) are pinned by the q qbar -> t tbar closed form, the
+ * diagram counts behind PAPER.md:57-58 (36 = 16 + 4 x 5, 267 = 123 + 4 x 36), tier 0 <-> tier 1 per amplitude and in
+ * the sums, Ward / Lorentz / basis / Bose / charge-conjugation invariance, and by running the diagram basis on the gg
+ * channels against the flow basis (tests/test_oracle_quark_channels.py); not pinned: the crossing relation between
+ * q qbar -> t tbar g and q g -> t tbar q (it needs wavefunctions at unphysical momenta).  g g -> t tbar g g g: counts,
+ * colour-matrix properties, the flow decomposition against tier-0 amplitudes, Ward / Lorentz / Bose invariance
+ * (tests/test_oracle_gg_ttxggg.py); its full tier-0 colour sum is out of reach ("parity pinned per amplitude only").
+ * Exceptions:
  *   - the Philox BIT PATTERN: pinned against a library Philox4x32-10 where one is importable
  *     (see tests/test_oracle_phase_space.py); otherwise "parity unpinned" beyond CPU == GPU.
  *   - the Vegas grid-update details (alpha = 1.5, 3-point smoothing): a READING,
