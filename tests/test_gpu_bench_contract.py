@@ -40,6 +40,10 @@ def test_default_workload_line():
     assert len(v["events_per_s_per_iteration"]) == 5 and min(v["events_per_s_per_iteration"]) > 1e6
     assert v["integral_pb_combined"] > 0 and v["sigma_pb_combined"] > 0 and 0 < v["cut_pass_fraction_last"] <= 1
     assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
+    ch = d["channels"]                              # SURVEY 8(f) N1 / N2 beside the headline
+    assert set(ch) == {"qqx_ttxgg", "qg_ttxqg", "gg_ttxggg"}
+    assert ch["gg_ttxggg"]["diagrams"] == 1240 and ch["gg_ttxggg"]["colour_flows"] == 120 and ch["qqx_ttxgg"]["diagrams"] == 36
+    assert all(c["events_per_s"] > 1e5 and 0.02 < c["frac_of_measured"] < 1.0 for c in ch.values())
 
 
 def test_vegas_workload_line():
