@@ -24,6 +24,12 @@
 #define MADME_INC(p) MADME_STR(generated/p.inc)
 #include MADME_INC(MADME_PROC)
 #include "tmem.cuh"
+#ifndef MADME_PREFETCH_CHUNKED
+#define MADME_PREFETCH_CHUNKED 1   // g g -> t tbar g g g: 1.45 M events/s (0: 1.39 M)
+#endif
+#ifndef MADME_PREFETCH
+#define MADME_PREFETCH 0   // 0: the next member's operands are fetched after the accumulation (58.7 M events/s); 1: one member ahead, copied (56.9 M); 2: between vertex and accumulation (56.8 M)
+#endif
 
 namespace madme {
 
@@ -126,7 +132,7 @@ __device__ __forceinline__ double cta_me2(double* smem, double mass, double scal
   for (int p = 0; p < P::N_STAGES; ++p) {
     const int end = P::stage_end(p);
 #pragma unroll 1
-    for (int i = it + warp; i < end; i += P::N_WARPS) me_run_item<!SPLIT>(c_items[i], c_members, j, sm_e, mass);
+    for (int i = it + warp; i < end; i += P::N_WARPS) me_run_item<MADME_PREFETCH>(c_items[i], c_members, j, sm_e, mass);
     it = end;
     __syncthreads();
     const int r = P::stage_dots(p);
@@ -267,7 +273,7 @@ __device__ __forceinline__ double cta_me2_chunked(double* smem, double mass, dou
     for (int p = 0; p < P::N_STAGES; ++p) {
       const int end = P::stage_end(p);
 #pragma unroll 1
-      for (int i = it + warp; i < end; i += NW) me_run_item<(NW <= 12), VPI>(c_items[i], c_members, j, sm_e, mass);
+      for (int i = it + warp; i < end; i += NW) me_run_item<MADME_PREFETCH_CHUNKED, VPI>(c_items[i], c_members, j, sm_e, mass);
       it = end;
       __syncthreads();
       const int r = P::stage_dots(p);

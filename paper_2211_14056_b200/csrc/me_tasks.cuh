@@ -37,8 +37,9 @@ namespace madme {
 //   w2: out0 | out1 << 16,  w3: out2 | out3 << 16          (offsets in doubles into the event's scratch, variant 0)
 // One member (32 B) = one bare vertex:
 //   w0: op | ksub_a << 8 | ksub_b << 16
-//   w1: a | b << 16,   w2: c | vmap_c << 16,   w3: vmap_a | vmap_b << 16
-//        (vmap: 4 bits per local variant j: which variant of the argument enters variant vbase + j of the outputs)
+//   w1: a | b << 16,   w2: c,   w3: vmap_a,   w5: vmap_b,   w6: vmap_c
+//        (vmap: which variant of the argument enters local variant j of the outputs.  VPI = 4: one byte per j, the
+//        variant's offset in 16-byte slots; VPI = 8: four bits per j, the variant index)
 //   w4: code of term 0 | code of term 1 << 9 | code of term 2 << 18      (see acc_term; terms 1, 2 exist for the
 //        four-gluon vertex only)
 struct MeItem { unsigned w0, w1, w2, w3; };
@@ -162,16 +163,14 @@ ME_HD void acc_term(wf4 (&acc)[ME_NSLOT], const wf4& x, unsigned code, bool wide
 // i + 1 before member i is evaluated (32 more registers; for CTAs with two warps per scheduler).
 // double offset of helicity variant v inside a stored object (gen/emit.py::voff): 16-byte slots of a 128-byte line; an
 // object with 16 variants continues in the next group of four lines
-// (VPI = 4, eight events per CTA: the generator asserts that no object has more than 8 variants, so this is 2 v)
-template <int VPI> ME_HD int me_voff(unsigned v) { return VPI == 4 ? static_cast<int>(2u * v) : static_cast<int>(2u * (v & 7u) + 64u * (v >> 3)); }
-// the variant of an argument that enters local variant j of the item: 4-bit entries; VPI = 4: a and b share word 3, c
-// sits in the high half of word 2; VPI = 8: words 3, 5, 6
-template <int VPI> ME_HD unsigned me_vmap_a(const MeMember* m, int j) { return VPI == 4 ? (m->w[3] >> (4 * j)) & 15u : (m->w[3] >> (4 * j)) & 15u; }
-template <int VPI> ME_HD unsigned me_vmap_b(const MeMember* m, int j) { return VPI == 4 ? (m->w[3] >> (16 + 4 * j)) & 15u : (m->w[5] >> (4 * j)) & 15u; }
-template <int VPI> ME_HD unsigned me_vmap_c(const MeMember* m, int j) { return VPI == 4 ? (m->w[2] >> (16 + 4 * j)) & 15u : (m->w[6] >> (4 * j)) & 15u; }
-
-template <bool PREFETCH, int VPI = 4>
+ME_HD int me_voff(unsigned v) { return static_cast<int>(2u * (v & 7u) + 64u * (v >> 3)); }
+// double offset of the variant of an argument that enters local variant j of the item (tables above)
+template <int VPI> ME_HD int me_arg_off(unsigned word, int j) {
+  return VPI == 4 ? static_cast<int>(2u * ((word >> (8 * j)) & 0xffu)) : me_voff((word >> (4 * j)) & 15u);
+}
+template <int PREFETCH, int VPI = 4>
 ME_HD void me_run_item(const MeItem H, const MeMember* __restrict__ members, int j, double* __restrict__ sm, double mass) {
+#define ME_LD_ARG(off) ld_wf(sm + (off))
   const int n_mem = H.w0 & 0xff;
   const int nv = (H.w0 >> 16) & 0xff, v = static_cast<int>(H.w0 >> 24) + j;
   if (n_mem == 0 || v >= nv) return;
@@ -181,27 +180,48 @@ ME_HD void me_run_item(const MeItem H, const MeMember* __restrict__ members, int
   for (int s = 0; s < ME_NSLOT; ++s)
     for (int c = 0; c < 4; ++c) acc[s].c[c] = mk(0.0, 0.0);
   const MeMember* m = members + (H.w1 & 0xffff);
-  unsigned w0 = m->w[0], w2 = m->w[2], w4 = m->w[4], vc = VPI == 4 ? 0u : me_vmap_c<VPI>(m, j);
+  unsigned w0 = m->w[0], w2 = m->w[2], w4 = m->w[4], w6 = m->w[6];
   wf4 A, B;
   {
     const unsigned w1 = m->w[1];
-    A = ld_wf(sm + (w1 & 0xffff) + me_voff<VPI>(me_vmap_a<VPI>(m, j)));
-    B = ld_wf(sm + (w1 >> 16) + me_voff<VPI>(me_vmap_b<VPI>(m, j)));
+    A = ME_LD_ARG((w1 & 0xffff) + me_arg_off<VPI>(m->w[3], j));
+    B = ME_LD_ARG((w1 >> 16) + me_arg_off<VPI>(m->w[5], j));
   }
 #if defined(__CUDA_ARCH__)
 #pragma unroll 1
 #endif
   for (int i = 0; i < n_mem; ++i) {
-    const unsigned c0 = w0, c2 = w2, c4 = w4, cvc = vc;
+    const unsigned c0 = w0, c2 = w2, c4 = w4, c6 = w6;
     const wf4 a = A, b = B;
-    if (PREFETCH ? (i + 1 < n_mem) : false) {
-      ++m;
-      const unsigned w1 = m->w[1];
-      w0 = m->w[0]; w2 = m->w[2]; w4 = m->w[4]; vc = VPI == 4 ? 0u : me_vmap_c<VPI>(m, j);
-      A = ld_wf(sm + (w1 & 0xffff) + me_voff<VPI>(me_vmap_a<VPI>(m, j)));
-      B = ld_wf(sm + (w1 >> 16) + me_voff<VPI>(me_vmap_b<VPI>(m, j)));
+    // the operands of member i + 1: PREFETCH 1 before member i is evaluated (copies), 2 between its vertex and its
+    // accumulation (no copies: a and b are dead by then), 0 after it
+#define ME_FETCH_NEXT()                                                                         \
+    if (i + 1 < n_mem) {                                                                        \
+      ++m;                                                                                      \
+      const unsigned w1 = m->w[1];                                                              \
+      w0 = m->w[0]; w2 = m->w[2]; w4 = m->w[4]; w6 = m->w[6];                                    \
+      A = ME_LD_ARG((w1 & 0xffff) + me_arg_off<VPI>(m->w[3], j));                                \
+      B = ME_LD_ARG((w1 >> 16) + me_arg_off<VPI>(m->w[5], j));                                   \
     }
+    if (PREFETCH == 1) { ME_FETCH_NEXT() }
     const int op = c0 & 0xff;
+    if (PREFETCH == 2) {
+      wf4 t1, t2, t3;
+      if (op == OP_SLASH_ROW) t1 = slash_row(a, b);
+      else if (op == OP_SLASH_COL) t1 = slash_col(b, a);
+      else if (op == OP_FFV_VEC) t1 = ffv_vec_bare(a, b);
+      else if (op == OP_VVV) t1 = vvv_vec_bare(a, ld_k(sm + 8 * ((c0 >> 8) & 0xff)), b, ld_k(sm + 8 * ((c0 >> 16) & 0xff)));
+      else {
+        const wf4 C = ME_LD_ARG((c2 & 0xffff) + me_arg_off<VPI>(c6, j));
+        vvvv_vec_bare(a, b, C, t1, t2, t3);
+      }
+      ME_FETCH_NEXT()
+      acc_term(acc, t1, c4 & 0x1ffu, wide);
+      if (op == OP_VVVV) {
+        acc_term(acc, t2, (c4 >> 9) & 0x1ffu, wide);
+        acc_term(acc, t3, (c4 >> 18) & 0x1ffu, wide);
+      }
+    } else {
     if (op == OP_SLASH_ROW) {
       acc_term(acc, slash_row(a, b), c4 & 0x1ffu, wide);
     } else if (op == OP_SLASH_COL) {
@@ -211,34 +231,31 @@ ME_HD void me_run_item(const MeItem H, const MeMember* __restrict__ members, int
     } else if (op == OP_VVV) {
       acc_term(acc, vvv_vec_bare(a, ld_k(sm + 8 * ((c0 >> 8) & 0xff)), b, ld_k(sm + 8 * ((c0 >> 16) & 0xff))), c4 & 0x1ffu, wide);
     } else {
-      const wf4 C = ld_wf(sm + (c2 & 0xffff) + me_voff<VPI>(VPI == 4 ? (c2 >> (16 + 4 * j)) & 15u : cvc));
+      const wf4 C = ME_LD_ARG((c2 & 0xffff) + me_arg_off<VPI>(c6, j));
       wf4 t1, t2, t3;
       vvvv_vec_bare(a, b, C, t1, t2, t3);
       acc_term(acc, t1, c4 & 0x1ffu, wide);
       acc_term(acc, t2, (c4 >> 9) & 0x1ffu, wide);
       acc_term(acc, t3, (c4 >> 18) & 0x1ffu, wide);
     }
-    if (!PREFETCH && i + 1 < n_mem) {
-      ++m;
-      const unsigned w1 = m->w[1];
-      w0 = m->w[0]; w2 = m->w[2]; w4 = m->w[4]; vc = VPI == 4 ? 0u : me_vmap_c<VPI>(m, j);
-      A = ld_wf(sm + (w1 & 0xffff) + me_voff<VPI>(me_vmap_a<VPI>(m, j)));
-      B = ld_wf(sm + (w1 >> 16) + me_voff<VPI>(me_vmap_b<VPI>(m, j)));
     }
+    if (PREFETCH == 0) { ME_FETCH_NEXT() }
+#undef ME_FETCH_NEXT
+#undef ME_LD_ARG
   }
   // the common propagator, once per colour-ordered current
   const double* ks = sm + 8 * (H.w1 >> 16);
   const unsigned outs[ME_NSLOT] = {H.w2 & 0xffff, H.w2 >> 16, H.w3 & 0xffff, H.w3 >> 16};
   if (kind == KIND_OPEN) {
     for (int s = 0; s < ME_NSLOT; ++s)
-      if (s < n_out) st_wf(sm + outs[s] + me_voff<VPI>(v), acc[s]);
+      if (s < n_out) st_wf(sm + outs[s] + me_voff(v), acc[s]);
   } else if (kind == KIND_VEC) {
     const double f = ks[4];
     for (int s = 0; s < ME_NSLOT; ++s)
       if (s < n_out) {
         wf4 y;
         for (int c = 0; c < 4; ++c) y.c[c] = f * acc[s].c[c];
-        st_wf(sm + outs[s] + me_voff<VPI>(v), y);
+        st_wf(sm + outs[s] + me_voff(v), y);
       }
   } else {
     const bool massive = (H.w0 >> 15) & 1;
@@ -246,10 +263,10 @@ ME_HD void me_run_item(const MeItem H, const MeMember* __restrict__ members, int
     const vec4 K = ld_k(ks);
     if (kind == KIND_ROW) {
       for (int s = 0; s < ME_NSLOT; ++s)
-        if (s < n_out) st_wf(sm + outs[s] + me_voff<VPI>(v), prop_row(K, -1.0, mm, f, acc[s]));
+        if (s < n_out) st_wf(sm + outs[s] + me_voff(v), prop_row(K, -1.0, mm, f, acc[s]));
     } else {
       for (int s = 0; s < ME_NSLOT; ++s)
-        if (s < n_out) st_wf(sm + outs[s] + me_voff<VPI>(v), prop_col(K, 1.0, mm, f, acc[s]));
+        if (s < n_out) st_wf(sm + outs[s] + me_voff(v), prop_col(K, 1.0, mm, f, acc[s]));
     }
   }
 }

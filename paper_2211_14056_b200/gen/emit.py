@@ -451,9 +451,10 @@ def _emit_process(name, n_rounds, geo):
             assert max(offs) < 65536
             ks = [sub_i(a.legs) for a in args[:2]]
             code = lambda term: u.swap[term] | (sum(c << (2 * sl) for sl, c in enumerate(u.sign[term])) << 1)
-            if VPI == 4:    # four 4-bit entries per argument
-                members.append((u.op | (ks[0] << 8) | (ks[1] << 16), offs[0] | (offs[1] << 16), offs[2] | (vmaps[2] << 16),
-                                vmaps[0] | (vmaps[1] << 16), code(0) | (code(1) << 9) | (code(2) << 18), 0, 0, 0))
+            if VPI == 4:    # four entries per argument, one byte each: the variant's offset in 16-byte slots
+                slot = lambda vm: sum((voff((vm >> (4 * j)) & 15) // 2) << (8 * j) for j in range(4))
+                members.append((u.op | (ks[0] << 8) | (ks[1] << 16), offs[0] | (offs[1] << 16), offs[2],
+                                slot(vmaps[0]), code(0) | (code(1) << 9) | (code(2) << 18), slot(vmaps[1]), slot(vmaps[2]), 0))
             else:           # eight 4-bit entries per argument: a word each (w3, w5, w6)
                 assert VPI == 8
                 members.append((u.op | (ks[0] << 8) | (ks[1] << 16), offs[0] | (offs[1] << 16), offs[2],

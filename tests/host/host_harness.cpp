@@ -36,8 +36,10 @@ FOR_EACH_PROCESS(DEF_TABLES)
 template <class P> void items(double* sm, int begin, int end, double mass) {
   for (int it = begin; it < end; ++it)
     for (int j = 0; j < P::VPI; ++j) {
-      if (it & 1) me_run_item<true, P::VPI>(Tables<P>::items()[it], Tables<P>::members(), j, sm, mass);   // both forms of the member loop
-      else me_run_item<false, P::VPI>(Tables<P>::items()[it], Tables<P>::members(), j, sm, mass);
+      // all three forms of the member loop
+      if (it % 3 == 1) me_run_item<1, P::VPI>(Tables<P>::items()[it], Tables<P>::members(), j, sm, mass);
+      else if (it % 3 == 2) me_run_item<2, P::VPI>(Tables<P>::items()[it], Tables<P>::members(), j, sm, mass);
+      else me_run_item<0, P::VPI>(Tables<P>::items()[it], Tables<P>::members(), j, sm, mass);
     }
 }
 
