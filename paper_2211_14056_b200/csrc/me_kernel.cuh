@@ -278,13 +278,12 @@ __device__ __forceinline__ double cta_me2_chunked(double* smem, double mass, dou
       __syncthreads();
       const int r = P::stage_dots(p);
       if (r >= 0) {
-        // the (event, chunk) units of this sub-partition that the round feeds, dealt to its warps in turn
-        int n = 0;
+        // the (event, chunk) units of this sub-partition that the round feeds, dealt to its warps by cost (generator)
 #pragma unroll 1
         for (int u = 0; u < EG * NC; ++u) {
           const int ei = u / NC, c = u % NC;
           if (!P::has_dots(r, c)) continue;
-          if ((n++) % WG != k_w) continue;
+          if ((P::dot_owner(r, c) + ei) % WG != k_w) continue;
           if (4 * ei + sub >= W) continue;
           const uint32_t ta = tsub + ei * 4 * CH * NC + 4 * CH * c;
           double jr[CH], ji[CH];

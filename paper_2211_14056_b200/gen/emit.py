@@ -35,6 +35,7 @@ N_ROUNDS = int(os.environ.get("MADME_GEN_ROUNDS", "0"))   # 0: the fewest rounds
 # helicities, so that one lane still holds one helicity combination and J of one pass fits tensor memory); chunk: colour
 # flows held in registers at a time by the dot stages (0: all of them), the others wait in tensor memory.
 GEOMETRY = {"gg_ttxggg": dict(w_events=4, frozen=(0, 6), chunk=int(os.environ.get("MADME_GEN_CHUNK7", "15")),
+                              split_items=os.environ.get("MADME_GEN_SPLIT7", "1") == "1",
                               n_warps=int(os.environ.get("MADME_GEN_WARPS7", "12")))}
 if os.environ.get("MADME_GEN_CHUNK6"):      # g g -> t tbar g g with J in tensor memory and more warps than events
     GEOMETRY["gg_ttxgg"] = dict(chunk=int(os.environ["MADME_GEN_CHUNK6"]), n_warps=int(os.environ.get("MADME_GEN_WARPS6", "12")))
@@ -395,10 +396,44 @@ def _emit_process(name, n_rounds, geo):
 
     out_phase = {}        # stored object id -> a: true current = i^a x stored current
 
+    def makespan(task_list):
+        """longest-processing-time-first makespan of the stage's items over the warps, and the task that ends last"""
+        pend = sorted(((L.task_flops(t), k) for k, t in enumerate(task_list) for _ in range(0, L.nv(t.outputs[0]), VPI)), reverse=True)
+        q = [[0, -1] for _ in range(NWARPS)]
+        for c, k in pend:
+            b = min(q, key=lambda x: x[0])
+            b[0] += c
+            b[1] = k if b[1] < 0 or L.task_flops(task_list[k]) > L.task_flops(task_list[b[1]]) else b[1]
+        worst = max(q, key=lambda x: x[0])
+        return worst[0], worst[1]
+
+    def split_for_balance(task_list, fixed_zero):
+        """A stage ends when its longest warp does.  With few large items per stage (g g -> t tbar g g g: 11-16 items over 12
+        warps, the largest with 36 bare vertices) the largest item IS the stage: split the largest task of the critical warp
+        by outputs (two currents each instead of four; the bare vertices both halves need are evaluated twice) while that
+        shortens the stage."""
+        start = list(task_list)
+        task_list = list(task_list)
+        for _ in range(64):
+            mean = sum(L.task_flops(t) * ((L.nv(t.outputs[0]) + VPI - 1) // VPI) for t in task_list) / NWARPS
+            cands = [k for k, t in enumerate(task_list) if len(t.outputs) >= 2 and L.task_flops(t) > 1.2 * mean]
+            if not cands:
+                break
+            k = max(cands, key=lambda k: L.task_flops(task_list[k]))
+            t = task_list[k]
+            half = (len(t.outputs) + 1) // 2
+            parts = L.make_tasks(t.outputs[:half], fixed_zero) + L.make_tasks(t.outputs[half:], fixed_zero)
+            if max(L.task_flops(p) for p in parts) > 0.9 * L.task_flops(t):
+                break       # the halves share nearly every bare vertex: nothing to gain
+            task_list = task_list[:k] + parts + task_list[k + 1:]
+        return task_list if makespan(task_list)[0] < 0.97 * makespan(start)[0] else start
+
     def add_stage(task_list, dots_round):
         """Items of the tasks, balanced over the warps by estimated cost (longest first), then interleaved so that
         warp w runs items w, w + W_EVENTS, ... of the stage."""
         nonlocal cur_flops, n_tasks, n_units
+        if geo.get("split_items"):
+            task_list = split_for_balance(task_list, dots_round < 0)
         pending = []
         for t in task_list:
             o = t.outputs[0]
@@ -629,7 +664,7 @@ def _emit_process(name, n_rounds, geo):
     w("  // a7-a8: the dot products of round r for helicity combination h (bit k of h is the helicity of the k-th leg that")
     w("  // is not frozen, 0 <-> -1, 1 <-> +1), accumulated into the colour-flow vector J = (jr, ji).")
     if CHUNK:
-        return _emit_chunked(W, w, P, L, nf, CHUNK, n_pass, n, cur_flops, emit_round_body, hel_bits)
+        return _emit_chunked(W, w, P, L, nf, CHUNK, n_pass, n, cur_flops, emit_round_body, hel_bits, NWARPS)
     amp_flops = emit_dots("dots", set(range(nf)), {f: f for f in range(nf)})
 
     # ---- colour contraction grouped by distinct CF numerator (9 distinct values for 4 gluons) ----
@@ -715,7 +750,7 @@ def _emit_process(name, n_rounds, geo):
     return "\n".join(W) + "\n"
 
 
-def _emit_chunked(W, w, P, L, nf, CHUNK, n_pass, n, cur_flops, emit_round_body, hel_bits):
+def _emit_chunked(W, w, P, L, nf, CHUNK, n_pass, n, cur_flops, emit_round_body, hel_bits, NWARPS):
     """The dot and colour stages of a process whose colour-flow vector does not fit the registers of a lane: J lives in
     tensor memory (4 N_FLOW 32-bit columns of the warp's lanes), CHUNK flows at a time are loaded, updated by the dot
     products of the round that feed them, and stored back; J^dagger CF J is summed over pairs of chunks."""
@@ -723,6 +758,7 @@ def _emit_chunked(W, w, P, L, nf, CHUNK, n_pass, n, cur_flops, emit_round_body, 
     chunk_of = lambda f: f // CHUNK
     flops = ncon = 0
     has = []
+    unit_cost = {}
     w("  // dot products of round r that feed the colour flows of chunk c (flow f = c * CHUNK + index into jr / ji)")
     w("  static ME_HD void dots(int r, int c, const double* __restrict__ sm, int h, double* __restrict__ jr, double* __restrict__ ji) {")
     hel_bits()
@@ -740,6 +776,7 @@ def _emit_chunked(W, w, P, L, nf, CHUNK, n_pass, n, cur_flops, emit_round_body, 
             flops += fl
             ncon += k
             has.append(r * nc + c)
+            unit_cost[(r, c)] = fl
     w("      default: break;")
     w("    }")
     w("  }")
@@ -749,6 +786,24 @@ def _emit_chunked(W, w, P, L, nf, CHUNK, n_pass, n, cur_flops, emit_round_body, 
         w("      case %d:" % k)
     w("        return true;")
     w("      default: return false;")
+    w("    }")
+    w("  }")
+    # which of the WG warps of a tensor-memory sub-partition takes the (event, chunk) unit of round r: longest first
+    wg = NWARPS // 4
+    owner = {}
+    for r in range(len(L.rounds)):
+        load = [0] * wg
+        for c in sorted((c for (rr, c) in unit_cost if rr == r), key=lambda c: -unit_cost[(r, c)]):
+            k = load.index(min(load))
+            load[k] += unit_cost[(r, c)]
+            owner[(r, c)] = k
+    w("  // the warp (index within the %d warps of a tensor-memory sub-partition) that takes chunk c in round r: by cost" % wg)
+    w("  static ME_HD int dot_owner(int r, int c) {")
+    w("    switch (r * N_CHUNK + c) {")
+    for (r, c), k in sorted(owner.items()):
+        if k:
+            w("      case %d: return %d;" % (r * nc + c, k))
+    w("      default: return 0;")
     w("    }")
     w("  }")
     w("  static constexpr int N_CONTRACTIONS = %d;  // per helicity combination (a contraction shared by flows of different chunks counts twice)" % ncon)
