@@ -51,7 +51,8 @@ __device__ const int d_extoff[] = MADME_TAB(_EXT_OFF);
 // (neighbouring lanes in the current stages) falls into different banks.
 template <class P> struct EventSmem {
   static constexpr int RAW = 4 * P::N_EXT + P::SMEM_DOUBLES;
-  static constexpr int DOUBLES = ((RAW + 13) / 16) * 16 + 2;
+  // eight events: 16 B mod 128 B; four events (eight variants = one line per event and component): half a line
+  static constexpr int DOUBLES = ((RAW + 13) / 16) * 16 + (P::VPI == 8 ? 8 : 2);
 };
 
 // Events per CTA: P::W_EVENTS (gen/emit.py: the item tables are laid out for it; 8, or 4 for g g -> t tbar g g g).  A CTA
