@@ -210,6 +210,13 @@ int vegas_refine_ref(double* edges, int n_dim, int n_bins, const double* S, doub
 // Toy gluon density of the hadronic mode (reading R-N3): g(x) = 3 x^-1.2 (1-x)^5.
 // A DECLARED toy parametrisation (no LHAPDF grids in the container); it only has to be the same on both sides.
 static double toy_gluon_density(double x) { return 3.0 * std::pow(x, -1.2) * std::pow(1.0 - x, 5); }
+// The beams of the quark-initiated channels (SURVEY §8(f) N1 x N3): DECLARED toys as well, a valence-like quark density
+// q(x) = 2 x^-0.5 (1-x)^3 and a sea-like antiquark density qbar(x) = 0.3 x^-1.1 (1-x)^7.
+static double toy_density(int leg_kind, double x) {
+  if (leg_kind == F_IN) return 2.0 * std::pow(x, -0.5) * std::pow(1.0 - x, 3);
+  if (leg_kind == FB_IN) return 0.3 * std::pow(x, -1.1) * std::pow(1.0 - x, 7);
+  return toy_gluon_density(x);
+}
 
 // f(x) = jac_Vegas * W_ps * Theta_cuts * me2 / (2 s) * C,  C = 0.3893793721e9 pb GeV^2
 // ps_mode 2 (hadronic, D = 3n-4+2): x_1 = x[0], x_2 = x[1] are the momentum fractions, s_hat = x_1 x_2 s, the remaining
@@ -240,7 +247,7 @@ int vegas_integrand_ref(me_handle_ref* h, const vegas_grid_ref* g, double sqrt_s
       if (rs_hat > msum) {
         const double wps = rambo_event(x + 2, rs_hat, masses.data(), nf, 1, mom);
         if (passes_cuts(mom, nf, isg.data(), h->par.ptj_min, h->par.dr_min))
-          val = jac * toy_gluon_density(x[0]) * toy_gluon_density(x[1]) * wps * me2_tier1(*h, mom) / (2.0 * rs_hat * rs_hat) * conv;
+          val = jac * toy_density(h->P.kind[0], x[0]) * toy_density(h->P.kind[1], x[1]) * wps * me2_tier1(*h, mom) / (2.0 * rs_hat * rs_hat) * conv;
       }
     } else {
       const double wps = rambo_event(x, sqrt_s, masses.data(), nf, g->ps_mode, mom);
@@ -312,7 +319,7 @@ int vegas_generate_ref(me_handle_ref* h, const vegas_grid_ref* g, double sqrt_s,
     if (g->ps_mode == 2) {
       const double rs_hat = std::sqrt(x[0] * x[1]) * sqrt_s;
       if (rs_hat > msum) {
-        weights[k] = jac * toy_gluon_density(x[0]) * toy_gluon_density(x[1]) * rambo_event(x + 2, rs_hat, masses.data(), nf, 1, mom) /
+        weights[k] = jac * toy_density(h->P.kind[0], x[0]) * toy_density(h->P.kind[1], x[1]) * rambo_event(x + 2, rs_hat, masses.data(), nf, 1, mom) /
                      (2.0 * rs_hat * rs_hat) * conv;
       } else {
         weights[k] = 0;

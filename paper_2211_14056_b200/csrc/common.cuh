@@ -37,6 +37,7 @@ struct me_handle {
   double mass, scale, flops;
   double masses[madme::PS_MAX_FINAL];
   unsigned gluon_mask;
+  int beam_kind[2] = {0, 0};  // toy density of each beam in the hadronic Vegas mode: 0 gluon, 1 quark, 2 antiquark
   // launch geometry of the CTA-per-W-events kernels
   int warps, grid, smem_bytes, regs, ctas_per_sm, sms;
   int device = 0;  // the device that was current in me_init: every call runs there

@@ -207,7 +207,7 @@ __global__ void vegas_generate_kernel(VegasArgs a, const long long* __restrict__
     for (int i = 0; i < NF; ++i) msum += a.masses[i];
     rs = sqrt(x[0] * x[1]) * a.sqrt_s;
     ok = rs > msum;
-    if (ok) w = jac * toy_gluon_density(x[0]) * toy_gluon_density(x[1]) * rambo_event<NF>(x + 2, rs, a.masses, 1, rambo_volume(NF, rs * rs), p) *
+    if (ok) w = jac * toy_density(a.beam_kind[0], x[0]) * toy_density(a.beam_kind[1], x[1]) * rambo_event<NF>(x + 2, rs, a.masses, 1, rambo_volume(NF, rs * rs), p) *
                 (PB_GEV2 / (2.0 * rs * rs));
   } else {
     w = jac * rambo_event<NF>(x, a.sqrt_s, a.masses, a.ps_mode, a.w0, p) * a.prefactor;
@@ -239,7 +239,7 @@ void fill_args(const me_handle* h, const vegas_grid* g, double sqrt_s, long long
   a.iteration = static_cast<unsigned>(g->iteration); a.first_event = first_event; a.n_ev = n_ev; a.sqrt_s = sqrt_s;
   a.w0 = rambo_volume(nf, sqrt_s * sqrt_s); a.prefactor = PB_GEV2 / (2.0 * sqrt_s * sqrt_s);
   for (int i = 0; i < PS_MAX_FINAL; ++i) a.masses[i] = h->masses[i];
-  a.gluon_mask = h->gluon_mask; a.ptj_min = h->par.ptj_min; a.dr_min = h->par.dr_min; a.mass = h->mass; a.scale = h->scale;
+  a.gluon_mask = h->gluon_mask; a.beam_kind[0] = h->beam_kind[0]; a.beam_kind[1] = h->beam_kind[1]; a.ptj_min = h->par.ptj_min; a.dr_min = h->par.dr_min; a.mass = h->mass; a.scale = h->scale;
 }
 
 }  // namespace

@@ -226,6 +226,15 @@ __device__ __forceinline__ double toy_gluon_density(double x) {
   return 3.0 * pow(x, -1.2) * (y2 * y2 * y);
 }
 
+// the beams of the quark-initiated channels (N1 x N3): declared toys as well.  kind: 0 gluon, 1 quark: 2 x^-0.5 (1-x)^3,
+// 2 antiquark: 0.3 x^-1.1 (1-x)^7
+__device__ __forceinline__ double toy_density(int kind, double x) {
+  if (kind == 0) return toy_gluon_density(x);
+  const double y = 1.0 - x, y2 = y * y;
+  if (kind == 1) return 2.0 * rsqrt(x) * (y2 * y);
+  return 0.3 * pow(x, -1.1) * (y2 * y2 * y2 * y);
+}
+
 // ---- a4: cuts (DESIGN.md R-G5) -----------------------------------------------------------------------------
 // every final gluon: pT > ptj_min and DeltaR(g, X) = sqrt(dy^2 + dphi^2) > dr_min to every other final parton;
 // true rapidity; strict inequalities; a cut value <= 0 is off.  gluon_mask bit i <-> final particle i is a gluon.

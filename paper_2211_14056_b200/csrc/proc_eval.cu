@@ -41,6 +41,7 @@ int fill(me_handle* h) {
   // final-state particle i (leg i + 2): its mass, and whether the jet cuts apply to it (massless coloured partons)
   for (int i = 0; i < PS_MAX_FINAL; ++i) h->masses[i] = ((P::FINAL_MASSIVE_MASK >> i) & 1) ? h->par.m_top : 0.0;
   h->gluon_mask = P::JET_MASK;
+  h->beam_kind[0] = P::BEAM_KIND_0; h->beam_kind[1] = P::BEAM_KIND_1;
   const double g2 = P::QED ? 4.0 * PS_PI * h->par.alpha_em : 4.0 * PS_PI * h->par.alpha_s;  // g^2
   double c = 1.0;
   for (int i = 0; i < P::COUPLING_POWER / 2; ++i) c *= g2;

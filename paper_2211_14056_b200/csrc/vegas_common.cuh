@@ -20,6 +20,7 @@ struct VegasArgs {
   double sqrt_s, w0, prefactor;  // prefactor = C / (2 s)
   double masses[PS_MAX_FINAL];
   unsigned gluon_mask;
+  int beam_kind[2];  // hadronic mode: the toy density of each beam (0 gluon, 1 quark, 2 antiquark)
   double ptj_min, dr_min, mass, scale;
 };
 

@@ -56,7 +56,7 @@ __global__ void __launch_bounds__(32 * P::N_WARPS, 1) vegas_integrand_kernel(Veg
           if (rs > msum) {
             const double wps = rambo_event<NF>(x + 2, rs, a.masses, 1, rambo_volume(NF, rs * rs), p);
             pass = passes_cuts<NF>(p, a.gluon_mask, a.ptj_min, a.dr_min);
-            w = jac * toy_gluon_density(x[0]) * toy_gluon_density(x[1]) * wps * (PB_GEV2 / (2.0 * rs * rs));
+            w = jac * toy_density(a.beam_kind[0], x[0]) * toy_density(a.beam_kind[1], x[1]) * wps * (PB_GEV2 / (2.0 * rs * rs));
           }
         } else {
           const double wps = rambo_event<NF>(x, a.sqrt_s, a.masses, a.ps_mode, a.w0, p);

@@ -40,6 +40,8 @@ GEOMETRY = {"gg_ttxggg": dict(w_events=4, frozen=(0, 6), chunk=int(os.environ.ge
 if os.environ.get("MADME_GEN_CHUNK6"):      # g g -> t tbar g g with J in tensor memory and more warps than events
     GEOMETRY["gg_ttxgg"] = dict(chunk=int(os.environ["MADME_GEN_CHUNK6"]), n_warps=int(os.environ.get("MADME_GEN_WARPS6", "12")))
 FROZEN = (0,)        # set per process by emit_process
+LPT_PER_UNIT = int(os.environ.get("MADME_GEN_LPT_UNIT", "120"))   # 0 / 0: 58.6 M, 60 / 120: 59.2 M, 120 / 240: 59.7 M, 200 / 100: 58.5 M events/s (g g -> t tbar g g)
+LPT_PER_ITEM = int(os.environ.get("MADME_GEN_LPT_ITEM", "240"))
 
 
 def geometry(name):
@@ -444,7 +446,8 @@ def _emit_process(name, n_rounds, geo):
             n_units += len(t.units)
             cur_flops += L.task_flops(t) * nv
             for vbase in range(0, nv, VPI):
-                pending.append((L.task_flops(t), t, vbase))
+                # the balance cost adds the interpreter's overhead per bare vertex and per item (fetch, decode, stores)
+                pending.append((L.task_flops(t) + LPT_PER_UNIT * len(t.units) + LPT_PER_ITEM, t, vbase))
         pending.sort(key=lambda x: -x[0])
         if DYNAMIC:     # handed out through a shared counter, longest first
             for cost, t, vbase in pending:
@@ -555,6 +558,8 @@ def _emit_process(name, n_rounds, geo):
     w("  static constexpr int CF_DEN = %d, AVG_DEN = %d, COUPLING_POWER = %d;  // me2 = g^(2*(n-2)) sum / (CF_DEN*AVG_DEN)"
       % (P.cf_den, P.avg, 2 * (n - 2)))
     w("  static constexpr bool QED = %s;" % ("true" if P.coupling == "ee" else "false"))
+    beam = lambda leg: {0: 0, 4: 1, 5: 2}[leg.kind]      # V_IN gluon, F_IN quark, FB_IN antiquark
+    w("  static constexpr int BEAM_KIND_0 = %d, BEAM_KIND_1 = %d;  // toy density of each beam in the hadronic Vegas mode" % (beam(P.legs[0]), beam(P.legs[1])))
     w("  // final-state particle i = leg i + 2: massive (m_top), a jet (massless coloured parton: the cuts apply to it)")
     w("  static constexpr unsigned FINAL_MASSIVE_MASK = %d, JET_MASK = %d;"
       % (sum(1 << (l - 2) for l in range(2, n) if P.legs[l].massive),

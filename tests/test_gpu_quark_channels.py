@@ -102,6 +102,23 @@ def test_vegas_integrand_matches_oracle(handles, proc, mode, n):
     assert np.max(np.abs(sg - so) / (np.abs(so) + 1e-300 + 1e-12 * np.abs(so).max())) < 1e-9
 
 
+@pytest.mark.parametrize("proc", ["qg_ttxqg", "qqx_ttxgg"])
+def test_vegas_hadronic_mode_matches_oracle(handles, proc):
+    """ps_mode 2 with the declared toy quark / antiquark / gluon density of each beam (DESIGN.md R-N3): the hadronic
+    channels behind the paper's p p -> t tbar g g."""
+    D, n = 3 * 4 - 2, 1500 + 3
+    go = ref.GridRef(D, VEGAS_BINS, VEGAS_ALPHA, seed=10, ps_mode=2)
+    gg = api.VegasGrid(D, VEGAS_BINS, VEGAS_ALPHA, 10, 2)
+    so, fo = ref.MatrixElementRef(proc).vegas_integrand(go, 13000.0, 9, n, want_f=True)
+    sg, fg = api.vegas_integrand(handles[proc], gg, 13000.0, 9, n, want_f=True)
+    sg, fg = sg.cpu().numpy(), fg.cpu().numpy()
+    assert np.array_equal(fg != 0, fo != 0)
+    nz = fo != 0
+    assert nz.sum() > 100
+    assert np.max(np.abs(fg[nz] / fo[nz] - 1)) < ME_RTOL
+    assert np.max(np.abs(sg - so) / (np.abs(so) + 1e-300 + 1e-12 * np.abs(so).max())) < 1e-9
+
+
 def test_cuts_apply_to_the_final_light_quark():
     w = BY_NAME["qg_ttxqg"]
     mom = oracle_events("qg_ttxqg", 20000)

@@ -102,8 +102,14 @@ def test_refine_hand_case():
     assert abs(e[1] - want1) < 1e-14 and abs(e[2] - want2) < 1e-14 and e[0] == 0 and e[3] == 1
 
 
-def test_hadronic_mode_factorises_into_pinned_pieces():
-    """ps_mode 2 (DESIGN.md R-N3): f = jac g(x1) g(x2) x [the partonic integrand at sqrt(s_hat) =
+import pytest  # noqa: E402
+
+
+@pytest.mark.parametrize("proc", ["gg_ttxgg", "qg_ttxqg", "qqx_ttxgg"])
+def test_hadronic_mode_factorises_into_pinned_pieces(proc):
+    """The beams of the quark-initiated channels (N1 x N3) carry their own DECLARED toy densities: quark
+    2 x^-0.5 (1-x)^3, antiquark 0.3 x^-1.1 (1-x)^7 (checked by hand at x = 1/4).
+    ps_mode 2 (DESIGN.md R-N3): f = jac g(x1) g(x2) x [the partonic integrand at sqrt(s_hat) =
     sqrt(x1 x2 S)].  Every factor on the right is produced by an already pinned routine called separately (vegas_map,
     rambo_generate in diet mode at sqrt(s_hat), cuts, tier-1 |M|^2); the toy density 3 x^-1.2 (1-x)^5 is the declared
     reading, checked at x = 1/4 where it is 3 * 4^1.2 * (3/4)^5 by hand.  Also: events below threshold give exactly 0."""
@@ -116,12 +122,16 @@ def test_hadronic_mode_factorises_into_pinned_pieces():
     e = np.sort(rng.uniform(size=(10, 51)), axis=1)
     e[:, 0], e[:, -1] = 0.0, 1.0
     g.edges[:] = e
-    me = ref.MatrixElementRef("gg_ttxgg")
+    me = ref.MatrixElementRef(proc)
     sums, f = me.vegas_integrand(g, S, 5, n, want_f=True)
     y = ref.philox_uniform(9, 0, 5, 10, n)
     x, jac, idx = ref.vegas_map(e, y)
-    dens = lambda t: 3.0 * t ** -1.2 * (1.0 - t) ** 5
-    assert abs(dens(0.25) - 3 * 4 ** 1.2 * 0.75 ** 5) < 1e-12
+    glu = lambda t: 3.0 * t ** -1.2 * (1.0 - t) ** 5
+    qrk = lambda t: 2.0 * t ** -0.5 * (1.0 - t) ** 3
+    aqk = lambda t: 0.3 * t ** -1.1 * (1.0 - t) ** 7
+    assert abs(glu(0.25) - 3 * 4 ** 1.2 * 0.75 ** 5) < 1e-12 and abs(qrk(0.25) - 2 * 2 * 0.75 ** 3) < 1e-12
+    assert abs(aqk(0.25) - 0.3 * 4 ** 1.1 * 0.75 ** 7) < 1e-12
+    dens1, dens2 = {"gg_ttxgg": (glu, glu), "qg_ttxqg": (qrk, glu), "qqx_ttxgg": (qrk, aqk)}[proc]
     masses = (173.0, 173.0, 0.0, 0.0)
     want = np.zeros(n)
     for i in range(n):
@@ -130,7 +140,7 @@ def test_hadronic_mode_factorises_into_pinned_pieces():
             continue
         mom, w = ref.rambo_generate(x[i:i + 1, 2:], rs, masses, 1)
         if ref.cuts(mom, (0, 0, 1, 1), PARAMS["ptj_min"], PARAMS["dr_min"])[0]:
-            want[i] = jac[i] * dens(x[i, 0]) * dens(x[i, 1]) * w[0] * me.eval(mom)[0] / (2 * rs * rs) * 0.3893793721e9
+            want[i] = jac[i] * dens1(x[i, 0]) * dens2(x[i, 1]) * w[0] * me.eval(mom)[0] / (2 * rs * rs) * 0.3893793721e9
     assert np.array_equal(f != 0, want != 0) and (want == 0).any() and (want != 0).sum() > 100
     nz = want != 0
     assert np.max(np.abs(f[nz] / want[nz] - 1)) < 1e-12
