@@ -133,7 +133,7 @@ __device__ __forceinline__ double cta_me2(double* smem, double mass, double scal
   for (int p = 0; p < P::N_STAGES; ++p) {
     const int end = P::stage_end(p);
 #pragma unroll 1
-    for (int i = it + warp; i < end; i += P::N_WARPS) me_run_item<MADME_PREFETCH>(c_items[i], c_members, j, sm_e, mass);
+    for (int i = it + warp; i < end; i += P::N_WARPS) me_run_item<MADME_PREFETCH, 4, P::NSLOT>(c_items[i], c_members, j, sm_e, mass);
     it = end;
     __syncthreads();
     const int r = P::stage_dots(p);
@@ -274,7 +274,7 @@ __device__ __forceinline__ double cta_me2_chunked(double* smem, double mass, dou
     for (int p = 0; p < P::N_STAGES; ++p) {
       const int end = P::stage_end(p);
 #pragma unroll 1
-      for (int i = it + warp; i < end; i += NW) me_run_item<MADME_PREFETCH_CHUNKED, VPI>(c_items[i], c_members, j, sm_e, mass);
+      for (int i = it + warp; i < end; i += NW) me_run_item<MADME_PREFETCH_CHUNKED, VPI, P::NSLOT>(c_items[i], c_members, j, sm_e, mass);
       it = end;
       __syncthreads();
       const int r = P::stage_dots(p);

@@ -46,7 +46,7 @@ struct MeItem { unsigned w0, w1, w2, w3; };
 struct MeMember { unsigned w[8]; };
 enum MeOp { OP_SLASH_ROW = 0, OP_SLASH_COL = 1, OP_FFV_VEC = 2, OP_VVV = 3, OP_VVVV = 4 };
 enum MeKind { KIND_VEC = 0, KIND_ROW = 1, KIND_COL = 2, KIND_OPEN = 3 };
-constexpr int ME_NSLOT = 4;
+constexpr int ME_NSLOT = 4;   // most accumulators of an item (gen/emit.py::NSLOT; a process may be generated with 2)
 
 constexpr int ME_WF_STRIDE = 16;  // doubles between the components of a stored wavefunction (one 128-byte line)
 ME_HD wf4 ld_wf(const double* p) {
@@ -140,21 +140,21 @@ ME_HD void acc_plain(wf4& acc, const wf4& x, double e) {
 ME_HD void acc_times_i(wf4& acc, const wf4& x, double e) {
   for (int c = 0; c < 4; ++c) { acc.c[c].re = fma(-e, x.c[c].im, acc.c[c].re); acc.c[c].im = fma(e, x.c[c].re, acc.c[c].im); }
 }
-ME_HD void acc_term(wf4 (&acc)[ME_NSLOT], const wf4& x, unsigned code, bool wide) {
+template <int NS> ME_HD void acc_term(wf4 (&acc)[NS], const wf4& x, unsigned code, bool wide) {
   const double e0 = sign_of((code >> 1) & 3u), e1 = sign_of((code >> 3) & 3u);
   if (code & 1u) {
     acc_times_i(acc[0], x, e0);
     acc_times_i(acc[1], x, e1);
-    if (wide) {
-      acc_times_i(acc[2], x, sign_of((code >> 5) & 3u));
-      acc_times_i(acc[3], x, sign_of((code >> 7) & 3u));
+    if (NS > 2 && wide) {
+      acc_times_i(acc[NS > 2 ? 2 : 0], x, sign_of((code >> 5) & 3u));
+      acc_times_i(acc[NS > 2 ? 3 : 0], x, sign_of((code >> 7) & 3u));
     }
   } else {
     acc_plain(acc[0], x, e0);
     acc_plain(acc[1], x, e1);
-    if (wide) {
-      acc_plain(acc[2], x, sign_of((code >> 5) & 3u));
-      acc_plain(acc[3], x, sign_of((code >> 7) & 3u));
+    if (NS > 2 && wide) {
+      acc_plain(acc[NS > 2 ? 2 : 0], x, sign_of((code >> 5) & 3u));
+      acc_plain(acc[NS > 2 ? 3 : 0], x, sign_of((code >> 7) & 3u));
     }
   }
 }
@@ -168,7 +168,7 @@ ME_HD int me_voff(unsigned v) { return static_cast<int>(2u * (v & 7u) + 64u * (v
 template <int VPI> ME_HD int me_arg_off(unsigned word, int j) {
   return VPI == 4 ? static_cast<int>(2u * ((word >> (8 * j)) & 0xffu)) : me_voff((word >> (4 * j)) & 15u);
 }
-template <int PREFETCH, int VPI = 4>
+template <int PREFETCH, int VPI = 4, int NS = ME_NSLOT>
 ME_HD void me_run_item(const MeItem H, const MeMember* __restrict__ members, int j, double* __restrict__ sm, double mass) {
 #define ME_LD_ARG(off) ld_wf(sm + (off))
   const int n_mem = H.w0 & 0xff;
@@ -176,8 +176,8 @@ ME_HD void me_run_item(const MeItem H, const MeMember* __restrict__ members, int
   if (n_mem == 0 || v >= nv) return;
   const int n_out = (H.w0 >> 8) & 0xf, kind = (H.w0 >> 12) & 7;
   const bool wide = n_out > 2;
-  wf4 acc[ME_NSLOT];
-  for (int s = 0; s < ME_NSLOT; ++s)
+  wf4 acc[NS];
+  for (int s = 0; s < NS; ++s)
     for (int c = 0; c < 4; ++c) acc[s].c[c] = mk(0.0, 0.0);
   const MeMember* m = members + (H.w1 & 0xffff);
   unsigned w0 = m->w[0], w2 = m->w[2], w4 = m->w[4], w6 = m->w[6];
@@ -245,13 +245,13 @@ ME_HD void me_run_item(const MeItem H, const MeMember* __restrict__ members, int
   }
   // the common propagator, once per colour-ordered current
   const double* ks = sm + 8 * (H.w1 >> 16);
-  const unsigned outs[ME_NSLOT] = {H.w2 & 0xffff, H.w2 >> 16, H.w3 & 0xffff, H.w3 >> 16};
+  const unsigned outs[4] = {H.w2 & 0xffff, H.w2 >> 16, H.w3 & 0xffff, H.w3 >> 16};
   if (kind == KIND_OPEN) {
-    for (int s = 0; s < ME_NSLOT; ++s)
+    for (int s = 0; s < NS; ++s)
       if (s < n_out) st_wf(sm + outs[s] + me_voff(v), acc[s]);
   } else if (kind == KIND_VEC) {
     const double f = ks[4];
-    for (int s = 0; s < ME_NSLOT; ++s)
+    for (int s = 0; s < NS; ++s)
       if (s < n_out) {
         wf4 y;
         for (int c = 0; c < 4; ++c) y.c[c] = f * acc[s].c[c];
@@ -262,10 +262,10 @@ ME_HD void me_run_item(const MeItem H, const MeMember* __restrict__ members, int
     const double mm = massive ? mass : 0.0, f = ks[4];
     const vec4 K = ld_k(ks);
     if (kind == KIND_ROW) {
-      for (int s = 0; s < ME_NSLOT; ++s)
+      for (int s = 0; s < NS; ++s)
         if (s < n_out) st_wf(sm + outs[s] + me_voff(v), prop_row(K, -1.0, mm, f, acc[s]));
     } else {
-      for (int s = 0; s < ME_NSLOT; ++s)
+      for (int s = 0; s < NS; ++s)
         if (s < n_out) st_wf(sm + outs[s] + me_voff(v), prop_col(K, 1.0, mm, f, acc[s]));
     }
   }

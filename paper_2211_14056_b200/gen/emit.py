@@ -25,6 +25,7 @@ from .diagrams import PROCESSES, Program
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 OUT_DIR = os.path.join(os.path.dirname(HERE), "csrc", "generated")
+NSLOT_MAX = 4
 NSLOT = 4            # accumulators (colour-ordered currents) per item
 W_EVENTS = 8         # events per CTA (default geometry)
 N_WARPS = int(os.environ.get("MADME_GEN_WARPS", "8"))   # warps per CTA: W_EVENTS own an event in the dot stages, all run items
@@ -34,7 +35,7 @@ N_ROUNDS = int(os.environ.get("MADME_GEN_ROUNDS", "0"))   # 0: the fewest rounds
 # is fixed during one PASS over the event (leg 0 always: parity; more legs = 2^(len-1) passes, each summing the other
 # helicities, so that one lane still holds one helicity combination and J of one pass fits tensor memory); chunk: colour
 # flows held in registers at a time by the dot stages (0: all of them), the others wait in tensor memory.
-GEOMETRY = {"gg_ttxggg": dict(w_events=4, frozen=(0, 6), chunk=int(os.environ.get("MADME_GEN_CHUNK7", "15")),
+GEOMETRY = {"gg_ttxggg": dict(w_events=4, frozen=(0, 6), chunk=int(os.environ.get("MADME_GEN_CHUNK7", "15")), nslot=4,
                               split_items=os.environ.get("MADME_GEN_SPLIT7", "1") == "1",
                               n_warps=int(os.environ.get("MADME_GEN_WARPS7", "12")))}
 if os.environ.get("MADME_GEN_CHUNK6"):      # g g -> t tbar g g with J in tensor memory and more warps than events
@@ -45,7 +46,7 @@ LPT_PER_ITEM = int(os.environ.get("MADME_GEN_LPT_ITEM", "240"))
 
 
 def geometry(name):
-    g = dict(w_events=W_EVENTS, frozen=(0,), chunk=0, n_warps=N_WARPS)
+    g = dict(w_events=W_EVENTS, frozen=(0,), chunk=0, n_warps=N_WARPS, nslot=int(os.environ.get("MADME_GEN_NSLOT", "4")))
     g.update(GEOMETRY.get(name, {}))
     return g
 
@@ -93,9 +94,9 @@ class Unit:
 
     def __init__(self, op, args):
         self.op, self.args = op, args
-        self.codes = [[0] * NSLOT for _ in range(3)]     # [term][slot] -> 0 | 4 + k  (coefficient i^k)
+        self.codes = [[0] * NSLOT_MAX for _ in range(3)]     # [term][slot] -> 0 | 4 + k  (coefficient i^k)
         self.swap = [0, 0, 0]                            # [term] -> b: the term enters as i^b x   (Task.solve_phases)
-        self.sign = [[0] * NSLOT for _ in range(3)]      # [term][slot] -> 0 none | 1 plus | 2 minus
+        self.sign = [[0] * NSLOT_MAX for _ in range(3)]      # [term][slot] -> 0 none | 1 plus | 2 minus
 
 
 class Task:
@@ -362,13 +363,14 @@ def pick_rounds(P, budget):
 
 
 def emit_process(name, n_rounds=None):
-    global FROZEN
+    global FROZEN, NSLOT
     geo = geometry(name)
     FROZEN = tuple(geo["frozen"])
+    NSLOT = geo["nslot"]
     try:
         return _emit_process(name, n_rounds, geo)
     finally:
-        FROZEN = (0,)
+        FROZEN, NSLOT = (0,), 4
 
 
 def _emit_process(name, n_rounds, geo):
@@ -497,7 +499,7 @@ def _emit_process(name, n_rounds, geo):
                 assert VPI == 8
                 members.append((u.op | (ks[0] << 8) | (ks[1] << 16), offs[0] | (offs[1] << 16), offs[2],
                                 vmaps[0], code(0) | (code(1) << 9) | (code(2) << 18), vmaps[1], vmaps[2], 0))
-        outs = [L.off[x.id] for x in t.outputs] + [0] * NSLOT
+        outs = [L.off[x.id] for x in t.outputs] + [0] * NSLOT_MAX
         assert first < 65536 and len(t.units) < 256 and nv < 256
         w0 = len(t.units) | (len(t.outputs) << 8) | (L.kind_of(o) << 12) | (massive_of(o) << 15) | (nv << 16) | (vbase << 24)
         return (w0, first | (sub_i(o.legs) << 16), outs[0] | (outs[1] << 16), outs[2] | (outs[3] << 16))
@@ -542,6 +544,7 @@ def _emit_process(name, n_rounds, geo):
     w("  static constexpr int W_EVENTS = %d, VPI = %d, N_PASS = %d, CHUNK = %d, N_CHUNK = %d;"
       % (W_EV, VPI, n_pass, CHUNK, (nf + CHUNK - 1) // CHUNK if CHUNK else 1))
     w("  static constexpr bool CHUNKED = %s;" % ("true" if CHUNK else "false"))
+    w("  static constexpr int NSLOT = %d;  // accumulators (colour-ordered currents) per item" % NSLOT)
     w("  static constexpr unsigned FROZEN_MASK = %d;" % sum(1 << l for l in FROZEN))
     w("  // helicity of every leg (bit l) for lane index h of pass p; leg 0 at +1")
     w("  static ME_HD int full_helicity(int h, int p) {")

@@ -37,9 +37,9 @@ template <class P> void items(double* sm, int begin, int end, double mass) {
   for (int it = begin; it < end; ++it)
     for (int j = 0; j < P::VPI; ++j) {
       // all three forms of the member loop
-      if (it % 3 == 1) me_run_item<1, P::VPI>(Tables<P>::items()[it], Tables<P>::members(), j, sm, mass);
-      else if (it % 3 == 2) me_run_item<2, P::VPI>(Tables<P>::items()[it], Tables<P>::members(), j, sm, mass);
-      else me_run_item<0, P::VPI>(Tables<P>::items()[it], Tables<P>::members(), j, sm, mass);
+      if (it % 3 == 1) me_run_item<1, P::VPI, P::NSLOT>(Tables<P>::items()[it], Tables<P>::members(), j, sm, mass);
+      else if (it % 3 == 2) me_run_item<2, P::VPI, P::NSLOT>(Tables<P>::items()[it], Tables<P>::members(), j, sm, mass);
+      else me_run_item<0, P::VPI, P::NSLOT>(Tables<P>::items()[it], Tables<P>::members(), j, sm, mass);
     }
 }
 
