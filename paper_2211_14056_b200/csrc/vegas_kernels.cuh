@@ -12,6 +12,50 @@ namespace madme {
 // L2) so that the CTA then evaluates |M|^2 of exactly the surviving events, W at a time, whatever warp generated them;
 // cut events cost no matrix element.  Output per event: f (8 B) and the D bin indices packed one byte each
 // (n_bins <= 255) into idx_out[ev][ceil(D/8)].
+// One event of the stream: Philox -> Vegas map -> RAMBO -> cuts (steps a1-a4).  Writes the packed bin indices of the
+// event; returns whether it passes the cuts, its final-state momenta p, the weight w without |M|^2 and sqrt(s_hat).
+// NOT inlined: the prologue keeps 8 momenta, 24 uniforms and 24 mapped coordinates live, and inlined into the kernel it
+// made ptxas spill inside the matrix-element part (724 B); as a function it has its own register allocation.
+template <int NF>
+__device__ __noinline__ bool vegas_generate_one(const VegasArgs& a, long long ev, unsigned long long* __restrict__ idx_out, int idx_words,
+                                                double (&p)[NF][4], double& w, double& rs) {
+  double y[VEGAS_MAX_DIM], x[VEGAS_MAX_DIM];
+  unsigned long long packed[VEGAS_IDX_WORDS] = {};   // one byte per dimension
+  bool pass = false;
+  w = 0.0;
+  rs = a.sqrt_s;
+  philox_fill<VEGAS_MAX_DIM>(a.seed, a.iteration, static_cast<uint64_t>(a.first_event + ev), a.n_dim, y);
+  double jac = 1.0;
+#pragma unroll
+  for (int d = 0; d < VEGAS_MAX_DIM; ++d) {
+    if (d < a.n_dim) {
+      int bin;
+      x[d] = vegas_map_1d(a.edges + d * (a.n_bins + 1), a.n_bins, y[d], jac, bin);
+      packed[d >> 3] |= static_cast<unsigned long long>(bin) << (8 * (d & 7));
+    } else {
+      x[d] = 0.5;
+    }
+  }
+  if (a.ps_mode == 2) {
+    // hadronic mode (DESIGN.md R-N3): x[0], x[1] are the momentum fractions, the rest drives RAMBO on diet at sqrt(s_hat)
+    double msum = 0.0;
+#pragma unroll
+    for (int i = 0; i < NF; ++i) msum += a.masses[i];
+    rs = sqrt(x[0] * x[1]) * a.sqrt_s;
+    if (rs > msum) {
+      const double wps = rambo_event<NF>(x + 2, rs, a.masses, 1, rambo_volume(NF, rs * rs), p);
+      pass = passes_cuts<NF>(p, a.gluon_mask, a.ptj_min, a.dr_min);
+      w = jac * toy_density(a.beam_kind[0], x[0]) * toy_density(a.beam_kind[1], x[1]) * wps * (PB_GEV2 / (2.0 * rs * rs));
+    }
+  } else {
+    const double wps = rambo_event<NF>(x, a.sqrt_s, a.masses, a.ps_mode, a.w0, p);
+    pass = passes_cuts<NF>(p, a.gluon_mask, a.ptj_min, a.dr_min);
+    w = jac * wps * a.prefactor;
+  }
+  for (int k = 0; k < idx_words; ++k) idx_out[ev * idx_words + k] = packed[k];
+  return pass;
+}
+
 template <class P>
 __global__ void __launch_bounds__(32 * P::N_WARPS, 1) vegas_integrand_kernel(VegasArgs a, double* __restrict__ f_out,
                                                                  unsigned long long* __restrict__ idx_out, int idx_words,
@@ -30,40 +74,11 @@ __global__ void __launch_bounds__(32 * P::N_WARPS, 1) vegas_integrand_kernel(Veg
     const long long ev = (b * NW + warp) * 32 + lane;
     const bool live = ev < a.n_ev;
     {
-      double p[NF][4], y[VEGAS_MAX_DIM], x[VEGAS_MAX_DIM];
-      unsigned long long packed[VEGAS_IDX_WORDS] = {};   // one byte per dimension
+      double p[NF][4];
       bool pass = false;
       double w = 0.0, rs = a.sqrt_s;
       if (live) {
-        philox_fill<VEGAS_MAX_DIM>(a.seed, a.iteration, static_cast<uint64_t>(a.first_event + ev), a.n_dim, y);
-        double jac = 1.0;
-#pragma unroll
-        for (int d = 0; d < VEGAS_MAX_DIM; ++d) {
-          if (d < a.n_dim) {
-            int bin;
-            x[d] = vegas_map_1d(a.edges + d * (a.n_bins + 1), a.n_bins, y[d], jac, bin);
-            packed[d >> 3] |= static_cast<unsigned long long>(bin) << (8 * (d & 7));
-          } else {
-            x[d] = 0.5;
-          }
-        }
-        if (a.ps_mode == 2) {
-          // hadronic mode (DESIGN.md R-N3): x[0], x[1] are the momentum fractions, the rest drives RAMBO on diet at sqrt(s_hat)
-          double msum = 0.0;
-#pragma unroll
-          for (int i = 0; i < NF; ++i) msum += a.masses[i];
-          rs = sqrt(x[0] * x[1]) * a.sqrt_s;
-          if (rs > msum) {
-            const double wps = rambo_event<NF>(x + 2, rs, a.masses, 1, rambo_volume(NF, rs * rs), p);
-            pass = passes_cuts<NF>(p, a.gluon_mask, a.ptj_min, a.dr_min);
-            w = jac * toy_density(a.beam_kind[0], x[0]) * toy_density(a.beam_kind[1], x[1]) * wps * (PB_GEV2 / (2.0 * rs * rs));
-          }
-        } else {
-          const double wps = rambo_event<NF>(x, a.sqrt_s, a.masses, a.ps_mode, a.w0, p);
-          pass = passes_cuts<NF>(p, a.gluon_mask, a.ptj_min, a.dr_min);
-          w = jac * wps * a.prefactor;
-        }
-        for (int k = 0; k < idx_words; ++k) idx_out[ev * idx_words + k] = packed[k];
+        pass = vegas_generate_one<NF>(a, ev, idx_out, idx_words, p, w, rs);
         if (!pass) f_out[ev] = 0.0;
       }
       // compaction: position of this survivor among the CTA's survivors, in event order
