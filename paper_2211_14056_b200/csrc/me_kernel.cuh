@@ -118,7 +118,7 @@ __device__ __forceinline__ double cta_me2(double* smem, double mass, double scal
   __syncthreads();
   double* base = smem + 4 * P::N_EXT;  // event e's scratch = base + e * STRIDE
   static_assert(P::N_HEL_EVAL <= 32, "one helicity combination per lane");
-  static_assert(P::VPI == 4 && P::N_PASS == 1, "the register-resident form is laid out for eight events per CTA");
+  static_assert(P::N_PASS == 1 && P::W_EVENTS * P::VPI == 32, "the register-resident form evaluates the event in one pass");
   constexpr int NFW = JPark<P>::NFW;
   double jr[NFW], ji[NFW];
   const double* my = base + ev_w * STRIDE;
@@ -133,7 +133,7 @@ __device__ __forceinline__ double cta_me2(double* smem, double mass, double scal
   for (int p = 0; p < P::N_STAGES; ++p) {
     const int end = P::stage_end(p);
 #pragma unroll 1
-    for (int i = it + warp; i < end; i += P::N_WARPS) me_run_item<MADME_PREFETCH, 4, P::NSLOT>(c_items[i], c_members, j, sm_e, mass);
+    for (int i = it + warp; i < end; i += P::N_WARPS) me_run_item<MADME_PREFETCH, P::VPI, P::NSLOT>(c_items[i], c_members, j, sm_e, mass);
     it = end;
     __syncthreads();
     const int r = P::stage_dots(p);
