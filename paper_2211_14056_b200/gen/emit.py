@@ -42,6 +42,8 @@ if os.environ.get("MADME_GEN_CHUNK6"):      # g g -> t tbar g g with J in tensor
     GEOMETRY["gg_ttxgg"] = dict(chunk=int(os.environ["MADME_GEN_CHUNK6"]), n_warps=int(os.environ.get("MADME_GEN_WARPS6", "12")))
 if os.environ.get("MADME_GEN_W6"):          # g g -> t tbar g g with fewer events per CTA (two CTAs per SM)
     GEOMETRY["gg_ttxgg"] = dict(w_events=int(os.environ["MADME_GEN_W6"]), n_warps=int(os.environ.get("MADME_GEN_WARPS6", os.environ["MADME_GEN_W6"])))
+for _kv in filter(None, os.environ.get("MADME_GEN_WPROC", "").split(",")):      # "process:events_per_cta", measurement hook
+    GEOMETRY[_kv.split(":")[0]] = dict(w_events=int(_kv.split(":")[1]), n_warps=int(_kv.split(":")[1]))
 FROZEN = (0,)        # set per process by emit_process
 LPT_PER_UNIT = int(os.environ.get("MADME_GEN_LPT_UNIT", "120"))   # 0 / 0: 58.6 M, 60 / 120: 59.2 M, 120 / 240: 59.7 M, 200 / 100: 58.5 M events/s (g g -> t tbar g g)
 LPT_PER_ITEM = int(os.environ.get("MADME_GEN_LPT_ITEM", "240"))
