@@ -139,6 +139,32 @@ int me_amplitude_def_ref(me_handle_ref* h, const double* mom, const int* hel, co
   re_im[0] = a.real(); re_im[1] = a.imag();
   return 0;
 }
+// The tier-0 amplitude with the external wavefunctions STRIPPED: T[i_0][i_1]...[i_{n-1}] = amplitude with leg l carrying the
+// unit wavefunction e_{i_l} (spinor component or Lorentz index), for all-incoming momenta k that need not be physical
+// (negative energies allowed: the amplitude is a rational function of k).  The amplitude is multilinear in the
+// wavefunctions, so spin sums can be done with completeness relations outside — which is what crossing needs
+// (tests/test_oracle_quark_channels.py).  T: [4^n][2], leg 0 slowest.
+int me_open_tensor_ref(me_handle_ref* h, const double* k, const int* col, double* T) {
+  if (!h || h->P.qed || !k || !col || !T) return -1;
+  const int n = h->P.n_ext;
+  Ext E;
+  E.n = n;
+  for (int i = 0; i < n; ++i)
+    for (int mu = 0; mu < 4; ++mu) { E.k[i][mu] = k[4 * i + mu]; E.p[i][mu] = (i < 2 ? 1.0 : -1.0) * k[4 * i + mu]; }
+  long long total = 1;
+  for (int i = 0; i < n; ++i) total *= 4;
+  int hel[NMAX] = {0};
+  for (long long t = 0; t < total; ++t) {
+    long long r = t;
+    for (int i = n - 1; i >= 0; --i) {
+      const int c = int(r % 4); r /= 4;
+      for (int m = 0; m < 4; ++m) { E.eps[i][0][m] = (m == c) ? 1.0 : 0.0; E.sp[i][0][m] = (m == c) ? 1.0 : 0.0; }
+    }
+    const cd a = tier0_amplitude(*h, E, hel, col);
+    T[2 * t] = a.real(); T[2 * t + 1] = a.imag();
+  }
+  return 0;
+}
 int me_flows_ref(me_handle_ref* h, const double* mom, const int* hel, double* J) {
   if (!h || h->P.qed || !h->t1) return -1;
   Ext E; build_ext(*h, mom, E);

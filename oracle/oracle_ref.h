@@ -17,8 +17,9 @@
  * (tier 0 with two fermion lines, tier 1 in the diagram basis) are pinned by the q qbar -> t tbar closed form, the
  * diagram counts behind PAPER.md:57-58 (36 = 16 + 4 x 5, 267 = 123 + 4 x 36), tier 0 <-> tier 1 per amplitude and in
  * the sums, Ward / Lorentz / basis / Bose / charge-conjugation invariance, and by running the diagram basis on the gg
- * channels against the flow basis (tests/test_oracle_quark_channels.py); not pinned: the crossing relation between
- * q qbar -> t tbar g and q g -> t tbar q (it needs wavefunctions at unphysical momenta).  g g -> t tbar g g g: counts,
+ * channels against the flow basis, and by the crossing relation between q qbar -> t tbar g and q g -> t tbar q (the tier-0
+ * amplitude with its wavefunctions stripped, continued to crossed momenta, with completeness relations)
+ * (tests/test_oracle_quark_channels.py).  g g -> t tbar g g g: counts,
  * colour-matrix properties, the flow decomposition against tier-0 amplitudes, Ward / Lorentz / Bose invariance
  * (tests/test_oracle_gg_ttxggg.py); its full tier-0 colour sum is out of reach ("parity pinned per amplitude only").
  * Exceptions:
@@ -83,6 +84,8 @@ int me_colour_matrix_ref(const me_handle_ref* h, double* cf /*[n_flow][n_flow]*/
 int me_flow_perms_ref(const me_handle_ref* h, int* perms /*[n_flow][n_gluon]*/);
 int me_amplitude_def_ref(me_handle_ref* h, const double* mom, const int* hel, const int* col, double* re_im);
 int me_flows_ref(me_handle_ref* h, const double* mom, const int* hel, double* J /*[n_flow][2]*/);
+/* tier-0 amplitude with unit wavefunctions on every leg, all-incoming momenta k[n][4] (unphysical allowed): T[4^n][2] */
+int me_open_tensor_ref(me_handle_ref* h, const double* k, const int* col, double* T);
 int su3_generators_ref(double* T /*[8][3][3][2]*/, double* f /*[8][8][8]*/);
 /* kind: 0 u column, 1 v column, 2 polarisation vector; out = 4 complex (re,im interleaved) */
 int wavefunction_ref(int kind, const double* p, double mass, int s, int basis, double* out);

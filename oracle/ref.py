@@ -49,6 +49,7 @@ def lib():
         _lib.me_flow_perms_ref.argtypes = [C.c_void_p, C.c_void_p]
         _lib.me_amplitude_def_ref.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         _lib.me_flows_ref.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        _lib.me_open_tensor_ref.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         _lib.su3_generators_ref.argtypes = [C.c_void_p, C.c_void_p]
         _lib.wavefunction_ref.argtypes = [C.c_int, C.c_void_p, C.c_double, C.c_int, C.c_int, C.c_void_p]
         _lib.philox_raw_ref.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
@@ -180,6 +181,14 @@ class MatrixElementRef:
         out = np.empty(2)
         assert lib().me_amplitude_def_ref(self._h, _p(m), _p(hel), _p(col), _p(out)) == 0
         return complex(out[0], out[1])
+
+    def open_tensor(self, k, col):
+        """tier-0 amplitude with unit wavefunctions: complex array of shape (4,) * n_external, all-incoming momenta k"""
+        k = _f64(k).reshape(self.n_external, 4)
+        col = np.ascontiguousarray(col, dtype=np.int32)
+        T = np.empty((4 ** self.n_external, 2))
+        assert lib().me_open_tensor_ref(self._h, _p(k), _p(col), _p(T)) == 0
+        return (T[:, 0] + 1j * T[:, 1]).reshape((4,) * self.n_external)
 
     def flows(self, mom, hel):
         m = _f64(mom).reshape(self.n_external, 4)

@@ -181,3 +181,71 @@ def test_diagram_basis_equals_flow_basis(me, proc, cfg, n):
     assert np.max(np.abs(m.eval_diag(mom) / m.eval(mom) - 1)) < 1e-12
     i, d = m.info(), m.info_diag()
     assert (i["n_diag"], i["n_terms"], i["n_diag_4g"]) == (d["n_diag"], d["n_terms"], d["n_diag_4g"])
+
+
+# ---- crossing ----------------------------------------------------------------------------------------------------
+def _gamma():
+    s = [np.array([[0, 1], [1, 0]], complex), np.array([[0, -1j], [1j, 0]]), np.array([[1, 0], [0, -1]], complex)]
+    g = [np.diag([1, 1, -1, -1]).astype(complex)]
+    for k in range(3):
+        m = np.zeros((4, 4), complex)
+        m[:2, 2:] = s[k]
+        m[2:, :2] = -s[k]
+        g.append(m)
+    return g
+
+
+def _spin_sum(kind, k, mass):
+    """sum over the spin states of w_a conj(w_b) for the wavefunction w the oracle puts on a leg of this kind with
+    all-incoming momentum k, written with the completeness relations sum u ubar = pslash + m, sum v vbar = pslash - m,
+    sum eps*_mu eps_nu = -g_mu_nu (one external gluon) — analytic in k, so it continues to crossed (unphysical) momenta."""
+    g = _gamma()
+    sl = lambda p: p[0] * g[0] - p[1] * g[1] - p[2] * g[2] - p[3] * g[3]
+    one = np.eye(4)
+    if kind == "g":
+        return np.diag([-1.0, 1.0, 1.0, 1.0]).astype(complex)
+    if kind == "u":      # incoming fermion, column, p = k
+        return (sl(k) + mass * one) @ g[0]
+    if kind == "vbar":   # incoming antifermion, row, p = k
+        return g[0] @ ((sl(k) - mass * one) @ g[0]).T @ g[0]
+    if kind == "ubar":   # outgoing fermion, row, p = -k
+        return g[0] @ ((sl(-k) + mass * one) @ g[0]).T @ g[0]
+    if kind == "v":      # outgoing antifermion, column, p = -k
+        return (sl(-k) - mass * one) @ g[0]
+    raise ValueError(kind)
+
+
+def _summed_me2_from_open_tensor(m, k, kinds, masses):
+    """sum over colours and spins of |M|^2 from the wavefunction-stripped tier-0 amplitude and completeness relations"""
+    S = [_spin_sum(kd, k[i], masses[i]) for i, kd in enumerate(kinds)]
+    total = 0.0
+    for c0 in range(3):
+        for c1 in range(3):
+            for c2 in range(3):
+                for c3 in range(3):
+                    for a in range(8):
+                        T = m.open_tensor(k, [c0, c1, c2, c3, a])
+                        if not np.any(T):
+                            continue
+                        X = np.einsum("abcde,af,bg,ch,di,ej->fghij", T, S[0], S[1], S[2], S[3], S[4], optimize=True)
+                        total += np.real(np.vdot(T, X))      # sum conj(T)[fghij] X[fghij]
+    return total
+
+
+def test_crossing_qqx_ttxg_to_qg_ttxq(me):
+    """SURVEY §8(f) N1 pin: the colour- and spin-summed |M|^2 of q g -> t tbar q is minus that of q qbar -> t tbar g
+    continued to crossed momenta (antiquark in -> quark out, gluon out -> gluon in; one crossed fermion: the minus sign).
+    The continuation uses the q qbar -> t tbar g amplitude of tier 0 with its wavefunctions stripped (it is a rational
+    function of the momenta) and completeness relations; first checked on physical momenta against the same process."""
+    mt = PARAMS["m_top"]
+    kinds, masses = ["u", "vbar", "ubar", "v", "g"], [0.0, 0.0, mt, mt, 0.0]
+    qqx = me["qqx_ttxg"]
+    p = events("qqx_ttxg", 1)[0]
+    k = np.array([p[0], p[1], -p[2], -p[3], -p[4]])
+    assert abs(_summed_me2_from_open_tensor(qqx, k, kinds, masses) / 36.0 / qqx.eval(p[None])[0] - 1) < 1e-11
+    # q(p0) g(p1) -> t(p2) tbar(p3) q(p4): in the q qbar -> t tbar g amplitude the antiquark leg carries k = -p4 and the
+    # gluon leg k = +p1
+    q = events("qg_ttxq", 2)[1]
+    kx = np.array([q[0], -q[4], -q[2], -q[3], q[1]])
+    crossed = -_summed_me2_from_open_tensor(qqx, kx, kinds, masses) / 96.0
+    assert abs(crossed / me["qg_ttxq"].eval(q[None])[0] - 1) < 1e-10
