@@ -129,6 +129,38 @@ __device__ __forceinline__ double cta_me2(double* smem, double mass, double scal
   // ONE copy of the item interpreter and one of each round's dot products in the instruction stream.  Warp w runs
   // items w, w + N_WARPS, ... of a stage: the generator balanced them by cost (a shared work counter was measured
   // and lost 4 %, profiles/r2_me_eval_summary.md).
+  if constexpr (P::PIPELINED) {
+    // Stage p = the items of one round + the dot products of the round before it (they read the other round region).
+    // Warps 0-3 (one per scheduler) take the dot products first, warps 4-7 the items first, so that a scheduler mostly
+    // holds one warp in a latency-bound item and one in a pipe-bound dot stage.  One copy of each in the instruction stream.
+    static_assert(!SPLIT && P::N_WARPS == W && JPark<P>::ON, "pipelined form: eight warps, J parked in tensor memory");
+    const bool group_a = warp < W / 2;
+#pragma unroll 1
+    for (int p = 0; p < P::N_STAGES; ++p) {
+      const int end = P::stage_end(p), r = P::stage_dots(p);
+#pragma unroll 1
+      for (int ph = 0; ph < 2; ++ph) {
+        const bool want_dots = r >= 0 && ((ph == 0) == group_a);
+        const bool want_items = r < 0 ? ph == 0 : ((ph == 0) != group_a);
+        if (want_dots) {
+          if (r == 0) {
+#pragma unroll
+            for (int f = 0; f < NFW; ++f) { jr[f] = 0.0; ji[f] = 0.0; }
+          } else {
+            JPark<P>::template load<NFW>(tmem, warp, 0, jr, ji);
+          }
+          if (lane < P::N_HEL_EVAL) P::dots(r, my, lane, jr, ji);
+          if (r + 1 < P::N_ROUNDS) JPark<P>::park(tmem, warp, jr, ji);
+        }
+        if (want_items) {
+#pragma unroll 1
+          for (int i = it + warp; i < end; i += P::N_WARPS) me_run_item<MADME_PREFETCH, P::VPI, P::NSLOT>(c_items[i], c_members, j, sm_e, mass);
+        }
+      }
+      it = end;
+      if (p + 1 < P::N_STAGES) __syncthreads();
+    }
+  } else {
 #pragma unroll 1
   for (int p = 0; p < P::N_STAGES; ++p) {
     const int end = P::stage_end(p);
@@ -155,6 +187,7 @@ __device__ __forceinline__ double cta_me2(double* smem, double mass, double scal
       }
       if (r + 1 < P::N_ROUNDS) __syncthreads();   // the next round's items overwrite the round region
     }
+  }
   }
   double v = 0.0;
   if (!SPLIT) {

@@ -44,13 +44,15 @@ if os.environ.get("MADME_GEN_W6"):          # g g -> t tbar g g with fewer event
     GEOMETRY["gg_ttxgg"] = dict(w_events=int(os.environ["MADME_GEN_W6"]), n_warps=int(os.environ.get("MADME_GEN_WARPS6", os.environ["MADME_GEN_W6"])))
 for _kv in filter(None, os.environ.get("MADME_GEN_WPROC", "").split(",")):      # "process:events_per_cta", measurement hook
     GEOMETRY[_kv.split(":")[0]] = dict(w_events=int(_kv.split(":")[1]), n_warps=int(_kv.split(":")[1]))
+if os.environ.get("MADME_GEN_PIPE6"):       # g g -> t tbar g g pipelined over this many double-buffered rounds
+    GEOMETRY["gg_ttxgg"] = dict(pipe_rounds=int(os.environ["MADME_GEN_PIPE6"]))
 FROZEN = (0,)        # set per process by emit_process
 LPT_PER_UNIT = int(os.environ.get("MADME_GEN_LPT_UNIT", "120"))   # 0 / 0: 58.6 M, 60 / 120: 59.2 M, 120 / 240: 59.7 M, 200 / 100: 58.5 M events/s (g g -> t tbar g g)
 LPT_PER_ITEM = int(os.environ.get("MADME_GEN_LPT_ITEM", "240"))
 
 
 def geometry(name):
-    g = dict(w_events=W_EVENTS, frozen=(0,), chunk=0, n_warps=N_WARPS, nslot=int(os.environ.get("MADME_GEN_NSLOT", "4")))
+    g = dict(w_events=W_EVENTS, frozen=(0,), chunk=0, n_warps=N_WARPS, nslot=int(os.environ.get("MADME_GEN_NSLOT", "4")), pipe_rounds=0)
     g.update(GEOMETRY.get(name, {}))
     return g
 
@@ -143,7 +145,7 @@ class Layout:
     open side U | the rest); the operands of a split's dot products live in the round region while that split's
     round is processed."""
 
-    def __init__(self, P, n_rounds, cap=None):
+    def __init__(self, P, n_rounds, cap=None, pipelined=False):
         """cap: the most doubles the operands of one leg split may take in the round region; a larger split is divided
         into PARTS (its open currents U in groups, each with the dot products they enter) that go to different rounds."""
         self.P = P
@@ -235,8 +237,15 @@ class Layout:
         base_end = allocate(self.base, start)
         self.base_doubles = base_end
         tmax = base_end
-        for r in range(len(self.rounds)):
-            tmax = max(tmax, allocate(self.round_objs(r), base_end))
+        if pipelined:
+            # two round regions used in turn: the dot products of round r run while the items of round r + 1 are computed
+            size = max(allocate(self.round_objs(r), base_end) for r in range(len(self.rounds))) - base_end
+            for r in range(len(self.rounds)):
+                allocate(self.round_objs(r), base_end + (r % 2) * size)
+            tmax = base_end + 2 * size
+        else:
+            for r in range(len(self.rounds)):
+                tmax = max(tmax, allocate(self.round_objs(r), base_end))
         self.smem_doubles = tmax
 
     def nv(self, o):
@@ -383,7 +392,8 @@ def _emit_process(name, n_rounds, geo):
     DOTS_C_PER_U = NWARPS > W_EV or bool(CHUNK)
     P = Program(name, frozen=FROZEN)
     assert all(t.op.startswith("DOT") for t in P.terms), "every diagram must be a propagator-cut contraction"
-    L = Layout(P, n_rounds) if n_rounds else pick_rounds(P, smem_budget_doubles(W_EV))
+    PIPE = geo["pipe_rounds"]
+    L = Layout(P, PIPE, pipelined=True) if PIPE else (Layout(P, n_rounds) if n_rounds else pick_rounds(P, smem_budget_doubles(W_EV)))
     assert 4 * P.n + L.smem_doubles <= smem_budget_doubles(W_EV), "the event does not fit the CTA's shared memory"
     n = P.n
     nf = len(P.flow_perms)
@@ -521,7 +531,10 @@ def _emit_process(name, n_rounds, geo):
         tasks = []
         for key in sorted(cells):
             tasks += L.make_tasks(cells[key])
-        add_stage(tasks, r)
+        # pipelined: the stage computes the items of round r and the dot products of round r - 1
+        add_stage(tasks, r - 1 if PIPE else r)
+    if PIPE:
+        add_stage([], len(L.rounds) - 1)
 
     w("// GENERATED by paper_2211_14056_b200/gen/emit.py — do not edit; regenerate with")
     w("//   python -m paper_2211_14056_b200.gen.emit")
@@ -548,6 +561,9 @@ def _emit_process(name, n_rounds, geo):
     w("  static constexpr int W_EVENTS = %d, VPI = %d, N_PASS = %d, CHUNK = %d, N_CHUNK = %d;"
       % (W_EV, VPI, n_pass, CHUNK, (nf + CHUNK - 1) // CHUNK if CHUNK else 1))
     w("  static constexpr bool CHUNKED = %s;" % ("true" if CHUNK else "false"))
+    w("  // PIPELINED: stage p computes the items of one round while the dot products of the round before it are taken (two")
+    w("  // round regions in turn); half of the warps take the dot products first, half the items")
+    w("  static constexpr bool PIPELINED = %s;" % ("true" if PIPE else "false"))
     w("  static constexpr int NSLOT = %d;  // accumulators (colour-ordered currents) per item" % NSLOT)
     w("  static constexpr unsigned FROZEN_MASK = %d;" % sum(1 << l for l in FROZEN))
     w("  // helicity of every leg (bit l) for lane index h of pass p; leg 0 at +1")
