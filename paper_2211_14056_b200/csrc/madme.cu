@@ -554,7 +554,9 @@ int vegas_generate(me_handle* h, const vegas_grid* g, double sqrt_s, const long 
   switch (h->n_ext - 2) {
     case 2: vegas_generate_kernel<2><<<B, T, 0, s>>>(a, event_ids, n, momenta, weights); break;
     case 3: vegas_generate_kernel<3><<<B, T, 0, s>>>(a, event_ids, n, momenta, weights); break;
-    default: vegas_generate_kernel<4><<<B, T, 0, s>>>(a, event_ids, n, momenta, weights); break;
+    case 4: vegas_generate_kernel<4><<<B, T, 0, s>>>(a, event_ids, n, momenta, weights); break;
+    case 5: vegas_generate_kernel<5><<<B, T, 0, s>>>(a, event_ids, n, momenta, weights); break;
+    default: return fail(ME_EINVAL, "vegas_generate: 2 to 5 final-state particles%s%s");
   }
   CU(cudaGetLastError());
   return ME_OK;

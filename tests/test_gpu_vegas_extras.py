@@ -92,7 +92,8 @@ def test_unweight_matches_oracle_bit_exact():
     assert float(api.vegas_max_weight(torch.zeros(0, dtype=torch.float64, device="cuda"))[0]) == 0.0
 
 
-@pytest.mark.parametrize("cfg,ps_mode,n_dim,sqrt_s", [("config4", 1, 8, 1000.0), ("config3", 0, 16, 1000.0), ("config4_hadronic", 2, 10, 13000.0)])
+@pytest.mark.parametrize("cfg,ps_mode,n_dim,sqrt_s", [("config4", 1, 8, 1000.0), ("config3", 0, 16, 1000.0), ("config4_hadronic", 2, 10, 13000.0),
+                                                      ("gg_ttxggg", 1, 11, 1000.0), ("qg_ttxqg", 2, 10, 13000.0)])
 def test_generate_matches_oracle(cfg, ps_mode, n_dim, sqrt_s):
     h = api.me_init("gg_ttxgg", PARAMS)
     edges = random_grid(n_dim, 21)
@@ -112,19 +113,20 @@ def test_generate_matches_oracle(cfg, ps_mode, n_dim, sqrt_s):
     assert np.max(np.abs(w.cpu().numpy()[nz] / w_o[nz] - 1)) < 1e-10
 
 
-def test_unweighted_events_end_to_end():
+@pytest.mark.parametrize("cfg,D,n", [("config4", 8, 1 << 17), ("qg_ttxqg", 8, 1 << 17), ("gg_ttxggg", 11, 1 << 13)])
+def test_unweighted_events_end_to_end(cfg, D, n):
     """integrand -> max weight -> hit-or-miss -> kinematics of the kept events: for every kept event the regenerated
     momenta pass the cuts and weight x |M|^2 reproduces its integrand value; the kept fraction is <f>/w_max within
-    its binomial error; the oracle keeps the same events when given the GPU's weights."""
-    w = BY_NAME["config4"]
+    its binomial error; the oracle keeps the same events when given the GPU's weights.  Also for a quark-initiated channel
+    (the final light quark is a jet) and for g g -> t tbar g g g."""
+    w = BY_NAME[cfg]
     h = api.me_init(w.process, PARAMS)
-    g = api.VegasGrid(8, 50, 1.5, w.seed, 1)
-    n = 1 << 17
+    g = api.VegasGrid(D, 50, 1.5, w.seed, 1)
     api.vegas_iterate(h, g, w.sqrt_s, n)                       # one adaptation step, then unweight iteration 1
     _, f = api.vegas_integrand(h, g, w.sqrt_s, 0, n, want_f=True)
     w_max = float(api.vegas_max_weight(f)[0])
     ids, n_over = api.vegas_unweight(h, f, w_max, w.seed, g.iteration, 0)
-    assert n_over == 0 and len(ids) > 100
+    assert n_over == 0 and len(ids) > (100 if n > 10000 else 5)
     fh = f.cpu().numpy()
     want, _ = ref.vegas_unweight(fh, w_max, w.seed, g.iteration, 0)
     assert np.array_equal(ids.cpu().numpy(), want)
