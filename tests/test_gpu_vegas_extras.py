@@ -95,7 +95,8 @@ def test_unweight_matches_oracle_bit_exact():
 @pytest.mark.parametrize("cfg,ps_mode,n_dim,sqrt_s", [("config4", 1, 8, 1000.0), ("config3", 0, 16, 1000.0), ("config4_hadronic", 2, 10, 13000.0),
                                                       ("gg_ttxggg", 1, 11, 1000.0), ("qg_ttxqg", 2, 10, 13000.0)])
 def test_generate_matches_oracle(cfg, ps_mode, n_dim, sqrt_s):
-    h = api.me_init("gg_ttxgg", PARAMS)
+    proc = BY_NAME[cfg].process
+    h = api.me_init(proc, PARAMS)
     edges = random_grid(n_dim, 21)
     g = api.VegasGrid(n_dim, 50, 1.5, 4, ps_mode, edges=dev(edges))
     g.iteration = 1
@@ -105,7 +106,7 @@ def test_generate_matches_oracle(cfg, ps_mode, n_dim, sqrt_s):
     go = ref.GridRef(n_dim, 50, 1.5, seed=4, ps_mode=ps_mode)
     go.edges[:] = edges
     go.c.iteration = 1
-    mom_o, w_o = ref.MatrixElementRef("gg_ttxgg").vegas_generate(go, sqrt_s, ids)
+    mom_o, w_o = ref.MatrixElementRef(proc).vegas_generate(go, sqrt_s, ids)
     scale = np.maximum(mom_o[:, 0, 0] * 2, 1.0)[:, None, None]
     assert np.max(np.abs(mom.cpu().numpy() - mom_o) / scale) < 1e-11
     nz = w_o != 0
