@@ -125,3 +125,22 @@ def test_cuts_apply_to_the_final_light_quark():
     want = ref.cuts(mom, w.is_gluon, PARAMS["ptj_min"], PARAMS["dr_min"])
     got = api.apply_cuts(dev(mom), w.is_gluon, PARAMS["ptj_min"], PARAMS["dr_min"]).cpu().numpy()
     assert np.array_equal(got, want)
+
+
+def test_edge_kinematics(handles):
+    """q qbar -> t tbar with the tops exactly along the beam axis (both orientations) and 1e-9 off it: the massless beam
+    spinors and the massive top spinors in their degenerate branches; closed form as the second witness."""
+    m, e = PARAMS["m_top"], 500.0
+    pz = np.sqrt(e * e - m * m)
+    mom = np.array([[[e, 0, 0, e], [e, 0, 0, -e], [e, 0, 0, -pz], [e, 0, 0, pz]],
+                    [[e, 0, 0, e], [e, 0, 0, -e], [e, 0, 0, pz], [e, 0, 0, -pz]],
+                    [[e, 0, 0, e], [e, 0, 0, -e], [e, pz * 1e-9, 0, -pz * np.sqrt(1 - 1e-18)], [e, -pz * 1e-9, 0, pz * np.sqrt(1 - 1e-18)]]])
+    got = api.me_eval(handles["qqx_ttx"], dev(mom)).cpu().numpy()
+    want = ref.MatrixElementRef("qqx_ttx").eval(mom)
+    assert np.max(np.abs(got / want - 1)) < 1e-9
+    s = 4 * e * e
+    t = np.array([m * m - 2 * e * (e + pz), m * m - 2 * e * (e - pz), m * m - 2 * e * (e + pz)])   # (p_q - p_t)^2
+    u = 2 * m * m - s - t
+    closed = (4 * np.pi * PARAMS["alpha_s"]) ** 2 * (4.0 / 9) * (((m * m - t) / s) ** 2 + ((m * m - u) / s) ** 2 + 2 * m * m / s)
+    assert np.max(np.abs(got / closed - 1)) < 1e-9
+    assert api.me_eval(handles["qg_ttxqg"], torch.empty((0, 6, 4), dtype=torch.float64, device="cuda")).shape == (0,)
