@@ -118,7 +118,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--events", type=int, default=0, help="events per step per GPU (default: the workload's n_events)")
     ap.add_argument("--workload", default="config3", choices=["config3", "config4", "config4_hadronic", "config2", "config1", "qqx_ttx", "qqx_ttxg", "qg_ttxq",
-                                                           "qqx_ttxgg", "qg_ttxqg", "gg_ttxggg"])
+                                                           "qqx_ttxgg", "qg_ttxqg", "qxg_ttxqxg", "gg_ttxggg"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-vegas-leg", action="store_true", help="skip the config-4 Vegas integration reported beside config 3")

@@ -69,7 +69,8 @@ typedef struct {
  * process: "epem_mupmum" (e+ e- -> mu- mu+), "gg_ttx", "gg_ttxg", "gg_ttxgg" (BASELINE.json:configs[0-3]), and the
  * quark-initiated channels of the paper's hadronic processes (Table 1), legs in the
  * order of the name: "qqx_ttx", "qqx_ttxg", "qqx_ttxgg" (q qbar -> t tbar + 0, 1, 2 gluons) and "qg_ttxq", "qg_ttxqg"
- * (q g -> t tbar q + 0, 1 gluons); q is one massless flavour; and "gg_ttxggg" (g g -> t tbar g g g, SURVEY.md 8(f) N2:
+ * (q g -> t tbar q + 0, 1 gluons) with their charge conjugates "qxg_ttxqx", "qxg_ttxqxg" (qbar g -> t tbar qbar + 0, 1
+ * gluons); q is one massless flavour; and "gg_ttxggg" (g g -> t tbar g g g, SURVEY.md 8(f) N2:
  * 1 240 diagrams, 120 colour flows, evaluated in two passes with the colour-flow vector in tensor memory).
  * Allocates the handle and the fixed-size device scratch of the Vegas path (reduction partials, the survivor staging
  * of the fused integrand: about 25 MB, independent of the event count). */

@@ -26,7 +26,9 @@ static double me2_tier1(const me_handle_ref& h, const double* mom) {
   return h.t1 ? tier1_me2(h, mom) : tier1g_me2(h, *h.t1g, mom);
 }
 // the final-state partons the jet cuts apply to: gluons, and the massless final quark of q g -> t tbar q (g)
-static bool is_jet(const Process& P, int leg) { return P.kind[leg] == G_OUT || (P.kind[leg] == Q_OUT && P.mass[leg] == 0.0); }
+static bool is_jet(const Process& P, int leg) {
+  return P.kind[leg] == G_OUT || ((P.kind[leg] == Q_OUT || P.kind[leg] == QB_OUT) && P.mass[leg] == 0.0);
+}
 
 extern "C" {
 

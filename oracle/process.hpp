@@ -9,6 +9,7 @@
 //   gg -> t tbar (g)(g)(g):  g g | t tbar g g g
 //   q qbar -> t tbar (g)(g): q qbar | t tbar g g       (q: one massless flavour, different from t)
 //   q g -> t tbar q (g)    : q g | t tbar q g
+//   qbar g -> t tbar qbar (g): qbar g | t tbar qbar g    (the charge conjugates of the line above)
 //   e+ e- -> mu+ mu-      :  e- e+ | mu- mu+
 #pragma once
 #include <cstring>
@@ -84,11 +85,14 @@ inline bool make_process(const char* name, const me_params_ref& par, Process& P)
     return true;
   }
   extra_q = -1;
+  bool anti = false;
   if (!std::strcmp(name, "qg_ttxq")) extra_q = 0;
   else if (!std::strcmp(name, "qg_ttxqg")) extra_q = 1;
+  else if (!std::strcmp(name, "qxg_ttxqx")) { extra_q = 0; anti = true; }
+  else if (!std::strcmp(name, "qxg_ttxqxg")) { extra_q = 1; anti = true; }
   if (extra_q >= 0) {
     P.n_ext = 5 + extra_q;
-    P.kind = {F_IN, G_IN, Q_OUT, QB_OUT, Q_OUT};
+    P.kind = {anti ? FB_IN : F_IN, G_IN, Q_OUT, QB_OUT, anti ? QB_OUT : Q_OUT};
     P.mass = {0, 0, mt, mt, 0};
     P.line = {1, -1, 0, 0, 1};
     for (int i = 0; i < extra_q; ++i) { P.kind.push_back(G_OUT); P.mass.push_back(0); P.line.push_back(-1); }

@@ -23,7 +23,7 @@ def _sources():
     return out
 
 
-PROCESSES = ["epem_mupmum", "gg_ttx", "gg_ttxg", "gg_ttxgg", "gg_ttxggg", "qqx_ttx", "qqx_ttxg", "qg_ttxq", "qqx_ttxgg", "qg_ttxqg"]
+PROCESSES = ["epem_mupmum", "gg_ttx", "gg_ttxg", "gg_ttxgg", "gg_ttxggg", "qqx_ttx", "qqx_ttxg", "qg_ttxq", "qqx_ttxgg", "qg_ttxqg", "qxg_ttxqx", "qxg_ttxqxg"]
 
 
 def _compile(job):

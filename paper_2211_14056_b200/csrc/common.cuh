@@ -66,7 +66,7 @@ struct ProcOps {
 #define MADME_DECLARE_OPS(P) const ProcOps* ops_##P##_eval(); const ProcOps* ops_##P##_vegas();
 // every process of gen/diagrams.py::PROCESSES (build.py compiles proc_eval.cu / proc_vegas.cu once for each)
 #define MADME_FOR_EACH_PROCESS(X) \
-  X(epem_mupmum) X(gg_ttx) X(gg_ttxg) X(gg_ttxgg) X(gg_ttxggg) X(qqx_ttx) X(qqx_ttxg) X(qg_ttxq) X(qqx_ttxgg) X(qg_ttxqg)
+  X(epem_mupmum) X(gg_ttx) X(gg_ttxg) X(gg_ttxgg) X(gg_ttxggg) X(qqx_ttx) X(qqx_ttxg) X(qg_ttxq) X(qqx_ttxgg) X(qg_ttxqg) X(qxg_ttxqx) X(qxg_ttxqxg)
 MADME_FOR_EACH_PROCESS(MADME_DECLARE_OPS)
 
 }  // namespace madme

@@ -67,6 +67,11 @@ PROCESSES["qqx_ttxg"] = (_QQX + [_G_OUT], "gs", 4 * 9)
 PROCESSES["qg_ttxq"] = (_QG, "gs", 4 * 24)
 PROCESSES["qqx_ttxgg"] = (_QQX + [_G_OUT, _G_OUT], "gs", 4 * 9 * 2)
 PROCESSES["qg_ttxqg"] = (_QG + [_G_OUT], "gs", 4 * 24)
+# the charge conjugates qbar g -> t tbar qbar (g): an incoming and an outgoing ANTIquark of the light flavour
+_QXG = [Leg(LEG_FB_IN, "q", False), Leg(LEG_V_IN, "g", False), Leg(LEG_F_OUT, "t", True), Leg(LEG_FB_OUT, "t", True),
+        Leg(LEG_FB_OUT, "q", False)]
+PROCESSES["qxg_ttxqx"] = (_QXG, "gs", 4 * 24)
+PROCESSES["qxg_ttxqxg"] = (_QXG + [_G_OUT], "gs", 4 * 24)
 # Processes whose diagrams are ENUMERATED only (Program(name, count_only=True)): none at present.
 COUNT_ONLY = {}
 # g g -> t tbar g g g (1 240 diagrams, 120 colour flows; the gap to the

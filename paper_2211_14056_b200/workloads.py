@@ -34,6 +34,9 @@ WORKLOADS = [
     Workload("qg_ttxq", "qg_ttxq", 1000.0, (M_TOP, M_TOP, 0.0), (0, 0, 1), 13, 1 << 20, 0, 12, True),
     Workload("qqx_ttxgg", "qqx_ttxgg", 1000.0, (M_TOP, M_TOP, 0.0, 0.0), (0, 0, 1, 1), 14, 1 << 22, 0, 16, True),
     Workload("qg_ttxqg", "qg_ttxqg", 1000.0, (M_TOP, M_TOP, 0.0, 0.0), (0, 0, 1, 1), 15, 1 << 22, 0, 16, True),
+    # the antiquark-initiated mirror of q g -> t tbar q g (the other reading of the "4 x 36" of PAPER.md:58: q qbar, q g, qbar g)
+    Workload("qxg_ttxqxg", "qxg_ttxqxg", 1000.0, (M_TOP, M_TOP, 0.0, 0.0), (0, 0, 1, 1), 16, 1 << 22, 0, 16, True),
+    Workload("qxg_ttxqx", "qxg_ttxqx", 1000.0, (M_TOP, M_TOP, 0.0), (0, 0, 1), 17, 1 << 20, 0, 12, True),
     # g g -> t tbar g g g (2 -> 5; 1 240 diagrams, 120 colour flows) — the paper's point is that the
     # gap to the tensorised generator widens with the diagram count; events shaped like config 3
     Workload("gg_ttxggg", "gg_ttxggg", 1000.0, (M_TOP, M_TOP, 0.0, 0.0, 0.0), (0, 0, 1, 1, 1), 21, 1 << 20, 0, 20, True),

@@ -16,6 +16,8 @@
 #include "../../paper_2211_14056_b200/csrc/generated/qg_ttxq.inc"
 #include "../../paper_2211_14056_b200/csrc/generated/qqx_ttxgg.inc"
 #include "../../paper_2211_14056_b200/csrc/generated/qg_ttxqg.inc"
+#include "../../paper_2211_14056_b200/csrc/generated/qxg_ttxqx.inc"
+#include "../../paper_2211_14056_b200/csrc/generated/qxg_ttxqxg.inc"
 
 using namespace madme;
 
@@ -29,7 +31,7 @@ template <class P> struct Tables;
     static const int* massive() { static const int t[] = U##_LEG_MASSIVE; return t; }   \
     static const int* ext_off() { static const int t[] = U##_EXT_OFF; return t; }       \
   };
-#define FOR_EACH_PROCESS(X) X(epem_mupmum) X(gg_ttx) X(gg_ttxg) X(gg_ttxgg) X(gg_ttxggg) X(qqx_ttx) X(qqx_ttxg) X(qg_ttxq) X(qqx_ttxgg) X(qg_ttxqg)
+#define FOR_EACH_PROCESS(X) X(epem_mupmum) X(gg_ttx) X(gg_ttxg) X(gg_ttxgg) X(gg_ttxggg) X(qqx_ttx) X(qqx_ttxg) X(qg_ttxq) X(qqx_ttxgg) X(qg_ttxqg) X(qxg_ttxqx) X(qxg_ttxqxg)
 FOR_EACH_PROCESS(DEF_TABLES)
 
 // items [begin, end) of one stage for ONE event: the device runs them with lanes = (local variant j, event)

@@ -93,7 +93,8 @@ def test_generator_colour_matrix_golden():
 
 @pytest.mark.parametrize("split", [0, 1])
 @pytest.mark.parametrize("cfg,n", [("config0", 64), ("config1", 64), ("config2", 32), ("config3", 12), ("qqx_ttx", 64),
-                                   ("qqx_ttxg", 32), ("qg_ttxq", 32), ("qqx_ttxgg", 16), ("qg_ttxqg", 16)])
+                                   ("qqx_ttxg", 32), ("qg_ttxq", 32), ("qqx_ttxgg", 16), ("qg_ttxqg", 16), ("qxg_ttxqx", 32),
+                                   ("qxg_ttxqxg", 16)])
 def test_generated_program_matches_oracle(host, cfg, n, split):
     """split = 1: the form with two warps per event, each holding half of the colour flows (me_kernel.cuh, SPLIT_J)."""
     w = BY_NAME[cfg]

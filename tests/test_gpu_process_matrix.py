@@ -10,7 +10,7 @@ from paper_2211_14056_b200 import api
 from paper_2211_14056_b200.workloads import BY_NAME, PARAMS, VEGAS_ALPHA, VEGAS_BINS
 
 pytestmark = pytest.mark.gpu
-QCD = ["gg_ttx", "gg_ttxg", "gg_ttxgg", "gg_ttxggg", "qqx_ttx", "qqx_ttxg", "qqx_ttxgg", "qg_ttxq", "qg_ttxqg"]
+QCD = ["gg_ttx", "gg_ttxg", "gg_ttxgg", "gg_ttxggg", "qqx_ttx", "qqx_ttxg", "qqx_ttxgg", "qg_ttxq", "qg_ttxqg", "qxg_ttxqx", "qxg_ttxqxg"]
 WL = {"gg_ttx": "config1", "gg_ttxg": "config2", "gg_ttxgg": "config3"}
 
 

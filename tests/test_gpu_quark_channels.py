@@ -12,7 +12,7 @@ from tests.helpers import mdot, momentum_violation, random_lorentz, transform
 
 pytestmark = pytest.mark.gpu
 ME_RTOL = 1e-10
-CHANNELS = ["qqx_ttx", "qqx_ttxg", "qg_ttxq", "qqx_ttxgg", "qg_ttxqg"]
+CHANNELS = ["qqx_ttx", "qqx_ttxg", "qg_ttxq", "qqx_ttxgg", "qg_ttxqg", "qxg_ttxqx", "qxg_ttxqxg"]
 
 
 def dev(a):
@@ -31,7 +31,7 @@ def handles():
 
 
 @pytest.mark.parametrize("proc,n", [("qqx_ttx", 20000 + 13), ("qqx_ttxg", 6000 + 5), ("qg_ttxq", 6000 + 5), ("qqx_ttxgg", 3000 + 7),
-                                    ("qg_ttxqg", 3000 + 7)])
+                                    ("qg_ttxqg", 3000 + 7), ("qxg_ttxqx", 3000 + 5), ("qxg_ttxqxg", 3000 + 7)])
 def test_me_eval_matches_oracle(handles, proc, n):
     """Element by element; sizes span many CTAs and a ragged tail."""
     mom = oracle_events(proc, n)

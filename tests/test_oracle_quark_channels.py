@@ -183,6 +183,20 @@ def test_diagram_basis_equals_flow_basis(me, proc, cfg, n):
     assert (i["n_diag"], i["n_terms"], i["n_diag_4g"]) == (d["n_diag"], d["n_terms"], d["n_diag_4g"])
 
 
+def test_antiquark_initiated_mirror_channels():
+    """qbar g -> t tbar qbar (g): 5 / 36 diagrams like q g -> t tbar q (g); tier 0 == tier 1; by charge conjugation the
+    summed |M|^2 equals that of the quark-initiated channel with the t and tbar momenta exchanged."""
+    for a, b, nd in (("qxg_ttxqx", "qg_ttxq", 5), ("qxg_ttxqxg", "qg_ttxqg", 36)):
+        ma, mb = ref.MatrixElementRef(a), ref.MatrixElementRef(b)
+        assert ma.info()["n_diag"] == nd
+        mom = events(a, 6)
+        cc = mom.copy()
+        cc[:, [2, 3]] = cc[:, [3, 2]]
+        assert np.max(np.abs(ma.eval(mom) / mb.eval(cc) - 1)) < 1e-12
+        k = 2 if nd == 5 else 1
+        assert np.max(np.abs(ma.eval_def(mom[:k]) / ma.eval(mom[:k]) - 1)) < 1e-12
+
+
 # ---- crossing ----------------------------------------------------------------------------------------------------
 def _gamma():
     s = [np.array([[0, 1], [1, 0]], complex), np.array([[0, -1j], [1j, 0]]), np.array([[1, 0], [0, -1]], complex)]
