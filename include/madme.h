@@ -154,6 +154,19 @@ int vegas_finish(const double* sums, long long n_total, vegas_result* result, vo
 int vegas_max_weight(const double* f, long long n_ev, double* w_max, void* stream);
 int vegas_unweight(me_handle* h, const double* f, long long n_ev, double w_max, uint64_t seed, uint64_t iteration,
                    long long first_event, long long* accepted, long long* counts, void* stream);
+/* vegas_unweight_static — vegas_unweight for callers that cannot allocate (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): the same decision and the same output (accepted, counts as above), no handle,
+ * no me_reserve.  The per-block counters live in a file-scope device array of fixed size instead of a cudaMalloc'ed
+ * buffer: the call allocates and frees nothing and synchronises nothing.  Limits: n_ev <= VEGAS_UNWEIGHT_STATIC_MAX_EVENTS
+ * per call (more: ME_EINVAL); every GPU that loads the library holds the array (128 KB) until exit; all calls on a device
+ * share it, so calls that OVERLAP on the GPU (two streams, a graph replayed beside another call) race: one at a time
+ * per device.  Runs on the CURRENT device.  vegas_unweight_static_init looks the array's device address up for the
+ * current device (cudaGetSymbolAddress, once per device); the first vegas_unweight_static on a device does it itself,
+ * so call the init beforehand where even that look-up is unwelcome (before a capture). */
+#define VEGAS_UNWEIGHT_STATIC_MAX_EVENTS 4194304
+int vegas_unweight_static_init(void);
+int vegas_unweight_static(const double* f, long long n_ev, double w_max, uint64_t seed, uint64_t iteration,
+                          long long first_event, long long* accepted, long long* counts, void* stream);
 /* vegas_generate — the kinematics of LISTED events of iteration g->iteration on grid g (the grid the weights were
  * computed with, i.e. before its refinement): Philox -> Vegas map -> RAMBO for event_ids dev int64 [n].
  * momenta: dev [n][n_ext][4] (partonic centre-of-mass frame); weights: dev [n] = jac W_ps C/(2 s_hat) (times the

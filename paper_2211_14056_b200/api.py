@@ -42,7 +42,7 @@ class VegasResultC(C.Structure):
 SYMBOLS = ["me_init", "me_free", "me_reserve", "me_n_external", "me_n_final", "me_info", "me_flops_per_event", "me_eval",
            "me_eval_helicities", "philox_uniform", "rambo_generate", "apply_cuts", "vegas_map", "vegas_refine",
            "vegas_integrand", "vegas_iterate", "vegas_combine", "vegas_finish", "vegas_max_weight", "vegas_unweight",
-           "vegas_generate", "fp64_peak_probe", "me_last_error"]
+           "vegas_unweight_static", "vegas_unweight_static_init", "vegas_generate", "fp64_peak_probe", "me_last_error"]
 
 
 def lib():
@@ -78,6 +78,8 @@ def lib():
     L.vegas_finish.argtypes = [vp, ll, C.POINTER(VegasResultC), vp]
     L.vegas_max_weight.argtypes = [vp, ll, vp, vp]
     L.vegas_unweight.argtypes = [vp, vp, ll, dbl, u64, u64, ll, vp, vp, vp]
+    L.vegas_unweight_static.argtypes = [vp, ll, dbl, u64, u64, ll, vp, vp, vp]
+    L.vegas_unweight_static_init.argtypes = []
     L.vegas_generate.argtypes = [vp, C.POINTER(VegasGridC), dbl, vp, ll, vp, vp, vp]
     L.fp64_peak_probe.argtypes = [ll, vp, C.POINTER(dbl), vp]
     L.me_last_error.restype = C.c_char_p
@@ -287,6 +289,33 @@ def vegas_unweight(h, f, w_max, seed, iteration, first_event=0, stream=None):
     _check(lib().vegas_unweight(h.ptr, _dev(f, torch.float64, "f"), n_ev, float(w_max), seed, iteration, first_event,
                                 _dev(accepted, torch.int64, "accepted"), _dev(counts, torch.int64, "counts"), _stream(stream)))
     c = counts.tolist()      # marshalling: the two counters come back to size the view
+    return accepted[:c[0]], c[1]
+
+
+UNWEIGHT_STATIC_MAX_EVENTS = 4194304
+
+
+def vegas_unweight_static_init():
+    """Set-up of vegas_unweight_static on the current device (looks up the device address of its static scratch)."""
+    _check(lib().vegas_unweight_static_init())
+
+
+def vegas_unweight_static(f, w_max, seed, iteration, first_event=0, accepted=None, counts=None, stream=None):
+    """vegas_unweight without a handle and without any allocation inside the library (its scratch is a fixed device
+    array): at most UNWEIGHT_STATIC_MAX_EVENTS events per call, one call at a time per device.  Pass `accepted` (cuda
+    int64 [n_ev]) and `counts` (cuda int64 [2]) to keep the binding from allocating too; then the raw tensors are returned
+    and nothing is read back.  Otherwise returns (accepted view of length n_kept, n_overweight) like vegas_unweight."""
+    n_ev = f.shape[0]
+    raw = accepted is not None and counts is not None
+    if accepted is None:
+        accepted = torch.empty(n_ev, dtype=torch.int64, device=f.device)
+    if counts is None:
+        counts = torch.empty(2, dtype=torch.int64, device=f.device)
+    _check(lib().vegas_unweight_static(_dev(f, torch.float64, "f"), n_ev, float(w_max), seed, iteration, first_event,
+                                       _dev(accepted, torch.int64, "accepted"), _dev(counts, torch.int64, "counts"), _stream(stream)))
+    if raw:
+        return accepted, counts
+    c = counts.tolist()
     return accepted[:c[0]], c[1]
 
 

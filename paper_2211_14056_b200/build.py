@@ -44,7 +44,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
-    jobs = [("madme.cu", os.path.join(objdir, "madme.o"), [])]
+    jobs = [("madme.cu", os.path.join(objdir, "madme.o"), []), ("unweight_static.cu", os.path.join(objdir, "unweight_static.o"), [])]
     for p in reversed(PROCESSES):   # the big ones first
         jobs.append(("proc_eval.cu", os.path.join(objdir, "eval_%s.o" % p), ["-DMADME_PROC=" + p]))
         jobs.append(("proc_vegas.cu", os.path.join(objdir, "vegas_%s.o" % p), ["-DMADME_PROC=" + p]))

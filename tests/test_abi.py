@@ -66,6 +66,8 @@ def test_no_cpu_fallback(lib):
     p = api.MeParams(0.118, 1 / 132.507, 173.0, 0.0, 20.0, 0.4)
     assert lib.me_init(b"gg_ttx", C.byref(p), C.byref(out)) == api.ME_ENODEV
     assert lib.philox_uniform(0, 0, 0, 8, C.c_void_p(16), 4, None) == api.ME_ENODEV
+    assert lib.vegas_unweight_static_init() == api.ME_ENODEV
+    assert lib.vegas_unweight_static(C.c_void_p(16), 4, 1.0, 0, 0, 0, C.c_void_p(16), C.c_void_p(16), None) == api.ME_ENODEV
     with pytest.raises(api.MadmeError):
         api.me_init("gg_ttxgg", dict(alpha_s=0.118, alpha_em=1 / 132.507, m_top=173.0, w_top=0.0, ptj_min=20.0, dr_min=0.4))
 
