@@ -19,7 +19,8 @@
  * the sums, Ward / Lorentz / basis / Bose / charge-conjugation invariance, and by running the diagram basis on the gg
  * channels against the flow basis, and by the crossing relation between q qbar -> t tbar g and q g -> t tbar q (the tier-0
  * amplitude with its wavefunctions stripped, continued to crossed momenta, with completeness relations)
- * (tests/test_oracle_quark_channels.py).  g g -> t tbar g g g: counts,
+ * (tests/test_oracle_quark_channels.py); the antiquark-initiated mirrors qbar g -> t tbar qbar (g) are pinned to the
+ * quark-initiated ones by charge conjugation and by tier 0.  g g -> t tbar g g g: counts,
  * colour-matrix properties, the flow decomposition against tier-0 amplitudes, Ward / Lorentz / Bose invariance
  * (tests/test_oracle_gg_ttxggg.py); its full tier-0 colour sum is out of reach ("parity pinned per amplitude only").
  * Exceptions:
