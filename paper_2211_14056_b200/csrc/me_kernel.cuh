@@ -31,6 +31,10 @@
 #define MADME_PREFETCH 0   // 0: the next member's operands are fetched after the accumulation (58.7 M events/s); 1: one member ahead, copied (56.9 M); 2: between vertex and accumulation (56.8 M)
 #endif
 
+#ifndef MADME_STRIDE8
+#define MADME_STRIDE8 8   // doubles mod 16 between the events of a four-event CTA
+#endif
+
 namespace madme {
 
 #define MADME_CAT2_(a, b) a##b
@@ -52,7 +56,7 @@ __device__ const int d_extoff[] = MADME_TAB(_EXT_OFF);
 template <class P> struct EventSmem {
   static constexpr int RAW = 4 * P::N_EXT + P::SMEM_DOUBLES;
   // eight events: 16 B mod 128 B; four events (eight variants = one line per event and component): half a line
-  static constexpr int DOUBLES = ((RAW + 13) / 16) * 16 + (P::VPI == 8 ? 8 : 2);
+  static constexpr int DOUBLES = ((RAW + 13) / 16) * 16 + (P::VPI == 8 ? MADME_STRIDE8 : 2);
 };
 
 // Events per CTA: P::W_EVENTS (gen/emit.py: the item tables are laid out for it; 8, or 4 for g g -> t tbar g g g).  A CTA

@@ -47,6 +47,7 @@ for _kv in filter(None, os.environ.get("MADME_GEN_WPROC", "").split(",")):      
 if os.environ.get("MADME_GEN_PIPE6"):       # g g -> t tbar g g pipelined over this many double-buffered rounds
     GEOMETRY["gg_ttxgg"] = dict(pipe_rounds=int(os.environ["MADME_GEN_PIPE6"]))
 FROZEN = (0,)        # set per process by emit_process
+SPLIT_THRESHOLD = float(os.environ.get("MADME_GEN_SPLIT_THR", "1.2"))   # split_for_balance: tasks above this x the mean warp load
 LPT_PER_UNIT = int(os.environ.get("MADME_GEN_LPT_UNIT", "120"))   # 0 / 0: 58.6 M, 60 / 120: 59.2 M, 120 / 240: 59.7 M, 200 / 100: 58.5 M events/s (g g -> t tbar g g)
 LPT_PER_ITEM = int(os.environ.get("MADME_GEN_LPT_ITEM", "240"))
 
@@ -434,7 +435,7 @@ def _emit_process(name, n_rounds, geo):
         task_list = list(task_list)
         for _ in range(64):
             mean = sum(L.task_flops(t) * ((L.nv(t.outputs[0]) + VPI - 1) // VPI) for t in task_list) / NWARPS
-            cands = [k for k, t in enumerate(task_list) if len(t.outputs) >= 2 and L.task_flops(t) > 1.2 * mean]
+            cands = [k for k, t in enumerate(task_list) if len(t.outputs) >= 2 and L.task_flops(t) > SPLIT_THRESHOLD * mean]
             if not cands:
                 break
             k = max(cands, key=lambda k: L.task_flops(task_list[k]))
