@@ -31,6 +31,9 @@
 #define MADME_PREFETCH 0   // 0: the next member's operands are fetched after the accumulation (58.7 M events/s); 1: one member ahead, copied (56.9 M); 2: between vertex and accumulation (56.8 M)
 #endif
 
+#ifndef MADME_PREFETCH_MOMENTA
+#define MADME_PREFETCH_MOMENTA 1   // me_eval: the next batch's momenta are fetched (cp.async) while this batch is computed
+#endif
 #ifndef MADME_STRIDE8
 #define MADME_STRIDE8 8   // doubles mod 16 between the events of a four-event CTA
 #endif
@@ -391,10 +394,32 @@ __global__ void __launch_bounds__(32 * P::N_WARPS, 1) me_eval_kernel(const doubl
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t tmem = JPark<P>::ON ? tmem_alloc<JPark<P>::COLS>() : 0u;
   const long long n_batches = (n_ev + W - 1) / W;
+  // (not for the chunked processes: their shared memory is full and a batch takes millions of cycles)
+  constexpr bool PRE = MADME_PREFETCH_MOMENTA && !P::CHUNKED;
+  // The momenta of the NEXT batch travel from HBM into a small staging buffer (cp.async, one double per thread) while this
+  // batch is computed: the DRAM latency at the head of a batch was 2.7 % of the kernel's samples (7 % for the small
+  // processes).  Every thread copies, waits for and reads its own element, so no barrier is involved.
+  __shared__ __align__(16) double next_mom[PRE ? W : 1][PRE ? 4 * P::N_EXT : 2];
+  const bool loader = (P::N_WARPS == W || warp < W) && lane < 4 * P::N_EXT;
+  auto prefetch = [&](long long b) {
+    if (PRE && loader) {
+      const long long ev = min(b * W + (warp & (W - 1)), n_ev - 1);   // events past the end repeat the last one
+      const unsigned dst = static_cast<unsigned>(__cvta_generic_to_shared(&next_mom[warp][lane]));
+      asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" :: "r"(dst), "l"(momenta + ev * (4 * P::N_EXT) + lane) : "memory");
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+  if (PRE && static_cast<long long>(blockIdx.x) < n_batches) prefetch(blockIdx.x);
   for (long long b = blockIdx.x; b < n_batches; b += gridDim.x) {
     // events past the end repeat the last one (computed, not stored)
     const long long ev = min(b * W + (warp & (W - 1)), n_ev - 1);
-    if ((P::N_WARPS == W || warp < W) && lane < 4 * P::N_EXT) smem[warp * STRIDE + lane] = momenta[ev * (4 * P::N_EXT) + lane];
+    if constexpr (PRE) {
+      asm volatile("cp.async.wait_all;" ::: "memory");
+      if (loader) smem[warp * STRIDE + lane] = next_mom[warp][lane];
+      if (b + gridDim.x < n_batches) prefetch(b + gridDim.x);
+    } else {
+      if (loader) smem[warp * STRIDE + lane] = momenta[ev * (4 * P::N_EXT) + lane];
+    }
     __syncthreads();
     const double r = cta_me2<P>(smem, mass, scale, (me2_hel && b * W + (warp & (W - 1)) < n_ev) ? me2_hel + ev * P::N_HEL : nullptr, tmem);
     if ((P::N_WARPS == W || warp < W) && lane == 0 && me2 && b * W + warp < n_ev) me2[ev] = r;
