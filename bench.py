@@ -29,7 +29,7 @@ NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12  # SMs x DFMA lanes/SM x 2 f
 # dram__bytes_read.sum + dram__bytes_write.sum of me_eval_kernel<gg_ttxgg> per event, from the ncu --set full capture
 # of the kernel at HEAD summarised in profiles/r2_me_eval_summary.md (817.7 MB + 37.1 MB for 4 194 304 events;
 # algorithmic: 200 B/event)
-NCU_DRAM_BYTES_PER_EVENT = {"gg_ttxgg": 203.7, "gg_ttxggg": 228.7, "qqx_ttxgg": 201.4}
+NCU_DRAM_BYTES_PER_EVENT = {"gg_ttxgg": 202.7, "gg_ttxggg": 228.7, "qqx_ttxgg": 201.4}
 NCU_SUMMARY = "profiles/r2_me_eval_summary.md, profiles/r2_n1_n2_summary.md"
 
 
